@@ -1,0 +1,123 @@
+"""ctypes face of the CPU oracle (oracle/no_oracle.cpp) -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this module.  The product package (paper_2603_24532_b200) never does.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+import sys
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "no_oracle.cpp")
+_LIB = os.path.join(_HERE, "liboracle.so")
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with g++ (OpenMP over configurations).  Returns the library path."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["g++", "-O2", "-fopenmp", "-fcx-limited-range", "-shared", "-fPIC", "-Wall", "-Wextra",
+               "-o", _LIB, _SRC]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+class _Params(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_double) for n in
+                ("kf_n", "kf_p", "c1", "c3", "c4", "cD", "cE", "gA", "fpi", "mpi", "lambda_chi", "Lambda")] + \
+               [(n, ctypes.c_int) for n in ("n_reg", "n_r", "n_cos", "n_phi")]
+
+
+_DEFAULTS = dict(kf_n=0.0, kf_p=0.0, c1=0.0, c3=0.0, c4=0.0, cD=0.0, cE=0.0, gA=1.27, fpi=92.4,
+                 mpi=138.04, lambda_chi=700.0, Lambda=500.0, n_reg=4, n_r=4, n_cos=4, n_phi=4)
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        dp = ctypes.POINTER(ctypes.c_double)
+        pp = ctypes.POINTER(_Params)
+        lib.oracle_gauss_legendre.argtypes = [ctypes.c_int, ctypes.c_double, ctypes.c_double, dp, dp]
+        lib.oracle_v3n.argtypes = [pp, dp, dp]
+        lib.oracle_av3n.argtypes = [pp, dp, dp, dp]
+        for name in ("oracle_no_level0_ld", "oracle_no_level1_ld", "oracle_no_level1_f64"):
+            getattr(lib, name).argtypes = [pp, dp, ctypes.c_longlong, dp]
+            getattr(lib, name).restype = None
+        lib.oracle_hf3n_bruteforce.argtypes = [pp]
+        lib.oracle_hf3n_bruteforce.restype = ctypes.c_double
+        lib.oracle_num_threads.restype = ctypes.c_int
+        _lib = lib
+    return _lib
+
+
+def _params(kw: dict) -> _Params:
+    d = dict(_DEFAULTS)
+    for k, v in kw.items():
+        if k not in d:
+            raise TypeError(f"unknown oracle parameter {k!r}")
+        d[k] = v
+    return _Params(**d)
+
+
+def _dptr(a: np.ndarray):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def gauss_legendre(n: int, a: float, b: float):
+    x = np.empty(n)
+    w = np.empty(n)
+    _load().oracle_gauss_legendre(n, a, b, _dptr(x), _dptr(w))
+    return x, w
+
+
+def v3n(q, **params) -> np.ndarray:
+    """Bare operator V(q1,q2,q3): complex [64,64]; index = 8*(4 s1+2 s2+s3) + (4 t1+2 t2+t3)."""
+    q = np.ascontiguousarray(q, dtype=np.float64).reshape(3, 3)
+    out = np.empty((64, 64, 2))
+    _load().oracle_v3n(ctypes.byref(_params(params)), _dptr(q), _dptr(out))
+    return out[..., 0] + 1j * out[..., 1]
+
+
+def av3n(kin, kout, **params) -> np.ndarray:
+    """Regulated antisymmetrised F * A_123 V for explicit momenta: complex [64,64]."""
+    kin = np.ascontiguousarray(kin, dtype=np.float64).reshape(3, 3)
+    kout = np.ascontiguousarray(kout, dtype=np.float64).reshape(3, 3)
+    out = np.empty((64, 64, 2))
+    _load().oracle_av3n(ctypes.byref(_params(params)), _dptr(kin), _dptr(kout), _dptr(out))
+    return out[..., 0] + 1j * out[..., 1]
+
+
+def normal_order(cfg, level: int = 1, precision: str = "ld", **params) -> np.ndarray:
+    """M[n_cfg,16,16] complex for configurations cfg[n_cfg,9] = (p, p', P) in fm^-1; output fm^2.
+
+    level 0 = definition (64x64 per node); level 1 = spin and isospin traced separately.
+    precision "ld" = long double arithmetic (parity reference), "f64" = double (level 1 only).
+    """
+    cfg = np.ascontiguousarray(cfg, dtype=np.float64).reshape(-1, 9)
+    n = cfg.shape[0]
+    out = np.empty((n, 16, 16, 2))
+    name = {(0, "ld"): "oracle_no_level0_ld", (1, "ld"): "oracle_no_level1_ld",
+            (1, "f64"): "oracle_no_level1_f64"}[(level, precision)]
+    if n:
+        getattr(_load(), name)(ctypes.byref(_params(params)), _dptr(cfg), n, _dptr(out))
+    return out[..., 0] + 1j * out[..., 1]
+
+
+def hf3n_bruteforce(**params) -> float:
+    """(1/6) sum_{123} <123|F A_123 V|123> on the product grid of every particle (pin P8); fm^-4."""
+    return float(_load().oracle_hf3n_bruteforce(ctypes.byref(_params(params))))
+
+
+def num_threads() -> int:
+    return int(_load().oracle_num_threads())
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv))

@@ -1,0 +1,422 @@
+"""Pins of the CPU oracle (oracle/no_oracle.cpp) against what the paper and the mathematics fix.
+
+None of these tests touches the CUDA path.  Each pin names the passage or the DESIGN.md /
+SURVEY.md section 8(c) item it comes from.  A plausible mistake in the oracle (a dropped term, a
+wrong sign, a transposed index, a wrong permutation convention, a wrong Jacobian or 1/(2 pi)^3)
+fails at least one of them.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+
+HBARC = 197.3269804
+PHYS = dict(c1=-0.81, c3=-3.2, cD=1.0, cE=-0.5, gA=1.27, fpi=92.4, mpi=138.04, lambda_chi=700.0,
+            Lambda=500.0, n_reg=4)
+RNG = np.random.default_rng(20260324)
+
+
+def idx(s1, s2, t1, t2):
+    return 8 * s1 + 4 * s2 + 2 * t1 + t2
+
+
+def p12_matrix():
+    """Exchange of (s1,t1) <-> (s2,t2) on the 16-dim two-body index."""
+    P = np.zeros((16, 16))
+    for s1 in range(2):
+        for s2 in range(2):
+            for t1 in range(2):
+                for t2 in range(2):
+                    P[idx(s2, s1, t2, t1), idx(s1, s2, t1, t2)] = 1.0
+    return P
+
+
+def rand_cfg(n, scale=1.0):
+    return RNG.uniform(-1.0, 1.0, size=(n, 9)) * scale
+
+
+def only(**kw):
+    """Parameter set with every LEC zero except the named ones."""
+    d = dict(PHYS)
+    for k in ("c1", "c3", "cD", "cE"):
+        d[k] = 0.0
+    d["c4"] = 0.0
+    d.update(kw)
+    return d
+
+
+# ----------------------------------------------------------------------------------------------
+# Gauss-Legendre (reading R11): against numpy's library routine, and exactness on monomials.
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n", [1, 2, 3, 7, 16, 32, 40, 48, 64, 128])
+def test_gauss_legendre_matches_library_and_is_exact(n):
+    x, w = O.gauss_legendre(n, -1.0, 1.0)
+    xr, wr = np.polynomial.legendre.leggauss(n)
+    assert np.allclose(x, xr, rtol=0, atol=3e-15)
+    assert np.allclose(w, wr, rtol=1e-10, atol=1e-16)      # numpy's own weights are only ~1e-12 accurate
+    for k in {2 * n - 2, 2 * n - 1, n, min(2, 2 * n - 1)}:   # exact up to degree 2n-1 (numpy reaches ~1e-14)
+        exact = 2.0 / (k + 1) if k % 2 == 0 else 0.0
+        assert abs(np.dot(w, x ** k) - exact) <= 4e-16
+    assert np.all(np.diff(x) > 0)
+    assert np.array_equal(x, -x[::-1]) and np.array_equal(w, w[::-1])   # symmetric pairs enforced
+    a, b = 0.0, 1.7
+    x, w = O.gauss_legendre(n, a, b)
+    for k in range(0, min(2 * n, 12)):
+        exact = (b ** (k + 1) - a ** (k + 1)) / (k + 1)
+        assert abs(np.dot(w, x ** k) - exact) <= 1e-14 * exact
+
+
+# ----------------------------------------------------------------------------------------------
+# Bare operator (reading R1): hand-evaluated matrix elements, Hermiticity, relabelling symmetry.
+# ----------------------------------------------------------------------------------------------
+def test_operator_hand_evaluated_elements():
+    """All spins up, three protons, all transfers along z: every Pauli dot product is a number.
+    t_i.t_j = 1 between protons, (sigma_i.q)(sigma_j.q') = q_z q'_z on |up up up>."""
+    a, b = 0.7, -0.4
+    q = np.array([[0, 0, a], [0, 0, b], [0, 0, -a - b]])
+    m = PHYS["mpi"] / HBARC
+    f = PHYS["fpi"] / HBARC
+    L = PHYS["lambda_chi"] / HBARC
+    qz = q[:, 2]
+    D = qz ** 2 + m ** 2
+    row = 8 * 0 + 0          # spin index 0 = up up up, isospin index 0 = p p p
+    # cE: cE/(2 f^4 L) * sum_{j != k} 1
+    V = O.v3n(q, **only(cE=-0.5))
+    assert V[row, row] == pytest.approx(-0.5 / (2 * f ** 4 * L) * 6, rel=1e-14)
+    # cD: -gA/(8 f^2) cD/(f^2 L) sum_{i != j} q_j^2 / D_j
+    V = O.v3n(q, **only(cD=1.0))
+    want = -PHYS["gA"] / (8 * f ** 2) * 1.0 / (f ** 2 * L) * 2 * np.sum(qz ** 2 / D)
+    assert V[row, row] == pytest.approx(want, rel=1e-14)
+    # c1, c3: 1/2 (gA/2f)^2 sum_{i != j} q_i q_j /(D_i D_j) (-4 c1 m^2/f^2 + 2 c3/f^2 q_i q_j)
+    c1 = -0.81e-3 * HBARC
+    c3 = -3.2e-3 * HBARC
+    V = O.v3n(q, **only(c1=-0.81, c3=-3.2))
+    want = 0.0
+    for i in range(3):
+        for j in range(3):
+            if i != j:
+                want += 0.5 * (PHYS["gA"] / (2 * f)) ** 2 * qz[i] * qz[j] / (D[i] * D[j]) * (
+                    -4 * c1 * m ** 2 / f ** 2 + 2 * c3 / f ** 2 * qz[i] * qz[j])
+    assert V[row, row] == pytest.approx(want, rel=1e-14)
+    # c4: (t_i x t_j).t_k has no diagonal element between isospin product states with all t_z equal
+    V = O.v3n(RNG.normal(size=(3, 3)), **only(c4=5.4))
+    assert abs(V[row, row]) < 1e-18
+    assert np.abs(V).max() > 1e-3
+
+
+def _perm_matrix64(pi):
+    """<b'|Pi_pi|b> = prod_m delta(b'_{pi(m)}, b_m) on spin (x) isospin of three particles."""
+    P8 = np.zeros((8, 8))
+    for b in range(8):
+        bits = [(b >> 2) & 1, (b >> 1) & 1, b & 1]
+        out = [0, 0, 0]
+        for m in range(3):
+            out[pi[m]] = bits[m]
+        P8[4 * out[0] + 2 * out[1] + out[2], b] = 1.0
+    return np.kron(P8, P8)
+
+
+def test_operator_is_hermitian_even_and_symmetric_under_relabelling():
+    kw = dict(PHYS, c4=5.4)
+    q = RNG.normal(size=(3, 3))
+    q[2] = -q[0] - q[1]
+    V = O.v3n(q, **kw)
+    scale = np.abs(V).max()
+    assert np.abs(V - V.conj().T).max() < 1e-15 * scale
+    assert np.abs(V - O.v3n(-q, **kw)).max() < 1e-15 * scale
+    for pi in ([1, 0, 2], [2, 1, 0], [0, 2, 1], [1, 2, 0], [2, 0, 1]):
+        Pm = _perm_matrix64(pi)
+        qp = np.empty_like(q)
+        for m in range(3):
+            qp[pi[m]] = q[m]          # particle m, relabelled pi(m), keeps its momentum transfer
+        assert np.abs(Pm @ V @ Pm.T - O.v3n(qp, **kw)).max() < 2e-15 * scale
+
+
+def test_antisymmetrised_matrix_is_antisymmetric_in_both_indices():
+    """A_123 V A-symmetry at the untraced level, with the regulator on."""
+    kw = dict(PHYS, c4=5.4)
+    kin = RNG.normal(size=(3, 3)) * 0.6
+    kout = RNG.normal(size=(3, 3)) * 0.6
+    kout[2] = kin.sum(axis=0) - kout[0] - kout[1]
+    AV = O.av3n(kin, kout, **kw)
+    scale = np.abs(AV).max()
+    assert scale > 1e-3
+    for pi, sgn in (([1, 0, 2], -1), ([2, 1, 0], -1), ([1, 2, 0], +1)):
+        Pm = _perm_matrix64(pi)
+        ko = np.empty_like(kout)
+        ki = np.empty_like(kin)
+        for m in range(3):
+            ko[pi[m]] = kout[m]
+            ki[pi[m]] = kin[m]
+        # permuting the outgoing labels (momenta with spin-isospin) gives the sign of pi
+        assert np.abs(Pm @ AV - sgn * O.av3n(kin, ko, **kw)).max() < 4e-15 * scale
+        assert np.abs(AV @ Pm.T - sgn * O.av3n(ki, kout, **kw)).max() < 4e-15 * scale
+
+
+# ----------------------------------------------------------------------------------------------
+# P1 / P2: closed forms of the contact term (north_star (c)).
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kf", [0.8, 1.33, 1.7])
+@pytest.mark.parametrize("level", [0, 1])
+def test_P1_cE_closed_form_snm_unregulated(kf, level):
+    kw = only(cE=-0.5, Lambda=-1.0, kf_n=kf, kf_p=kf, n_r=3, n_cos=2, n_phi=2)
+    cfg = rand_cfg(3, 2.0)
+    M = O.normal_order(cfg, level=level, **kw)
+    f = PHYS["fpi"] / HBARC
+    L = PHYS["lambda_chi"] / HBARC
+    pref = -(-0.5) * kf ** 3 / (math.pi ** 2 * f ** 4 * L)
+    want = pref * (np.eye(16) - p12_matrix())
+    for m in M:
+        assert np.abs(m - want).max() < 2e-15 * abs(pref)
+    # scales as kF^3, and the number quoted in SURVEY.md Appendix A for kF = 1.33
+    if kf == 1.33:
+        assert pref == pytest.approx(0.6988301080442392, rel=1e-12)
+
+
+def test_P2_cE_energy_closed_form():
+    kf = 1.33
+    kw = only(cE=-0.5, Lambda=-1.0, kf_n=kf, kf_p=kf, n_r=2, n_cos=2, n_phi=2)
+    M = O.normal_order(rand_cfg(1), **kw)[0]
+    dens = kf ** 3 / (6 * math.pi ** 2)           # per spin-isospin state
+    e_from_m = np.trace(M).real * dens ** 2 / 6
+    rho = 2 * kf ** 3 / (3 * math.pi ** 2)
+    f = PHYS["fpi"] / HBARC
+    L = PHYS["lambda_chi"] / HBARC
+    assert e_from_m == pytest.approx(-(3.0 / 16.0) * (-0.5) * rho ** 3 / (f ** 4 * L), rel=1e-14)
+
+
+# ----------------------------------------------------------------------------------------------
+# P3: cD, cE (and c4) vanish in pure neutron matter (Sec. VI A; reading R17).
+# ----------------------------------------------------------------------------------------------
+NN_BLOCK = [idx(s1, s2, 1, 1) for s1 in range(2) for s2 in range(2)]
+
+
+@pytest.mark.parametrize("which", ["cD", "cE", "c4"])
+def test_P3_pnm_vanishing(which):
+    lec = {"cD": 1.0, "cE": -0.5, "c4": 5.4}[which]
+    kw = only(**{which: lec}, kf_n=1.3, kf_p=0.0, n_r=3, n_cos=3, n_phi=3)
+    cfg = rand_cfg(4, 1.5)
+    M = O.normal_order(cfg, **kw)
+    ref = O.normal_order(cfg, **only(c1=-0.81, c3=-3.2, kf_n=1.3, kf_p=0.0, n_r=3, n_cos=3, n_phi=3))
+    scale = np.abs(ref[:, NN_BLOCK][:, :, NN_BLOCK]).max()
+    assert scale > 1e-3                                       # c1/c3 do NOT vanish
+    assert np.abs(M[:, NN_BLOCK][:, :, NN_BLOCK]).max() < 1e-16 * max(1.0, scale / 1e-2)
+    assert np.abs(M).max() > 1e-3                             # blocks with an external proton do not (R17)
+    # node by node, before the trace: the nnn isospin block of A_123 V vanishes identically
+    kin = RNG.normal(size=(3, 3)) * 0.6
+    kout = RNG.normal(size=(3, 3)) * 0.6
+    kout[2] = kin.sum(axis=0) - kout[0] - kout[1]
+    AV = O.av3n(kin, kout, **only(**{which: lec}))
+    nnn = [8 * s + 7 for s in range(8)]
+    assert np.abs(AV[np.ix_(nnn, nnn)]).max() < 1e-15 * np.abs(AV).max()
+
+
+# ----------------------------------------------------------------------------------------------
+# P4 Hermiticity, P5 antisymmetry, P6 sparsity, P9 isospin symmetry, P10 linearity, P11 levels.
+# ----------------------------------------------------------------------------------------------
+ASYM = dict(PHYS, c4=5.4, kf_n=1.2, kf_p=0.9, n_r=3, n_cos=4, n_phi=3)
+
+
+def _swap(cfg, what):
+    c = cfg.copy()
+    if what == "p<->p'":
+        c[:, 0:3], c[:, 3:6] = cfg[:, 3:6], cfg[:, 0:3]
+    elif what == "-p'":
+        c[:, 3:6] *= -1
+    elif what == "-p":
+        c[:, 0:3] *= -1
+    return c
+
+
+def test_P4_hermiticity():
+    cfg = rand_cfg(4, 1.5)
+    M = O.normal_order(cfg, **ASYM)
+    Mt = O.normal_order(_swap(cfg, "p<->p'"), **ASYM)
+    scale = np.abs(M).max()
+    assert np.abs(M - np.conj(np.swapaxes(Mt, 1, 2))).max() < 4e-16 * scale
+
+
+def test_P5_antisymmetry():
+    cfg = rand_cfg(4, 1.5)
+    P = p12_matrix()
+    M = O.normal_order(cfg, **ASYM)
+    scale = np.abs(M).max()
+    assert np.abs(P @ O.normal_order(_swap(cfg, "-p'"), **ASYM) + M).max() < 4e-16 * scale
+    assert np.abs(O.normal_order(_swap(cfg, "-p"), **ASYM) @ P + M).max() < 4e-16 * scale
+
+
+@pytest.mark.parametrize("level", [0, 1])
+def test_P6_sparsity(level):
+    """Charge conservation: 4^A * C(2A,A) = 96 possible non-zeros for A = 2."""
+    kw = dict(ASYM, n_r=2, n_cos=3, n_phi=2)
+    M = O.normal_order(rand_cfg(2, 1.5), level=level, **kw)
+    allowed = np.zeros((16, 16), bool)
+    for r in range(16):
+        for c in range(16):
+            allowed[r, c] = ((r >> 1) & 1) + (r & 1) == ((c >> 1) & 1) + (c & 1)
+    assert allowed.sum() == 96 == 4 ** 2 * math.comb(4, 2)
+    for m in M:
+        assert np.abs(m[~allowed]).max() < 1e-16 * np.abs(m).max()
+        assert (np.abs(m[allowed]) > 1e-9 * np.abs(m).max()).all()
+
+
+def test_P9_isospin_symmetry_snm_and_its_breaking_in_asymmetric_matter():
+    def blocks(m):
+        B = {}
+        for a, (t1o, t2o) in enumerate(((0, 0), (0, 1), (1, 0), (1, 1))):
+            for b, (t1, t2) in enumerate(((0, 0), (0, 1), (1, 0), (1, 1))):
+                rows = [idx(s1, s2, t1o, t2o) for s1 in range(2) for s2 in range(2)]
+                cols = [idx(s1, s2, t1, t2) for s1 in range(2) for s2 in range(2)]
+                B[a, b] = m[np.ix_(rows, cols)]
+        return B
+    cfg = rand_cfg(2, 1.5)
+    snm = dict(ASYM, kf_n=1.1, kf_p=1.1)
+    for m in O.normal_order(cfg, **snm):
+        B = blocks(m)
+        scale = np.abs(m).max()
+        t1 = (B[1, 1] + B[1, 2] + B[2, 1] + B[2, 2]) / 2
+        assert np.abs(B[0, 0] - B[3, 3]).max() < 4e-16 * scale
+        assert np.abs(B[0, 0] - t1).max() < 4e-16 * scale
+        assert np.abs(B[1, 1] - B[1, 2] + B[2, 1] - B[2, 2]).max() < 4e-16 * scale
+    m = O.normal_order(cfg, **ASYM)[0]
+    B = blocks(m)
+    assert np.abs(B[0, 0] - B[3, 3]).max() > 1e-3 * np.abs(m).max()
+
+
+def test_P10_linearity_in_the_lecs():
+    cfg = rand_cfg(2, 1.5)
+    geo = dict(kf_n=1.2, kf_p=0.9, n_r=3, n_cos=2, n_phi=3)
+    full = O.normal_order(cfg, **dict(PHYS, c4=5.4, **geo))
+    each = [O.normal_order(cfg, **only(**{k: v}, **geo))
+            for k, v in (("c1", -0.81), ("c3", -3.2), ("c4", 5.4), ("cD", 1.0), ("cE", -0.5))]
+    assert min(np.abs(e).max() for e in each) > 1e-3          # every topology contributes
+    # each part is rounded to double on output: tolerance = a few ulp of the largest part
+    assert np.abs(full - sum(each)).max() < 4e-16 * sum(np.abs(e).max() for e in each)
+
+
+@pytest.mark.parametrize("geo", [dict(kf_n=1.2, kf_p=0.9, n_r=2, n_cos=3, n_phi=4),
+                                 dict(kf_n=1.0, kf_p=0.0, n_r=3, n_cos=2, n_phi=2),
+                                 dict(kf_n=1.3, kf_p=1.3, n_r=2, n_cos=2, n_phi=5, Lambda=450.0, n_reg=3)])
+def test_P11_level0_equals_level1(geo):
+    cfg = rand_cfg(3, 2.0)
+    kw = dict(PHYS, c4=5.4)
+    kw.update(geo)
+    M0 = O.normal_order(cfg, level=0, **kw)
+    M1 = O.normal_order(cfg, level=1, **kw)
+    assert np.abs(M0 - M1).max() < 1e-16 * np.abs(M0).max()
+    M1d = O.normal_order(cfg, level=1, precision="f64", **kw)
+    assert np.abs(M1d - M1).max() < 1e-14 * np.abs(M0).max()
+
+
+# ----------------------------------------------------------------------------------------------
+# P7: kF -> 0 (pins 1/(2 pi)^3, the weights and the r^2 Jacobian).
+# ----------------------------------------------------------------------------------------------
+def test_P7_low_density_limit():
+    cfg = rand_cfg(1, 1.0)
+    p, pp, P = cfg[0, 0:3], cfg[0, 3:6], cfg[0, 6:9]
+    kin = np.array([P / 2 + p, P / 2 - p, np.zeros(3)])
+    kout = np.array([P / 2 + pp, P / 2 - pp, np.zeros(3)])
+    kw = dict(PHYS, c4=5.4)
+    AV = O.av3n(kin, kout, **kw)
+    # trace over the third particle's spin, third isospin fixed to neutron (t3 = 1)
+    lim = np.zeros((16, 16), complex)
+    for r in range(16):
+        for c in range(16):
+            s1o, s2o, t1o, t2o = (r >> 3) & 1, (r >> 2) & 1, (r >> 1) & 1, r & 1
+            s1, s2, t1, t2 = (c >> 3) & 1, (c >> 2) & 1, (c >> 1) & 1, c & 1
+            for s3 in range(2):
+                lim[r, c] += AV[8 * (4 * s1o + 2 * s2o + s3) + 4 * t1o + 2 * t2o + 1,
+                                8 * (4 * s1 + 2 * s2 + s3) + 4 * t1 + 2 * t2 + 1]
+    errs = []
+    for kf in (0.1, 0.01, 0.001):
+        M = O.normal_order(cfg, kf_n=kf, kf_p=0.0, n_r=4, n_cos=4, n_phi=4, **kw)[0]
+        assert np.abs(M).max() < 10 * kf ** 3          # M -> 0
+        ratio = M / (kf ** 3 / (6 * math.pi ** 2))
+        errs.append(np.abs(ratio - lim).max() / np.abs(lim).max())
+    assert errs[0] < 2e-2 and errs[1] < 2e-4 and errs[2] < 2e-6      # O(kF^2)
+    assert errs[0] / errs[1] == pytest.approx(100, rel=0.2)
+
+
+# ----------------------------------------------------------------------------------------------
+# P8: contracting once more over the Fermi sea gives the 3N Hartree-Fock energy of a brute-force
+#     9-D quadrature on the same tiny grids (north_star (c)).
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("geo", [dict(kf_n=1.2, kf_p=0.9), dict(kf_n=1.1, kf_p=0.0)])
+def test_P8_hartree_fock_identity(geo):
+    n = 2
+    kw = dict(PHYS, c4=5.4, n_r=n, n_cos=n, n_phi=n, **geo)
+    e_brute = O.hf3n_bruteforce(**kw)
+    # particles 1 and 2 on the same product grids, third particle integrated by normal ordering
+    nodes = []
+    for tau, kf in ((0, kw["kf_p"]), (1, kw["kf_n"])):
+        if kf <= 0:
+            continue
+        r, wr = O.gauss_legendre(n, 0.0, kf)
+        x, wx = O.gauss_legendre(n, -1.0, 1.0)
+        ph, wp = O.gauss_legendre(n, 0.0, 2 * math.pi)
+        for i in range(n):
+            for j in range(n):
+                for l in range(n):
+                    st = math.sqrt(1 - x[j] ** 2)
+                    k = r[i] * np.array([st * math.cos(ph[l]), st * math.sin(ph[l]), x[j]])
+                    nodes.append((k, r[i] ** 2 * wr[i] * wx[j] * wp[l] / (2 * math.pi) ** 3, tau))
+    cfgs, wts, isos = [], [], []
+    for k1, w1, t1 in nodes:
+        for k2, w2, t2 in nodes:
+            p = (k1 - k2) / 2
+            cfgs.append(np.concatenate([p, p, k1 + k2]))
+            wts.append(w1 * w2)
+            isos.append((t1, t2))
+    M = O.normal_order(np.array(cfgs), **kw)
+    e_no = 0.0
+    for m, w, (t1, t2) in zip(M, wts, isos):
+        for s1 in range(2):
+            for s2 in range(2):
+                e_no += w * m[idx(s1, s2, t1, t2), idx(s1, s2, t1, t2)].real
+    e_no /= 6
+    assert abs(e_brute) > 1e-6
+    assert e_no == pytest.approx(e_brute, rel=1e-13)
+
+
+# ----------------------------------------------------------------------------------------------
+# P12: values of an independent transcription -- a third opinion.
+# ----------------------------------------------------------------------------------------------
+def test_P12_cross_implementation_values():
+    path = os.path.join(os.path.dirname(__file__), "golden", "survey_appendix_a.txt")
+    rows = [l.split() for l in open(path) if l.strip() and not l.startswith("#")]
+    cfg = np.array([[0.3, -0.2, 0.5, -0.1, 0.4, 0.2, 0.2, 0.1, -0.3]])
+    for c4 in (0.0, 5.4):
+        M = O.normal_order(cfg, level=0, kf_p=0.9, kf_n=1.2, n_r=4, n_cos=4, n_phi=4, c4=c4, **PHYS)[0]
+        assert (np.abs(M) > 1e-14).sum() == 96
+        for row in rows:
+            if float(row[0]) != c4:
+                continue
+            r, c, re, im = int(row[1]), int(row[2]), float(row[3]), float(row[4])
+            if r == -1:
+                assert np.linalg.norm(M) == pytest.approx(re, rel=1e-13)
+            elif r == -2:
+                assert np.abs(M).max() == pytest.approx(re, rel=1e-13)
+            else:
+                assert abs(M[r, c] - complex(re, im)) < 1e-14
+
+
+# ----------------------------------------------------------------------------------------------
+# Regulator (reading R5): Jacobi form equals p^2 + |k3 - P/2|^2 / 3 and is ONE exponential.
+# ----------------------------------------------------------------------------------------------
+def test_regulator_reduces_to_the_normal_ordering_form():
+    cfg = rand_cfg(1, 1.0)
+    p, pp, P = cfg[0, 0:3], cfg[0, 3:6], cfg[0, 6:9]
+    k3 = RNG.normal(size=3) * 0.5
+    kin = np.array([P / 2 + p, P / 2 - p, k3])
+    kout = np.array([P / 2 + pp, P / 2 - pp, k3])
+    for Lam, n in ((500.0, 4), (450.0, 3), (400.0, 2)):
+        reg = O.av3n(kin, kout, **only(cE=1.0, Lambda=Lam, n_reg=n))
+        bare = O.av3n(kin, kout, **only(cE=1.0, Lambda=-1.0))
+        L2 = (Lam / HBARC) ** 2
+        d2 = np.dot(k3 - P / 2, k3 - P / 2)
+        want = math.exp(-((p @ p + d2 / 3) / L2) ** n - ((pp @ pp + d2 / 3) / L2) ** n)
+        i = np.unravel_index(np.abs(bare).argmax(), bare.shape)
+        assert (reg[i] / bare[i]).real == pytest.approx(want, rel=1e-14)
