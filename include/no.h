@@ -1,0 +1,109 @@
+/* no.h -- C ABI of the B200 (sm_100a) 3N normal-ordering library  (libno3n.so)
+ *
+ * Operation (arxiv/paper_2603_24532, /root/reference/PAPER.md):
+ *   the second term of Eq. (10) with xi = 1,
+ *
+ *       M(p,p',P)[a',a] = sum_i < i a' | A_123 V_3N | i a > ,
+ *
+ *   i.e. the antisymmetrised chiral N2LO three-nucleon interaction with one nucleon summed
+ *   over the occupied states of the reference state (hole sum of Eq. (6)-(7), PAPER.md:64-72:
+ *   spin, isospin and int d^3k3/(2 pi)^3 theta(kF_tau - k3), separate neutron and proton
+ *   Fermi spheres), evaluated "on the fly for given external momenta" by quadrature on the
+ *   GPU, many vertices per asynchronous transaction.  The interaction is
+ *   the operatorial definition as a 4^A x 4^A spin-isospin matrix with the
+ *   permutation-invariant nonlocal regulator of Eq. (13).  The k3 rule
+ *   is a Gauss-Legendre product grid radial x cos(theta) x phi in a fixed lab frame.
+ *   The operator, the regulator exponent and every other reading of the paper are listed in
+ *   DESIGN.md section 3 (R1-R20).
+ *
+ * Result: for every configuration c = (p, p', P) a complex 16x16 matrix in
+ *   spin(1,2) x isospin(1,2) space, units fm^2 (hbar = c = 1; multiply by hbarc for MeV fm^3),
+ *   index of a two-body state   idx = 8 s1 + 4 s2 + 2 t1 + t2,
+ *   s = 0 spin up / 1 down, t = 0 proton / 1 neutron; row = outgoing (p'), column = incoming (p).
+ *   k1 = P/2 + p, k2 = P/2 - p, k1' = P/2 + p', k2' = P/2 - p'.
+ *   The caller multiplies by xi = 1/2 or 2/3 and adds the NN part.
+ *
+ * All functions return 0 (NO_OK) on success or a positive NO_ERR_* code; they never throw
+ * and never exit.  There is no CPU fallback: without a CUDA device every call fails.
+ */
+#ifndef NO_H_
+#define NO_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NO_OK          0
+#define NO_ERR_INVALID 1   /* bad parameter, null pointer, n_cfg < 0, misaligned pointer   */
+#define NO_ERR_CUDA    2   /* CUDA runtime or launch failure; text via no_last_cuda_error() */
+#define NO_ERR_ALLOC   3   /* host or device allocation failed                              */
+
+typedef struct no_handle no_handle;   /* opaque; owns its device tables (and host-path scratch) */
+
+typedef struct no_params {
+  double kf_n, kf_p;        /* Fermi momenta, fm^-1; 0 allowed (empty sphere is skipped); <0 invalid */
+  double c1, c3, c4;        /* GeV^-1; c4 = 0 in all BASELINE configs (reading R2)                   */
+  double cD, cE;            /* dimensionless                                                         */
+  double gA;                /* dimensionless                                                         */
+  double fpi, mpi;          /* MeV, both > 0                                                         */
+  double lambda_chi;        /* MeV; <= 0 means the default 700 (reading R3)                          */
+  double Lambda;            /* MeV, 3N regulator cutoff; <= 0 means unregulated (f_R = 1)            */
+  int    n_reg;             /* regulator exponent n >= 1: exp(-((p^2+3q^2/4)/Lambda^2)^n) (R5)       */
+  int    n_r, n_cos, n_phi; /* Gauss-Legendre orders of the k3 grid, each 1..128                     */
+  int    device;            /* CUDA device ordinal                                                   */
+} no_params;
+
+/* Build the handle: validates *p, converts units (hbarc = 197.3269804 MeV fm), computes the
+ * Gauss-Legendre nodes and weights on [0,kF_tau], [-1,1], [0,2 pi] on the host (Newton on
+ * P_N), uploads the k3 tables of every non-empty Fermi sphere (equal kF_n = kF_p share one
+ * grid, full isospin trace of the third nucleon) to device `p->device`.
+ * *h is written only on success.  HOST pointers. */
+int no_init(no_handle **h, const no_params *p);
+
+/* Enqueue the normal ordering of n_cfg configurations on `cuda_stream` (a cudaStream_t; NULL is
+ * the default stream).  No synchronisation inside: the call returns as soon as the work is
+ * enqueued ("asynchronous GPU transaction"); one handle may be used from several
+ * streams at once.
+ *   d_cfg : DEVICE, const, [n_cfg][9] doubles = p(xyz), p'(xyz), P(xyz) in fm^-1, dense,
+ *           8-byte aligned, caller-owned
+ *   d_out : DEVICE, [n_cfg][16][16][2] doubles (re, im), row-major rows = outgoing state,
+ *           16-byte aligned, dense, caller-owned; every element is written (structural zeros
+ *           are written as 0)
+ * n_cfg == 0 succeeds and does nothing.  Non-finite inputs propagate to non-finite outputs. */
+int no_eval(const no_handle *h, const double *d_cfg, long long n_cfg, double *d_out, void *cuda_stream);
+
+/* Same operation with HOST buffers (pageable or pinned): copies h_cfg to a device scratch owned
+ * by the handle, runs the kernels, copies the result back and SYNCHRONISES `cuda_stream` before
+ * returning.  Not re-entrant for one handle (the scratch is shared).  Used for the end-to-end
+ * measurement. */
+int no_eval_host(no_handle *h, const double *h_cfg, long long n_cfg, double *h_out, void *cuda_stream);
+
+/* Release the handle and everything it owns.  NULL is a no-op. */
+int no_free(no_handle *h);
+
+/* Static description of a code. */
+const char *no_strerror(int code);
+
+/* Text of the last CUDA error seen by the calling thread ("" if none). */
+const char *no_last_cuda_error(void);
+
+/* Facts about the kernel no_eval launches for this handle (each pointer may be NULL):
+ * registers per thread, dynamic shared memory per CTA in bytes, threads per CTA, resident CTAs
+ * per SM (occupancy API), number of SMs, configurations per CTA. */
+int no_kernel_info(const no_handle *h, int *regs, int *smem_bytes, int *threads, int *ctas_per_sm,
+                   int *n_sm, int *cfg_per_cta);
+
+/* Number of k3-point evaluations one configuration costs with this handle:
+ * n_r * n_cos * n_phi * (number of distinct non-zero Fermi momenta). */
+long long no_evals_per_cfg(const no_handle *h);
+
+/* FP64 roofline probe: runs a register-resident chain of independent DFMAs on every SM of
+ * `device` for about `millis` milliseconds on `cuda_stream`, synchronises, and writes the achieved
+ * rate in TFLOP/s (2 flops per DFMA) and the SM count.  Used by bench.py to state the measured
+ * FP64 peak next to the nominal one. */
+int no_probe_fp64_peak(int device, int millis, double *tflops, int *n_sm, void *cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NO_H_ */

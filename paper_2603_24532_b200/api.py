@@ -1,0 +1,61 @@
+"""Convenience wrapper: a handle plus torch tensors (device memory and streams only)."""
+from __future__ import annotations
+
+import torch
+
+from . import binding
+
+
+class NormalOrdering:
+    """`NormalOrdering(**no_params fields)`; `__call__(cfg)` -> complex128 [n,16,16] on the device.
+
+    cfg: float64 tensor [n, 9] = (p, p', P) in fm^-1.  A CUDA tensor goes through no_eval on the
+    current stream (asynchronous); a CPU tensor goes through no_eval_host (copies inside, blocks).
+    """
+
+    def __init__(self, device: int = 0, **params):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2603_24532_b200 needs a CUDA device (no CPU fallback)")
+        self.device = device
+        self.params = dict(params)
+        self._h = binding.no_init(device=device, **params)
+
+    def close(self):
+        if getattr(self, "_h", None) is not None:
+            binding.no_free(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def evals_per_cfg(self) -> int:
+        return binding.no_evals_per_cfg(self._h)
+
+    def kernel_info(self) -> dict:
+        return binding.no_kernel_info(self._h)
+
+    def eval_into(self, cfg: torch.Tensor, out: torch.Tensor, stream: torch.cuda.Stream | None = None) -> None:
+        """Enqueue no_eval: cfg [n,9] float64 CUDA, out [n,16,16,2] float64 CUDA (both contiguous)."""
+        assert cfg.is_cuda and out.is_cuda and cfg.dtype == torch.float64 and out.dtype == torch.float64
+        assert cfg.is_contiguous() and out.is_contiguous()
+        n = cfg.shape[0]
+        assert cfg.numel() == 9 * n and out.numel() == 512 * n
+        s = stream if stream is not None else torch.cuda.current_stream(cfg.device)
+        binding.no_eval(self._h, cfg.data_ptr(), n, out.data_ptr(), s.cuda_stream)
+
+    def __call__(self, cfg: torch.Tensor) -> torch.Tensor:
+        cfg = cfg.to(torch.float64).contiguous().reshape(-1, 9)
+        n = cfg.shape[0]
+        if cfg.is_cuda:
+            out = torch.empty((n, 16, 16, 2), dtype=torch.float64, device=cfg.device)
+            self.eval_into(cfg, out)
+        else:
+            out = torch.empty((n, 16, 16, 2), dtype=torch.float64)
+            if n:
+                binding.no_eval_host(self._h, cfg.data_ptr(), n, out.data_ptr(),
+                                     torch.cuda.current_stream(self.device).cuda_stream)
+        return torch.view_as_complex(out)

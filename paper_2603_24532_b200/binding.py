@@ -1,0 +1,120 @@
+"""Thin ctypes binding of libno3n.so: the same names as include/no.h, argument marshalling only.
+
+PyTorch is used by callers for device memory and streams; every step of the hot path runs in the
+CUDA kernels behind no_eval.  There is no CPU fallback: if the library is missing or no CUDA
+device is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libno3n.so")
+
+NO_OK, NO_ERR_INVALID, NO_ERR_CUDA, NO_ERR_ALLOC = 0, 1, 2, 3
+
+EXPORTS = ("no_init", "no_eval", "no_eval_host", "no_free", "no_strerror", "no_last_cuda_error",
+           "no_kernel_info", "no_evals_per_cfg", "no_probe_fp64_peak")
+
+
+class no_params(ctypes.Structure):
+    """struct no_params of include/no.h."""
+    _fields_ = [(n, ctypes.c_double) for n in
+                ("kf_n", "kf_p", "c1", "c3", "c4", "cD", "cE", "gA", "fpi", "mpi", "lambda_chi", "Lambda")] + \
+               [(n, ctypes.c_int) for n in ("n_reg", "n_r", "n_cos", "n_phi", "device")]
+
+
+class NoError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        lib = load()
+        msg = lib.no_strerror(code).decode()
+        cuda = lib.no_last_cuda_error().decode()
+        super().__init__(f"{where}: {msg}" + (f" [{cuda}]" if code == NO_ERR_CUDA and cuda else ""))
+        self.code = code
+
+
+_lib = None
+
+
+def load() -> ctypes.CDLL:
+    """dlopen libno3n.so (built by `python -m paper_2603_24532_b200.build`); fails loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2603_24532_b200.build` "
+                               "(the package has no CPU fallback)")
+        lib = ctypes.CDLL(LIB_PATH)
+        H = ctypes.c_void_p
+        lib.no_init.argtypes = [ctypes.POINTER(H), ctypes.POINTER(no_params)]
+        lib.no_eval.argtypes = [H, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]
+        lib.no_eval_host.argtypes = [H, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]
+        lib.no_free.argtypes = [H]
+        lib.no_strerror.argtypes = [ctypes.c_int]
+        lib.no_strerror.restype = ctypes.c_char_p
+        lib.no_last_cuda_error.restype = ctypes.c_char_p
+        ip = ctypes.POINTER(ctypes.c_int)
+        lib.no_kernel_info.argtypes = [H, ip, ip, ip, ip, ip, ip]
+        lib.no_evals_per_cfg.argtypes = [H]
+        lib.no_evals_per_cfg.restype = ctypes.c_longlong
+        lib.no_probe_fp64_peak.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double), ip,
+                                           ctypes.c_void_p]
+        for name in ("no_init", "no_eval", "no_eval_host", "no_free", "no_kernel_info", "no_probe_fp64_peak"):
+            getattr(lib, name).restype = ctypes.c_int
+        _lib = lib
+    return _lib
+
+
+def no_init(device: int = 0, **params) -> ctypes.c_void_p:
+    """no_init: keyword arguments are the fields of struct no_params; returns the opaque handle."""
+    p = no_params(device=device, **params)
+    h = ctypes.c_void_p()
+    rc = load().no_init(ctypes.byref(h), ctypes.byref(p))
+    if rc != NO_OK:
+        raise NoError(rc, "no_init")
+    return h
+
+
+def no_eval(h, d_cfg_ptr: int, n_cfg: int, d_out_ptr: int, stream_ptr: Optional[int] = None) -> None:
+    """no_eval with raw DEVICE pointers (e.g. tensor.data_ptr()) and a cudaStream_t value."""
+    rc = load().no_eval(h, ctypes.c_void_p(d_cfg_ptr), n_cfg, ctypes.c_void_p(d_out_ptr),
+                        ctypes.c_void_p(stream_ptr or 0))
+    if rc != NO_OK:
+        raise NoError(rc, "no_eval")
+
+
+def no_eval_host(h, h_cfg_ptr: int, n_cfg: int, h_out_ptr: int, stream_ptr: Optional[int] = None) -> None:
+    """no_eval_host with raw HOST pointers; synchronises the stream before returning."""
+    rc = load().no_eval_host(h, ctypes.c_void_p(h_cfg_ptr), n_cfg, ctypes.c_void_p(h_out_ptr),
+                             ctypes.c_void_p(stream_ptr or 0))
+    if rc != NO_OK:
+        raise NoError(rc, "no_eval_host")
+
+
+def no_free(h) -> None:
+    rc = load().no_free(h)
+    if rc != NO_OK:
+        raise NoError(rc, "no_free")
+
+
+def no_kernel_info(h) -> dict:
+    v = [ctypes.c_int() for _ in range(6)]
+    rc = load().no_kernel_info(h, *[ctypes.byref(x) for x in v])
+    if rc != NO_OK:
+        raise NoError(rc, "no_kernel_info")
+    keys = ("regs", "smem_bytes", "threads", "ctas_per_sm", "n_sm", "cfg_per_cta")
+    return {k: x.value for k, x in zip(keys, v)}
+
+
+def no_evals_per_cfg(h) -> int:
+    return int(load().no_evals_per_cfg(h))
+
+
+def no_probe_fp64_peak(device: int = 0, millis: int = 200, stream_ptr: Optional[int] = None) -> dict:
+    t = ctypes.c_double()
+    n = ctypes.c_int()
+    rc = load().no_probe_fp64_peak(device, millis, ctypes.byref(t), ctypes.byref(n), ctypes.c_void_p(stream_ptr or 0))
+    if rc != NO_OK:
+        raise NoError(rc, "no_probe_fp64_peak")
+    return {"tflops": t.value, "n_sm": n.value}

@@ -1,0 +1,253 @@
+// no_api.cu -- C ABI of libno3n.so (include/no.h): no_init / no_eval / no_eval_host / no_free and
+// the small query and probe entry points.  Host setup lives in no_host.h, the kernel in
+// no_kernel.cuh.  sm_100a only; there is no CPU path.
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "../../include/no.h"
+#include "no_host.h"
+#include "no_kernel.cuh"
+
+using namespace no3n;
+
+namespace {
+
+thread_local char g_cuda_err[256] = "";
+
+int cuda_fail(cudaError_t e, const char* where) {
+  snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s (%s)", where, cudaGetErrorName(e), cudaGetErrorString(e));
+  return NO_ERR_CUDA;
+}
+
+#define NO_CUDA(call)                                 \
+  do {                                                \
+    cudaError_t e_ = (call);                          \
+    if (e_ != cudaSuccess) return cuda_fail(e_, #call); \
+  } while (0)
+
+constexpr int kWarps = 4;   // configurations per CTA
+
+typedef void (*KernelFn)(const DevParams, const double*, long long, double*);
+
+struct Variant {
+  KernelFn fn;
+  size_t smem;
+};
+
+template <int NREG, bool C4>
+Variant make_variant(int tab_doubles) {
+  Variant v;
+  v.fn = no3n_kernel<NREG, C4, kWarps, C4 ? 2 : 3>;
+  v.smem = smem_bytes<C4>(tab_doubles, kWarps);
+  return v;
+}
+
+template <bool C4>
+Variant pick_nreg(int nreg, int tab_doubles) {
+  switch (nreg) {
+    case -1: return make_variant<-1, C4>(tab_doubles);
+    case 1: return make_variant<1, C4>(tab_doubles);
+    case 2: return make_variant<2, C4>(tab_doubles);
+    case 3: return make_variant<3, C4>(tab_doubles);
+    case 4: return make_variant<4, C4>(tab_doubles);
+    default: return make_variant<0, C4>(tab_doubles);
+  }
+}
+
+}  // namespace
+
+struct no_handle {
+  HostPlan plan;
+  int device;
+  double* d_tab;
+  Variant var;
+  // scratch of the host-buffer path
+  double* d_cfg;
+  double* d_out;
+  long long scratch_cfg;
+};
+
+namespace {
+
+struct DeviceGuard {
+  int prev;
+  bool ok;
+  explicit DeviceGuard(int dev) : prev(-1), ok(false) {
+    if (cudaGetDevice(&prev) != cudaSuccess) return;
+    if (prev != dev && cudaSetDevice(dev) != cudaSuccess) return;
+    ok = true;
+  }
+  ~DeviceGuard() {
+    if (prev >= 0) cudaSetDevice(prev);
+  }
+};
+
+int launch(const no_handle* h, const double* d_cfg, long long n_cfg, double* d_out, cudaStream_t s) {
+  const long long blocks = (n_cfg + kWarps - 1) / kWarps;
+  if (blocks > 2147483647LL) return NO_ERR_INVALID;
+  h->var.fn<<<(unsigned)blocks, kWarps * 32, h->var.smem, s>>>(h->plan.dp, d_cfg, n_cfg, d_out);
+  NO_CUDA(cudaGetLastError());
+  return NO_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int no_init(no_handle** out, const no_params* p) {
+  if (!out || !p) return NO_ERR_INVALID;
+  no_handle* h = new (std::nothrow) no_handle();
+  if (!h) return NO_ERR_ALLOC;
+  h->d_tab = nullptr; h->d_cfg = nullptr; h->d_out = nullptr; h->scratch_cfg = 0;
+  int rc = build_plan(p, h->plan);
+  if (rc != NO_OK) { delete h; return rc; }
+  int n_dev = 0;
+  cudaError_t e = cudaGetDeviceCount(&n_dev);
+  if (e != cudaSuccess) { delete h; return cuda_fail(e, "cudaGetDeviceCount"); }
+  if (p->device < 0 || p->device >= n_dev) { delete h; return NO_ERR_INVALID; }
+  h->device = p->device;
+  DeviceGuard guard(h->device);
+  if (!guard.ok) { delete h; return cuda_fail(cudaGetLastError(), "cudaSetDevice"); }
+  h->var = h->plan.has_c4 ? pick_nreg<true>(h->plan.nreg_variant, h->plan.dp.tab_doubles)
+                          : pick_nreg<false>(h->plan.nreg_variant, h->plan.dp.tab_doubles);
+  e = cudaFuncSetAttribute((const void*)h->var.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->var.smem);
+  if (e != cudaSuccess) { delete h; return cuda_fail(e, "cudaFuncSetAttribute(smem)"); }
+  const size_t bytes = sizeof(double) * (size_t)(h->plan.dp.tab_doubles > 0 ? h->plan.dp.tab_doubles : 2);
+  e = cudaMalloc((void**)&h->d_tab, bytes);
+  if (e != cudaSuccess) { delete h; cuda_fail(e, "cudaMalloc(tables)"); return NO_ERR_ALLOC; }
+  if (h->plan.dp.tab_doubles > 0) {
+    e = cudaMemcpy(h->d_tab, h->plan.tab.data(), sizeof(double) * h->plan.dp.tab_doubles, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { cudaFree(h->d_tab); delete h; return cuda_fail(e, "cudaMemcpy(tables)"); }
+  }
+  h->plan.dp.tab = h->d_tab;
+  *out = h;
+  return NO_OK;
+}
+
+int no_eval(const no_handle* h, const double* d_cfg, long long n_cfg, double* d_out, void* cuda_stream) {
+  if (!h || n_cfg < 0) return NO_ERR_INVALID;
+  if (n_cfg == 0) return NO_OK;
+  if (!d_cfg || !d_out) return NO_ERR_INVALID;
+  if ((reinterpret_cast<uintptr_t>(d_cfg) & 7u) || (reinterpret_cast<uintptr_t>(d_out) & 15u)) return NO_ERR_INVALID;
+  DeviceGuard guard(h->device);
+  if (!guard.ok) return cuda_fail(cudaGetLastError(), "cudaSetDevice");
+  return launch(h, d_cfg, n_cfg, d_out, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int no_eval_host(no_handle* h, const double* h_cfg, long long n_cfg, double* h_out, void* cuda_stream) {
+  if (!h || n_cfg < 0) return NO_ERR_INVALID;
+  if (n_cfg == 0) return NO_OK;
+  if (!h_cfg || !h_out) return NO_ERR_INVALID;
+  DeviceGuard guard(h->device);
+  if (!guard.ok) return cuda_fail(cudaGetLastError(), "cudaSetDevice");
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  if (n_cfg > h->scratch_cfg) {
+    if (h->d_cfg) cudaFree(h->d_cfg);
+    if (h->d_out) cudaFree(h->d_out);
+    h->d_cfg = h->d_out = nullptr;
+    h->scratch_cfg = 0;
+    cudaError_t e = cudaMalloc((void**)&h->d_cfg, sizeof(double) * 9 * (size_t)n_cfg);
+    if (e != cudaSuccess) { cuda_fail(e, "cudaMalloc(cfg scratch)"); return NO_ERR_ALLOC; }
+    e = cudaMalloc((void**)&h->d_out, sizeof(double) * 512 * (size_t)n_cfg);
+    if (e != cudaSuccess) { cudaFree(h->d_cfg); h->d_cfg = nullptr; cuda_fail(e, "cudaMalloc(out scratch)"); return NO_ERR_ALLOC; }
+    h->scratch_cfg = n_cfg;
+  }
+  NO_CUDA(cudaMemcpyAsync(h->d_cfg, h_cfg, sizeof(double) * 9 * (size_t)n_cfg, cudaMemcpyHostToDevice, s));
+  const int rc = launch(h, h->d_cfg, n_cfg, h->d_out, s);
+  if (rc != NO_OK) return rc;
+  NO_CUDA(cudaMemcpyAsync(h_out, h->d_out, sizeof(double) * 512 * (size_t)n_cfg, cudaMemcpyDeviceToHost, s));
+  NO_CUDA(cudaStreamSynchronize(s));
+  return NO_OK;
+}
+
+int no_free(no_handle* h) {
+  if (!h) return NO_OK;
+  DeviceGuard guard(h->device);
+  if (h->d_tab) cudaFree(h->d_tab);
+  if (h->d_cfg) cudaFree(h->d_cfg);
+  if (h->d_out) cudaFree(h->d_out);
+  delete h;
+  return NO_OK;
+}
+
+const char* no_strerror(int code) {
+  switch (code) {
+    case NO_OK: return "success";
+    case NO_ERR_INVALID: return "invalid argument (parameter out of range, null or misaligned pointer, n_cfg < 0)";
+    case NO_ERR_CUDA: return "CUDA runtime or launch failure (see no_last_cuda_error)";
+    case NO_ERR_ALLOC: return "allocation failed";
+    default: return "unknown error code";
+  }
+}
+
+const char* no_last_cuda_error(void) { return g_cuda_err; }
+
+int no_kernel_info(const no_handle* h, int* regs, int* smem, int* threads, int* ctas_per_sm, int* n_sm,
+                   int* cfg_per_cta) {
+  if (!h) return NO_ERR_INVALID;
+  DeviceGuard guard(h->device);
+  if (!guard.ok) return cuda_fail(cudaGetLastError(), "cudaSetDevice");
+  cudaFuncAttributes a;
+  NO_CUDA(cudaFuncGetAttributes(&a, (const void*)h->var.fn));
+  int occ = 0;
+  NO_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void*)h->var.fn, kWarps * 32, h->var.smem));
+  int sms = 0;
+  NO_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device));
+  if (regs) *regs = a.numRegs;
+  if (smem) *smem = (int)h->var.smem;
+  if (threads) *threads = kWarps * 32;
+  if (ctas_per_sm) *ctas_per_sm = occ;
+  if (n_sm) *n_sm = sms;
+  if (cfg_per_cta) *cfg_per_cta = kWarps;
+  return NO_OK;
+}
+
+long long no_evals_per_cfg(const no_handle* h) { return h ? h->plan.evals_per_cfg : 0; }
+
+int no_probe_fp64_peak(int device, int millis, double* tflops, int* n_sm, void* cuda_stream) {
+  if (!tflops || millis < 1) return NO_ERR_INVALID;
+  int n_dev = 0;
+  NO_CUDA(cudaGetDeviceCount(&n_dev));
+  if (device < 0 || device >= n_dev) return NO_ERR_INVALID;
+  DeviceGuard guard(device);
+  if (!guard.ok) return cuda_fail(cudaGetLastError(), "cudaSetDevice");
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  int sms = 0;
+  NO_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device));
+  const int threads = 256, blocks = sms * 8;
+  double* sink = nullptr;
+  NO_CUDA(cudaMalloc((void**)&sink, sizeof(double) * threads * blocks));
+  cudaEvent_t e0, e1;
+  NO_CUDA(cudaEventCreate(&e0));
+  NO_CUDA(cudaEventCreate(&e1));
+  int iters = 1 << 12;
+  double best = 0.0;
+  float ms = 0.f;
+  // grow the launch until it lasts about `millis`, keep the best rate of the long launches
+  for (int rep = 0; rep < 24; ++rep) {
+    NO_CUDA(cudaEventRecord(e0, s));
+    dfma_probe_kernel<<<blocks, threads, 0, s>>>(sink, iters, 1.0);
+    NO_CUDA(cudaEventRecord(e1, s));
+    NO_CUDA(cudaEventSynchronize(e1));
+    NO_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+    const double flops = 2.0 * 16.0 * (double)iters * threads * (double)blocks;
+    const double rate = flops / (ms * 1e-3) * 1e-12;
+    if (ms >= 0.5f * millis) {
+      if (rate > best) best = rate;
+      if (rep >= 3 && ms >= (float)millis) break;
+    }
+    if (ms < (float)millis && iters < (1 << 28)) iters *= 2;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(sink);
+  NO_CUDA(cudaGetLastError());
+  *tflops = best;
+  if (n_sm) *n_sm = sms;
+  return NO_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,165 @@
+// no_host.h -- host-side setup of the 3N normal-ordering library (step a0 of SURVEY.md 8(a)):
+// parameter validation, unit conversion, Gauss-Legendre rules, k3 tables, kernel-variant choice.
+// Plain C++ (no CUDA calls) so that the CPU unit tests can drive it through tests/host_emu.cpp.
+#pragma once
+
+#include <cmath>
+#include <vector>
+
+#include "../../include/no.h"
+#include "no_core.h"
+
+namespace no3n {
+
+constexpr double kHbarc = 197.3269804;   // MeV fm (reading R9)
+constexpr int kMaxOrder = 128;
+
+// Gauss-Legendre rule of order n on [lo, hi].  Roots of P_n by Newton's method started from the
+// Chebyshev-like guess, evaluated with the three-term recurrence in long double; the rule is
+// built for the non-negative roots and mirrored so that nodes and weights are exactly symmetric.
+inline void gl_rule(int n, double lo, double hi, std::vector<double>& x, std::vector<double>& w) {
+  x.resize(n);
+  w.resize(n);
+  const long double pi = 3.141592653589793238462643383279502884L;
+  const long double c = 0.5L * ((long double)hi + (long double)lo), h = 0.5L * ((long double)hi - (long double)lo);
+  const int half = n / 2;
+  for (int k = 0; k < half; ++k) {          // k-th largest root, t > 0
+    long double t = cosl(pi * (4 * k + 3) / (4 * n + 2));
+    long double dp = 1;
+    for (int it = 0; it < 64; ++it) {
+      long double pm = 1, pc = t;            // P_0, P_1
+      for (int m = 2; m <= n; ++m) {
+        const long double pn = ((2 * m - 1) * t * pc - (m - 1) * pm) / m;
+        pm = pc;
+        pc = pn;
+      }
+      dp = n * (pm - t * pc) / (1 - t * t);  // P_n'(t)
+      const long double step = pc / dp;
+      t -= step;
+      if (fabsl(step) <= 4e-20L) {
+        // derivative at the final root
+        pm = 1; pc = t;
+        for (int m = 2; m <= n; ++m) {
+          const long double pn = ((2 * m - 1) * t * pc - (m - 1) * pm) / m;
+          pm = pc;
+          pc = pn;
+        }
+        dp = n * (pm - t * pc) / (1 - t * t);
+        break;
+      }
+    }
+    const long double wt = 2 / ((1 - t * t) * dp * dp);
+    x[n - 1 - k] = (double)(c + h * t);
+    x[k] = (double)(c - h * t);
+    w[n - 1 - k] = w[k] = (double)(h * wt);
+  }
+  if (n & 1) {                               // middle root t = 0: P_n'(0) from the recurrence
+    long double pm = 1, pc = 0;
+    for (int m = 2; m <= n; ++m) {
+      const long double pn = (-(long double)(m - 1) * pm) / m;   // t = 0
+      pm = pc;
+      pc = pn;
+    }
+    // after the loop pc = P_n(0) = 0 (n odd), pm = P_{n-1}(0);  P_n'(0) = n P_{n-1}(0)
+    const long double dp = n * pm;
+    x[half] = (double)c;
+    w[half] = (double)(h * 2 / (dp * dp));
+  }
+}
+
+struct HostPlan {
+  DevParams dp;               // dp.tab is filled by the caller after the upload
+  std::vector<double> tab;    // host copy of the device tables
+  int nreg_variant;           // -1 unregulated, 0 generic, 1..4 unrolled
+  bool has_c4;
+  int n_sph;                  // distinct non-zero Fermi momenta
+  long long evals_per_cfg;
+};
+
+inline bool finite_all(const no_params& p) {
+  const double v[] = {p.kf_n, p.kf_p, p.c1, p.c3, p.c4, p.cD, p.cE, p.gA, p.fpi, p.mpi, p.lambda_chi, p.Lambda};
+  for (double d : v) if (!std::isfinite(d)) return false;
+  return true;
+}
+
+inline int build_plan(const no_params* p, HostPlan& plan) {
+  if (!p || !finite_all(*p)) return NO_ERR_INVALID;
+  if (p->kf_n < 0 || p->kf_p < 0 || !(p->fpi > 0) || !(p->mpi > 0)) return NO_ERR_INVALID;
+  if (p->n_r < 1 || p->n_r > kMaxOrder || p->n_cos < 1 || p->n_cos > kMaxOrder || p->n_phi < 1 ||
+      p->n_phi > kMaxOrder)
+    return NO_ERR_INVALID;
+  const bool regulated = p->Lambda > 0;
+  if (regulated && (p->n_reg < 1 || p->n_reg > kMaxRegPoly)) return NO_ERR_INVALID;
+
+  DevParams& d = plan.dp;
+  d = DevParams();
+  d.tab = nullptr;
+  d.n_r = p->n_r; d.n_cos = p->n_cos; d.n_phi = p->n_phi;
+  const double mpi = p->mpi / kHbarc, fpi = p->fpi / kHbarc;
+  const double Lchi = (p->lambda_chi > 0 ? p->lambda_chi : 700.0) / kHbarc;
+  const double c1 = p->c1 * 1e-3 * kHbarc, c3 = p->c3 * 1e-3 * kHbarc, c4 = p->c4 * 1e-3 * kHbarc;
+  const double f2 = fpi * fpi;
+  d.m2 = mpi * mpi;
+  d.inv_L2 = regulated ? (kHbarc / p->Lambda) * (kHbarc / p->Lambda) : 0.0;
+  d.al = -4.0 * c1 * d.m2 / f2;
+  d.be = 2.0 * c3 / f2;
+  d.G2 = (p->gA / (2.0 * fpi)) * (p->gA / (2.0 * fpi));
+  d.gD = -p->gA * p->cD / (8.0 * f2 * f2 * Lchi);
+  d.gE2 = p->cE / (f2 * f2 * Lchi);
+  d.g4 = d.G2 * c4 / f2;
+  d.n_reg = regulated ? p->n_reg : 0;
+  plan.nreg_variant = !regulated ? -1 : (p->n_reg <= 4 ? p->n_reg : 0);
+  plan.has_c4 = (p->c4 != 0.0);
+
+  // passes: equal non-zero Fermi momenta share one grid with the full isospin trace (R12)
+  struct Pass { double kf, nsp, esum; };
+  std::vector<Pass> passes;
+  if (p->kf_n > 0 && p->kf_n == p->kf_p) {
+    passes.push_back({p->kf_n, 2.0, 0.0});
+  } else {
+    if (p->kf_p > 0) passes.push_back({p->kf_p, 1.0, +1.0});
+    if (p->kf_n > 0) passes.push_back({p->kf_n, 1.0, -1.0});
+  }
+  d.n_pass = (int)passes.size();
+  plan.n_sph = d.n_pass;
+  plan.evals_per_cfg = (long long)p->n_r * p->n_cos * p->n_phi * d.n_pass;
+
+  const int per = tab_pass_doubles(p->n_r, p->n_cos, p->n_phi);
+  int total = per * d.n_pass;
+  total = (total + 1) & ~1;               // 16-byte granularity of the bulk copy
+  d.tab_doubles = total;
+  plan.tab.assign(total, 0.0);
+  const double pi = 3.14159265358979323846;
+  const double norm = 1.0 / (8.0 * pi * pi * pi);
+  std::vector<double> xr, wr, xc, wc, xp, wp;
+  gl_rule(p->n_cos, -1.0, 1.0, xc, wc);
+  gl_rule(p->n_phi, 0.0, 2.0 * pi, xp, wp);
+  for (int s = 0; s < d.n_pass; ++s) {
+    d.pass_off[s] = per * s;
+    d.nsp[s] = passes[s].nsp;
+    d.esum[s] = passes[s].esum;
+    double* T = plan.tab.data() + per * s;
+    gl_rule(p->n_r, 0.0, passes[s].kf, xr, wr);
+    for (int i = 0; i < p->n_r; ++i) {
+      T[4 * i + 0] = xr[i];
+      T[4 * i + 1] = xr[i] * xr[i];
+      T[4 * i + 2] = wr[i] * xr[i] * xr[i] * norm;
+      T[4 * i + 3] = 0.0;
+    }
+    double* A = T + 4 * p->n_r;
+    for (int j = 0; j < p->n_cos; ++j) {
+      A[j] = xc[j];
+      A[p->n_cos + j] = std::sqrt((1.0 - xc[j]) * (1.0 + xc[j]));
+      A[2 * p->n_cos + j] = wc[j];
+    }
+    double* B = A + 3 * p->n_cos;
+    for (int l = 0; l < p->n_phi; ++l) {
+      B[l] = std::cos(xp[l]);
+      B[p->n_phi + l] = std::sin(xp[l]);
+      B[2 * p->n_phi + l] = wp[l];
+    }
+  }
+  return NO_OK;
+}
+
+}  // namespace no3n

@@ -1,0 +1,169 @@
+// no_kernel.cuh -- the sm_100a kernel of the 3N normal ordering.
+//
+// One warp integrates one configuration (p, p', P): lanes stride over the angular directions
+// of the k3 grid, every lane runs the radial loop of its direction with all sums in registers
+// (no3n::node, the hot loop), folds them into lane-private shared-memory accumulators
+// (no3n::second_level), then the warp reduces the 61 (101 with c4) moments, turns them into
+// Pauli-operator coefficients and writes the 16x16 complex matrix.  A CTA holds WARPS warps;
+// the quadrature tables of every Fermi sphere are staged once per CTA into shared memory with
+// one TMA bulk copy (cp.async.bulk + mbarrier).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "no_core.h"
+
+namespace no3n {
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+
+__device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t phase) {
+  uint32_t done = 0;
+  while (!done) {
+    asm volatile("{\n\t.reg .pred p;\n\t"
+                 "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+                 "selp.b32 %0, 1, 0, p;\n\t}"
+                 : "=r"(done) : "r"(smem_u32(bar)), "r"(phase) : "memory");
+  }
+}
+
+// shared memory per CTA, in doubles: tables | mbarrier (2) | mom[WARPS][rows_pad] | acc[WARPS][rows][32]
+template <bool C4> __host__ __device__ constexpr int rows_pad() { return (Layout<C4>::kRows + 3) & ~3; }
+
+template <bool C4>
+inline size_t smem_bytes(int tab_doubles, int warps) {
+  return sizeof(double) * (size_t)(tab_doubles + 2 + warps * (rows_pad<C4>() + Layout<C4>::kRows * kLanes));
+}
+
+template <int NREG, bool C4, int WARPS, int MINB>
+__global__ void __launch_bounds__(WARPS * 32, MINB)
+no3n_kernel(const DevParams P, const double* __restrict__ cfg, long long n_cfg, double* __restrict__ out) {
+  extern __shared__ __align__(16) double smem[];
+  using L = Layout<C4>;
+  double* s_tab = smem;
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem + P.tab_doubles);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  double* mom = smem + P.tab_doubles + 2 + warp * rows_pad<C4>();
+  double* acc = smem + P.tab_doubles + 2 + WARPS * rows_pad<C4>() + warp * (L::kRows * kLanes);
+
+  // ---- a0: stage the quadrature tables (TMA bulk copy, one per CTA) ----
+  if (threadIdx.x == 0) mbar_init(bar, 1);
+  __syncthreads();
+  if (threadIdx.x == 0 && P.tab_doubles > 0) {
+    const uint32_t bytes = (uint32_t)P.tab_doubles * 8u;
+    mbar_expect_tx(bar, bytes);
+    tma_bulk_g2s(s_tab, P.tab, bytes, bar);
+  }
+
+  const long long ic = (long long)blockIdx.x * WARPS + warp;
+  if (ic >= n_cfg) return;
+
+  // ---- a1: per-configuration constants (every lane holds them) ----
+  CfgConst c;
+  {
+    double q[9];
+#pragma unroll
+    for (int a = 0; a < 9; ++a) q[a] = __ldg(cfg + ic * 9 + a);
+    cfg_setup<NREG>(P, q, c);
+  }
+  if (P.tab_doubles > 0) mbar_wait(bar, 0);
+
+  double blk[6] = {0, 0, 0, 0, 0, 0};
+  for (int pass = 0; pass < P.n_pass; ++pass) {
+    const double* rad = s_tab + P.pass_off[pass];
+    const double* ct = rad + 4 * P.n_r;
+    const double* st = ct + P.n_cos;
+    const double* wc = st + P.n_cos;
+    const double* cph = wc + P.n_cos;
+    const double* sph = cph + P.n_phi;
+    const double* wph = sph + P.n_phi;
+#pragma unroll 1
+    for (int row = 0; row < L::kRows; ++row) acc[row * kLanes + lane] = 0.0;
+
+    // ---- a2 + a3: hot loop over the k3 nodes of this sphere ----
+    const int n_dir = P.n_cos * P.n_phi;
+#pragma unroll 1
+    for (int m = lane; m < n_dir; m += kLanes) {
+      const int j = m / P.n_phi, l = m - j * P.n_phi;
+      const double sj = st[j];
+      DirConst d;
+      dir_setup(c, sj * cph[l], sj * sph[l], ct[j], d);
+      const double w = wc[j] * wph[l];
+      First<C4> f;
+      first_zero<C4>(f);
+      const double4* rad4 = reinterpret_cast<const double4*>(rad);
+#pragma unroll 2
+      for (int i = 0; i < P.n_r; ++i) {
+        const double4 q = rad4[i];
+        node<NREG, C4>(P, c, d, q.x, q.y, q.z, f);
+      }
+      second_level<C4>(f, d, w, acc + lane);
+    }
+    __syncwarp();
+
+    // ---- a3: reduce the moments over the 32 lanes (fixed order) ----
+    for (int row = lane; row < L::kRows; row += kLanes) {
+      double s = 0.0;
+#pragma unroll 8
+      for (int t = 0; t < kLanes; ++t) s += acc[row * kLanes + ((lane + t) & 31)];
+      mom[row] = s;
+    }
+    __syncwarp();
+
+    // ---- a4: epilogue, phases 1 and 2 (records live in the dead accumulator area) ----
+    double* rec = acc;
+    if (lane < 6) phase1_job<C4>(P, c, mom, lane, rec);
+    __syncwarp();
+    phase2_lane(rec, lane, P.nsp[pass], P.esum[pass], NREG >= 0 ? exp(-c.E0) : 1.0, blk);
+    __syncwarp();
+  }
+
+  // ---- a4: phase 3, (1 - P12) and expansion to the 16x16 complex matrix ----
+  double* coef = acc;
+#pragma unroll
+  for (int b = 0; b < 6; ++b) coef[lane * 6 + b] = blk[b];
+  __syncwarp();
+  double2* o = reinterpret_cast<double2*>(out) + ic * 256;
+#pragma unroll 1
+  for (int it = 0; it < 8; ++it) {
+    const int row = 2 * it + (lane >> 4), col = lane & 15;
+    double re, im;
+    phase3_elem(coef, row, col, re, im);
+    o[row * 16 + col] = make_double2(re, im);
+  }
+}
+
+// ---- FP64 roofline probe: 16 independent DFMA chains per thread ----
+__global__ void __launch_bounds__(256) dfma_probe_kernel(double* sink, int iters, double seed) {
+  double a[16];
+#pragma unroll
+  for (int k = 0; k < 16; ++k) a[k] = seed + k + threadIdx.x;
+  const double x = 1.0 - 1e-9 * seed, y = 1e-9;
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int k = 0; k < 16; ++k) a[k] = fma(a[k], x, y);
+  }
+  double s = 0;
+#pragma unroll
+  for (int k = 0; k < 16; ++k) s += a[k];
+  if (s == 123.456) sink[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+}  // namespace no3n

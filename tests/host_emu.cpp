@@ -1,0 +1,154 @@
+// tests/host_emu.cpp -- lane-by-lane HOST emulation of the CUDA kernel's warp program, for the CPU
+// unit tests only (tests/test_host_logic.py).  It compiles the kernel's own arithmetic
+// (paper_2603_24532_b200/csrc/no_core.h, no_host.h) with g++ and walks the 32 lanes of one warp
+// sequentially through the same phases, in the same order, as no3n_kernel in no_kernel.cuh.
+// It is NOT part of the product library and is never loaded by the package: the product has no
+// CPU path.  It lets the host logic (tables, kernel-variant choice, moment algebra, epilogue) be
+// checked against the oracle on a machine without a GPU.
+#include <cstring>
+#include <vector>
+
+#include "../paper_2603_24532_b200/csrc/no_host.h"
+
+using namespace no3n;
+
+template <int NREG, bool C4>
+static void emu_cfg(const HostPlan& plan, const double* cfg, double* out /*[512]*/) {
+  using L = Layout<C4>;
+  const DevParams& P = plan.dp;
+  CfgConst c;
+  cfg_setup<NREG>(P, cfg, c);
+  std::vector<double> acc(L::kRows * kLanes), mom(L::kRows), rec(kRecDoubles), coef(32 * 6, 0.0);
+  for (int pass = 0; pass < P.n_pass; ++pass) {
+    const double* rad = plan.tab.data() + P.pass_off[pass];
+    const double* ct = rad + 4 * P.n_r;
+    const double* st = ct + P.n_cos;
+    const double* wc = st + P.n_cos;
+    const double* cph = wc + P.n_cos;
+    const double* sph = cph + P.n_phi;
+    const double* wph = sph + P.n_phi;
+    std::fill(acc.begin(), acc.end(), 0.0);
+    const int n_dir = P.n_cos * P.n_phi;
+    for (int lane = 0; lane < kLanes; ++lane) {
+      for (int m = lane; m < n_dir; m += kLanes) {
+        const int j = m / P.n_phi, l = m - j * P.n_phi;
+        DirConst d;
+        dir_setup(c, st[j] * cph[l], st[j] * sph[l], ct[j], d);
+        const double w = wc[j] * wph[l];
+        First<C4> f;
+        first_zero<C4>(f);
+        for (int i = 0; i < P.n_r; ++i) node<NREG, C4>(P, c, d, rad[4 * i], rad[4 * i + 1], rad[4 * i + 2], f);
+        second_level<C4>(f, d, w, acc.data() + lane);
+      }
+    }
+    for (int lane = 0; lane < kLanes; ++lane)
+      for (int row = lane; row < L::kRows; row += kLanes) {
+        double s = 0.0;
+        for (int t = 0; t < kLanes; ++t) s += acc[row * kLanes + ((lane + t) & 31)];
+        mom[row] = s;
+      }
+    for (int lane = 0; lane < 6; ++lane) phase1_job<C4>(P, c, mom.data(), lane, rec.data());
+    for (int lane = 0; lane < kLanes; ++lane)
+      phase2_lane(rec.data(), lane, P.nsp[pass], P.esum[pass], NREG >= 0 ? exp(-c.E0) : 1.0, &coef[lane * 6]);
+  }
+  for (int lane = 0; lane < kLanes; ++lane)
+    for (int it = 0; it < 8; ++it) {
+      const int row = 2 * it + (lane >> 4), col = lane & 15;
+      double re, im;
+      phase3_elem(coef.data(), row, col, re, im);
+      out[2 * (row * 16 + col)] = re;
+      out[2 * (row * 16 + col) + 1] = im;
+    }
+}
+
+template <bool C4>
+static void emu_dispatch(const HostPlan& plan, const double* cfg, double* out) {
+  switch (plan.nreg_variant) {
+    case -1: emu_cfg<-1, C4>(plan, cfg, out); break;
+    case 1: emu_cfg<1, C4>(plan, cfg, out); break;
+    case 2: emu_cfg<2, C4>(plan, cfg, out); break;
+    case 3: emu_cfg<3, C4>(plan, cfg, out); break;
+    case 4: emu_cfg<4, C4>(plan, cfg, out); break;
+    default: emu_cfg<0, C4>(plan, cfg, out); break;
+  }
+}
+
+extern "C" {
+
+int emu_eval(const no_params* p, const double* cfg, long long n_cfg, double* out) {
+  HostPlan plan;
+  const int rc = build_plan(p, plan);
+  if (rc != NO_OK) return rc;
+  for (long long i = 0; i < n_cfg; ++i) {
+    if (plan.has_c4) emu_dispatch<true>(plan, cfg + 9 * i, out + 512 * i);
+    else emu_dispatch<false>(plan, cfg + 9 * i, out + 512 * i);
+  }
+  return NO_OK;
+}
+
+// plan facts for the host-logic tests
+int emu_plan(const no_params* p, int* n_pass, int* nreg_variant, int* has_c4, long long* evals_per_cfg,
+             int* tab_doubles, double* tab_out, int tab_cap) {
+  HostPlan plan;
+  const int rc = build_plan(p, plan);
+  if (rc != NO_OK) return rc;
+  *n_pass = plan.dp.n_pass;
+  *nreg_variant = plan.nreg_variant;
+  *has_c4 = plan.has_c4 ? 1 : 0;
+  *evals_per_cfg = plan.evals_per_cfg;
+  *tab_doubles = plan.dp.tab_doubles;
+  for (int i = 0; i < plan.dp.tab_doubles && i < tab_cap; ++i) tab_out[i] = plan.tab[i];
+  return NO_OK;
+}
+
+void emu_gl_rule(int n, double lo, double hi, double* x, double* w) {
+  std::vector<double> xs, ws;
+  gl_rule(n, lo, hi, xs, ws);
+  for (int i = 0; i < n; ++i) { x[i] = xs[i]; w[i] = ws[i]; }
+}
+
+}  // extern "C"
+
+// debugging aid: reduced moments of one pass (c4 layout not supported)
+extern "C" int emu_moments(const no_params* p, const double* cfg, int pass, double* mom_out) {
+  HostPlan plan;
+  const int rc = build_plan(p, plan);
+  if (rc != NO_OK) return rc;
+  using L = Layout<false>;
+  const DevParams& P = plan.dp;
+  CfgConst c;
+  cfg_setup<-1>(P, cfg, c);
+  std::vector<double> acc(L::kRows * kLanes, 0.0);
+  const double* rad = plan.tab.data() + P.pass_off[pass];
+  const double* ct = rad + 4 * P.n_r;
+  const double* st = ct + P.n_cos;
+  const double* wc = st + P.n_cos;
+  const double* cph = wc + P.n_cos;
+  const double* sph = cph + P.n_phi;
+  const double* wph = sph + P.n_phi;
+  for (int m = 0; m < P.n_cos * P.n_phi; ++m) {
+    const int j = m / P.n_phi, l = m - j * P.n_phi;
+    DirConst d;
+    dir_setup(c, st[j] * cph[l], st[j] * sph[l], ct[j], d);
+    First<false> f;
+    first_zero<false>(f);
+    for (int i = 0; i < P.n_r; ++i) node<-1, false>(P, c, d, rad[4 * i], rad[4 * i + 1], rad[4 * i + 2], f);
+    second_level<false>(f, d, wc[j] * wph[l], acc.data() + (m & 31));
+  }
+  for (int row = 0; row < L::kRows; ++row) {
+    double s = 0;
+    for (int t = 0; t < kLanes; ++t) s += acc[row * kLanes + t];
+    mom_out[row] = s;
+  }
+  return NO_OK;
+}
+
+extern "C" int emu_records(const no_params* p, const double* cfg, const double* mom, double* rec_out) {
+  HostPlan plan;
+  const int rc = build_plan(p, plan);
+  if (rc != NO_OK) return rc;
+  CfgConst c;
+  cfg_setup<-1>(plan.dp, cfg, c);
+  for (int lane = 0; lane < 6; ++lane) phase1_job<false>(plan.dp, c, mom, lane, rec_out);
+  return NO_OK;
+}

@@ -1,0 +1,141 @@
+"""Host logic of the product, checked on the CPU: quadrature tables, kernel-variant choice, the seeded
+workloads, and -- through tests/host_emu.cpp, which compiles the kernel's own arithmetic
+(csrc/no_core.h) with g++ and walks one warp lane by lane -- the factored moment formulation and the
+epilogue against the oracle.  The emulation is test-only; the product has no CPU path."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2603_24532_b200 import workloads as W
+from tests import emu
+
+PHYS = dict(c1=-0.81, c3=-3.2, c4=0.0, cD=1.0, cE=-0.5, gA=1.27, fpi=92.4, mpi=138.04, lambda_chi=700.0,
+            Lambda=500.0, n_reg=4)
+REL_TOL = 1e-10      # north_star: max relative error on every element ...
+MAG_FLOOR = 1e-12    # ... whose magnitude exceeds 1e-12 of the matrix maximum
+
+
+def check_parity(got, want):
+    mx = np.abs(want).max(axis=(1, 2), keepdims=True)
+    mask = np.abs(want) > MAG_FLOOR * mx
+    rel = np.abs(got - want)[mask] / np.abs(want)[mask]
+    assert rel.max() < REL_TOL, rel.max()
+    assert (np.abs(got)[~mask] <= MAG_FLOOR * np.broadcast_to(mx, got.shape)[~mask]).all()
+    return rel.max()
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 5, 16, 31, 32, 40, 48, 64, 127, 128])
+def test_product_gauss_legendre_rule(n):
+    x, w = emu.emu_gl_rule(n, -1.0, 1.0)
+    xo, wo = O.gauss_legendre(n, -1.0, 1.0)             # independent implementation (oracle)
+    assert np.abs(x - xo).max() <= 2.3e-16
+    assert np.abs(w - wo).max() <= 1e-16 + 4e-16 * wo.max()
+    assert np.array_equal(x, -x[::-1]) and np.array_equal(w, w[::-1])
+    assert abs(math.fsum(w) - 2.0) < 4e-16
+    k = 2 * n - 2
+    assert abs(math.fsum(w * x ** k) - 2.0 / (k + 1)) < 4e-16
+    x, w = emu.emu_gl_rule(n, 0.0, 2 * math.pi)
+    assert abs(w.sum() - 2 * math.pi) < 4e-15 and x.min() > 0 and x.max() < 2 * math.pi
+
+
+def test_plan_passes_variants_and_tables():
+    base = dict(PHYS, n_r=3, n_cos=4, n_phi=5)
+    p = emu.emu_plan(kf_n=1.2, kf_p=0.9, **base)
+    assert (p["n_pass"], p["nreg_variant"], p["has_c4"], p["evals_per_cfg"]) == (2, 4, 0, 2 * 60)
+    per = 4 * 3 + 3 * 4 + 3 * 5
+    assert p["tab_doubles"] == 2 * per + (2 * per) % 2
+    r, wr = O.gauss_legendre(3, 0.0, 0.9)               # pass 0 = protons
+    t = p["tab"]
+    assert np.allclose(t[0:12:4], r, rtol=0, atol=3e-16)
+    assert np.allclose(t[1:12:4], r * r, rtol=1e-15)
+    assert np.allclose(t[2:12:4], wr * r * r / (2 * math.pi) ** 3, rtol=1e-14)
+    x, wx = O.gauss_legendre(4, -1.0, 1.0)
+    assert np.allclose(t[12:16], x, atol=3e-16) and np.allclose(t[16:20], np.sqrt(1 - x * x), atol=3e-16)
+    assert np.allclose(t[20:24], wx, rtol=1e-14)
+    ph, wp = O.gauss_legendre(5, 0.0, 2 * math.pi)
+    assert np.allclose(t[24:29], np.cos(ph), atol=1e-15) and np.allclose(t[29:34], np.sin(ph), atol=1e-15)
+    assert np.allclose(t[34:39], wp, rtol=1e-14)
+    rn, _ = O.gauss_legendre(3, 0.0, 1.2)               # pass 1 = neutrons
+    assert np.allclose(t[per:per + 12:4], rn, atol=3e-16)
+    # equal Fermi momenta share one grid; empty spheres are skipped; regulator variants
+    assert emu.emu_plan(kf_n=1.3, kf_p=1.3, **base)["n_pass"] == 1
+    assert emu.emu_plan(kf_n=1.3, kf_p=1.3, **base)["evals_per_cfg"] == 60
+    assert emu.emu_plan(kf_n=1.3, kf_p=0.0, **base)["n_pass"] == 1
+    assert emu.emu_plan(kf_n=0.0, kf_p=0.0, **base)["n_pass"] == 0
+    assert emu.emu_plan(kf_n=1.0, kf_p=0.0, **dict(base, Lambda=-1.0))["nreg_variant"] == -1
+    assert emu.emu_plan(kf_n=1.0, kf_p=0.0, **dict(base, n_reg=3))["nreg_variant"] == 3
+    assert emu.emu_plan(kf_n=1.0, kf_p=0.0, **dict(base, n_reg=7))["nreg_variant"] == 0
+    assert emu.emu_plan(kf_n=1.0, kf_p=0.0, **dict(base, c4=5.4))["has_c4"] == 1
+    with pytest.raises(ValueError):
+        emu.emu_plan(kf_n=-1.0, kf_p=0.0, **base)
+
+
+GEOS = [dict(kf_n=1.2, kf_p=0.9), dict(kf_n=1.0, kf_p=0.0), dict(kf_n=1.33, kf_p=1.33), dict(kf_n=0.0, kf_p=0.8),
+        dict(kf_n=1.4, kf_p=0.8, Lambda=450.0, n_reg=3), dict(kf_n=1.4, kf_p=0.8, Lambda=-1.0),
+        dict(kf_n=1.4, kf_p=0.8, Lambda=600.0, n_reg=6), dict(kf_n=1.4, kf_p=0.8, Lambda=400.0, n_reg=2),
+        dict(kf_n=1.4, kf_p=0.8, Lambda=400.0, n_reg=1)]
+
+
+@pytest.mark.parametrize("c4", [0.0, 5.4])
+@pytest.mark.parametrize("geo", GEOS)
+def test_kernel_arithmetic_matches_oracle(geo, c4):
+    rng = np.random.default_rng(5)
+    kw = dict(PHYS, c4=c4, n_r=6, n_cos=7, n_phi=8)      # 56 directions: ragged over 32 lanes
+    kw.update(geo)
+    cfg = rng.uniform(-1, 1, (3, 9)) * 1.5
+    check_parity(emu.emu_eval(cfg, **kw), O.normal_order(cfg, **kw))
+
+
+def test_kernel_arithmetic_on_the_cfg1_distribution():
+    """p, p' up to 4 fm^-1: regulators down to 1e-100; parity is per matrix (reading R18)."""
+    run = W.workload("cfg1").runs[0].shrunk(24, 8)
+    cfg = run.configurations()
+    want = O.normal_order(cfg, **run.params())
+    assert np.abs(want).max(axis=(1, 2)).min() < 1e-12      # some matrices are tiny in absolute terms
+    check_parity(emu.emu_eval(cfg, **run.params()), want)
+
+
+def test_empty_fermi_sea_gives_zero():
+    out = emu.emu_eval(np.ones((2, 9)), kf_n=0.0, kf_p=0.0, n_r=2, n_cos=2, n_phi=2, **PHYS)
+    assert np.count_nonzero(out) == 0
+
+
+# ----------------------------------------------------------------------------------------------
+# seeded synthetic workloads
+# ----------------------------------------------------------------------------------------------
+def test_workload_tables_match_baseline():
+    evals = {n: W.workload(n).evals for n in ("cfg1", "cfg2", "cfg3", "cfg4", "cfg5")}
+    assert evals["cfg1"] == 256 * 16 ** 3
+    assert evals["cfg2"] == 12 * 8192 * 32 ** 3
+    assert evals["cfg3"] == 65536 * 40 ** 3
+    assert evals["cfg4"] == 131072 * 48 ** 3 * 2
+    assert evals["cfg5"] == (1 << 20) * 64 ** 3 + (1 << 18) * 64 ** 3 * (1 + 2 + 2 + 2 + 1)
+    r = W.workload("cfg4").runs[0]
+    assert r.kf_n == pytest.approx(1.621540614038, abs=1e-11) and r.kf_p == pytest.approx(0.779555417944, abs=1e-11)
+    assert (r.Lambda, r.n_reg, r.n_sph) == (450.0, 3, 2)
+    kfs = [(q.kf_n, q.kf_p) for q in W.workload("cfg5").runs[1:]]
+    want = [(2.116038959580, 0.0), (2.080166962512, 0.779555417944), (2.043013152886, 0.982178280627),
+            (1.964356561255, 1.237467090512), (1.679501235221, 1.679501235221)]
+    assert np.allclose(kfs, want, atol=1e-11)
+    assert [q.n_sph for q in W.workload("cfg5").runs] == [1, 1, 2, 2, 2, 1]
+    assert all(q.c4 == 0.0 for n in ("cfg1", "cfg2", "cfg3", "cfg4", "cfg5") for q in W.workload(n).runs)
+
+
+def test_seeded_configurations_are_reproducible_and_in_range():
+    r = W.workload("cfg2").runs[5]
+    a = r.configurations(1000)
+    assert np.array_equal(a, r.configurations(1000))
+    assert np.array_equal(a[:100], r.configurations(100))              # a prefix of the same stream
+    assert not np.array_equal(a[:100], W.workload("cfg2").runs[4].configurations(100))
+    pn = np.linalg.norm(a[:, 0:3], axis=1)
+    ppn = np.linalg.norm(a[:, 3:6], axis=1)
+    Pn = np.linalg.norm(a[:, 6:9], axis=1)
+    assert pn.max() < 4.0 and ppn.max() < 4.0 and Pn.max() < 2 * r.kf_n
+    # uniform in the ball: <r^2>/R^2 = 3/5
+    assert np.mean(pn ** 2) / 16.0 == pytest.approx(0.6, abs=0.03)
+    assert np.mean(Pn ** 2) / (2 * r.kf_n) ** 2 == pytest.approx(0.6, abs=0.03)
+    d = W.splitmix64_doubles(0, 0, 0, 5)
+    assert np.array_equal(d, W.splitmix64_doubles(0, 0, 0, 8)[:5]) and (0 <= d).all() and (d < 1).all()
+    assert np.array_equal(W.splitmix64_doubles(0, 0, 3, 2), W.splitmix64_doubles(0, 0, 0, 8)[3:5])

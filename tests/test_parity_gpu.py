@@ -1,0 +1,244 @@
+"""Parity of the CUDA path (libno3n.so through the C ABI) with the CPU oracle, element by element on
+the same seeded inputs.  Tolerance (north_star, BASELINE.json): maximum relative error 1e-10 on every
+element whose magnitude exceeds 1e-12 of its matrix maximum; structural zeros must be below that floor.
+All tests here need a B200 (`-m gpu`)."""
+import ctypes
+import os
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from oracle import oracle as O                                   # noqa: E402
+from paper_2603_24532_b200 import NormalOrdering, binding, build, workloads as W   # noqa: E402
+
+pytestmark = pytest.mark.gpu
+
+REL_TOL = 1e-10
+MAG_FLOOR = 1e-12
+PHYS = dict(c1=-0.81, c3=-3.2, c4=0.0, cD=1.0, cE=-0.5, gA=1.27, fpi=92.4, mpi=138.04, lambda_chi=700.0,
+            Lambda=500.0, n_reg=4)
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    build.build()
+    binding.load()
+
+
+def gpu_eval(cfg, **params):
+    no = NormalOrdering(device=0, **params)
+    out = no(torch.from_numpy(np.ascontiguousarray(cfg)).cuda())
+    torch.cuda.synchronize()
+    res = out.cpu().numpy()
+    no.close()
+    return res
+
+
+def check_parity(got, want, label=""):
+    mx = np.abs(want).max(axis=(1, 2), keepdims=True)
+    mask = np.abs(want) > MAG_FLOOR * mx
+    rel = np.abs(got - want)[mask] / np.abs(want)[mask]
+    worst = rel.max() if rel.size else 0.0
+    assert worst < REL_TOL, f"{label}: max rel err {worst:.3e}"
+    floor = np.broadcast_to(MAG_FLOOR * mx, got.shape)
+    assert (np.abs(got)[~mask] <= floor[~mask]).all(), f"{label}: structural zero above the floor"
+    return worst
+
+
+def sample_indices(n, k):
+    """first k/2 and k/2 evenly strided configurations."""
+    head = list(range(min(k // 2, n)))
+    stride = [int(i) for i in np.linspace(0, n - 1, k - len(head))] if n > len(head) else []
+    return sorted(set(head + stride))
+
+
+# ----------------------------------------------------------------------------------------------
+# config 1 in full; configs 2-5 at full size with sampled outputs; extra c4 case (R2)
+# ----------------------------------------------------------------------------------------------
+def test_cfg1_all_configurations():
+    run = W.workload("cfg1").runs[0]
+    cfg = run.configurations()
+    got = gpu_eval(cfg, **run.params())
+    want = O.normal_order(cfg, **run.params())
+    worst = check_parity(got, want, "cfg1")
+    nn = [3, 7, 11, 15]
+    assert np.abs(got[:, nn][:, :, nn]).max() > 0            # c1/c3 survive in the nn block of PNM
+    print(f"cfg1: 256 configurations, max rel err {worst:.2e}")
+
+
+FULL_SIZE = [("cfg2", 4), ("cfg3", 8), ("cfg4", 4), ("cfg5", 2)]
+
+
+@pytest.mark.parametrize("name,n_sample", FULL_SIZE)
+def test_full_size_launch_sampled_outputs(name, n_sample):
+    """The launch bench.py times (all configurations of every run, full k3 grid); the oracle computes
+    the sampled matrices one by one."""
+    for run in W.workload(name).runs:
+        cfg = run.configurations()
+        no = NormalOrdering(device=0, **run.params())
+        d_cfg = torch.from_numpy(cfg).cuda()
+        out = torch.empty((run.n_cfg, 16, 16, 2), dtype=torch.float64, device="cuda")
+        no.eval_into(d_cfg, out)
+        torch.cuda.synchronize()
+        assert no.evals_per_cfg == run.nodes_per_cfg
+        idx = sample_indices(run.n_cfg, n_sample)
+        got = torch.view_as_complex(out[idx]).cpu().numpy()
+        want = O.normal_order(cfg[idx], **run.params())
+        worst = check_parity(got, want, run.name)
+        # properties that hold at any size, on a 1% subsample of the whole launch (P4, P5, P6)
+        sub = np.arange(0, run.n_cfg, 100)
+        M = torch.view_as_complex(out[sub]).cpu().numpy()
+        assert np.isfinite(M.view(np.float64)).all()
+        allowed = np.array([[((r >> 1) & 1) + (r & 1) == ((c >> 1) & 1) + (c & 1) for c in range(16)]
+                            for r in range(16)])
+        assert np.count_nonzero(M[:, ~allowed]) == 0
+        swapped = cfg[sub].copy()
+        swapped[:, 0:3], swapped[:, 3:6] = cfg[sub][:, 3:6], cfg[sub][:, 0:3]
+        Mt = no(torch.from_numpy(swapped).cuda()).cpu().numpy()
+        mx = np.abs(M).max(axis=(1, 2), keepdims=True)
+        assert (np.abs(M - np.conj(np.swapaxes(Mt, 1, 2))) <= 1e-12 * mx).all(), run.name   # Hermiticity
+        flipped = cfg[sub].copy()
+        flipped[:, 3:6] *= -1
+        Mf = no(torch.from_numpy(flipped).cuda()).cpu().numpy()
+        assert (np.abs(_p12() @ Mf + M) <= 1e-12 * mx).all(), run.name                        # antisymmetry
+        no.close()
+        del out, d_cfg
+        torch.cuda.empty_cache()
+        print(f"{run.name}: {run.n_cfg} configurations x {run.nodes_per_cfg} nodes, "
+              f"{len(idx)} sampled, max rel err {worst:.2e}")
+
+
+def _p12():
+    P = np.zeros((16, 16))
+    for s1 in range(2):
+        for s2 in range(2):
+            for t1 in range(2):
+                for t2 in range(2):
+                    P[8 * s2 + 4 * s1 + 2 * t2 + t1, 8 * s1 + 4 * s2 + 2 * t1 + t2] = 1.0
+    return P
+
+
+def test_c4_topology_extra_case():
+    run = W.workload("c4").runs[0]
+    cfg = run.configurations()
+    got = gpu_eval(cfg, **run.params())
+    idx = sample_indices(run.n_cfg, 32)
+    want = O.normal_order(cfg[idx], **run.params())
+    check_parity(got[idx], want, "c4")
+    without = O.normal_order(cfg[idx[:2]], **dict(run.params(), c4=0.0))
+    assert np.abs(without - want[:2]).max() > 1e-3 * np.abs(want[:2]).max()     # the term is exercised
+
+
+# ----------------------------------------------------------------------------------------------
+# edge cases
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n_cfg", [0, 1, 3, 4, 5, 7, 130])
+def test_ragged_batch_sizes(n_cfg):
+    """4 configurations per CTA: every remainder, plus the empty batch."""
+    run = W.workload("cfg4").runs[0].shrunk(n_cfg, 6)
+    cfg = run.configurations()
+    got = gpu_eval(cfg, **run.params())
+    assert got.shape == (n_cfg, 16, 16)
+    if n_cfg:
+        check_parity(got, O.normal_order(cfg, **run.params()), f"n_cfg={n_cfg}")
+
+
+@pytest.mark.parametrize("orders", [(5, 7, 3), (1, 1, 1), (2, 33, 1), (3, 5, 13), (128, 3, 2), (2, 128, 2), (2, 2, 128)])
+def test_ragged_and_maximum_quadrature_orders(orders):
+    """direction counts that do not fill the 32 lanes, single-node rules, the maximum order per axis."""
+    n_r, n_cos, n_phi = orders
+    kw = dict(PHYS, kf_n=1.3, kf_p=0.9, n_r=n_r, n_cos=n_cos, n_phi=n_phi)
+    cfg = W.momentum_configurations(3, 1, 6, 1.5, 2.0)
+    check_parity(gpu_eval(cfg, **kw), O.normal_order(cfg, **kw), str(orders))
+
+
+@pytest.mark.parametrize("geo", [dict(kf_n=1.0, kf_p=0.0), dict(kf_n=0.0, kf_p=0.8), dict(kf_n=1.33, kf_p=1.33),
+                                 dict(kf_n=1.4, kf_p=0.8, Lambda=-1.0), dict(kf_n=1.4, kf_p=0.8, Lambda=400.0, n_reg=1),
+                                 dict(kf_n=1.4, kf_p=0.8, Lambda=400.0, n_reg=2), dict(kf_n=1.4, kf_p=0.8, Lambda=450.0, n_reg=3),
+                                 dict(kf_n=1.4, kf_p=0.8, Lambda=600.0, n_reg=6), dict(kf_n=1.4, kf_p=0.8, Lambda=700.0, n_reg=12)])
+@pytest.mark.parametrize("c4", [0.0, 5.4])
+def test_every_kernel_variant(geo, c4):
+    """all regulator variants (unregulated, n = 1..4 unrolled, generic) x (c4 = 0, c4 != 0), each matter type."""
+    kw = dict(PHYS, c4=c4, n_r=6, n_cos=7, n_phi=8)
+    kw.update(geo)
+    cfg = W.momentum_configurations(5, 2, 9, 1.5, 2.0)
+    check_parity(gpu_eval(cfg, **kw), O.normal_order(cfg, **kw), f"{geo} c4={c4}")
+
+
+def test_degenerate_inputs():
+    kw = dict(PHYS, kf_n=1.2, kf_p=0.9, n_r=4, n_cos=4, n_phi=4)
+    # empty Fermi sea: exactly zero
+    assert np.count_nonzero(gpu_eval(np.ones((5, 9)), **dict(kw, kf_n=0.0, kf_p=0.0))) == 0
+    # p = p' (forward), P = 0, p = 0: finite and equal to the oracle
+    cfg = np.zeros((4, 9))
+    cfg[0, 0:3] = cfg[0, 3:6] = (0.3, -0.2, 0.5)
+    cfg[1, 0:3] = (0.4, 0.1, -0.2)
+    cfg[1, 3:6] = (-0.4, -0.1, 0.2)                     # p' = -p
+    cfg[2, 6:9] = (0.2, 0.1, -0.3)                      # p = p' = 0
+    check_parity(gpu_eval(cfg[:3], **kw), O.normal_order(cfg[:3], **kw), "degenerate")
+    # everything zero: the pion-exchange terms vanish, the contact term survives
+    got = gpu_eval(cfg[3:], **kw)
+    check_parity(got, O.normal_order(cfg[3:], **kw), "all-zero momenta")
+    # non-finite inputs propagate (no checking on the hot path), neighbours are untouched
+    bad = W.momentum_configurations(1, 1, 3, 1.0, 1.0)
+    good = gpu_eval(bad, **kw)
+    bad2 = bad.copy()
+    bad2[1, 4] = np.nan
+    out = gpu_eval(bad2, **kw)
+    assert not np.isfinite(out[1].view(np.float64)).all()
+    assert np.array_equal(out[0], good[0]) and np.array_equal(out[2], good[2])
+
+
+def test_abi_pointer_checks_streams_and_host_path():
+    run = W.workload("cfg3").runs[0].shrunk(37, 8)
+    cfg = run.configurations()
+    h = binding.no_init(device=0, **run.params())
+    lib = binding.load()
+    d_cfg = torch.from_numpy(cfg).cuda()
+    out = torch.zeros((37, 16, 16, 2), dtype=torch.float64, device="cuda")
+    s = torch.cuda.current_stream().cuda_stream
+    vp = ctypes.c_void_p
+    assert lib.no_eval(h, vp(d_cfg.data_ptr() + 4), 37, vp(out.data_ptr()), vp(s)) == binding.NO_ERR_INVALID
+    assert lib.no_eval(h, vp(d_cfg.data_ptr()), 37, vp(out.data_ptr() + 8), vp(s)) == binding.NO_ERR_INVALID
+    assert lib.no_eval(h, vp(d_cfg.data_ptr()), -1, vp(out.data_ptr()), vp(s)) == binding.NO_ERR_INVALID
+    assert lib.no_eval(h, None, 5, vp(out.data_ptr()), vp(s)) == binding.NO_ERR_INVALID
+    assert lib.no_eval(h, None, 0, None, vp(s)) == binding.NO_OK
+    assert int(out.abs().sum().item()) == 0                      # nothing was written by the failed calls
+    # default stream
+    binding.no_eval(h, d_cfg.data_ptr(), 37, out.data_ptr(), None)
+    torch.cuda.synchronize()
+    ref = out.clone()
+    # two user streams at once on one handle (threads time-share the GPU via streams)
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    o1, o2 = torch.empty_like(out), torch.empty_like(out)
+    binding.no_eval(h, d_cfg.data_ptr(), 37, o1.data_ptr(), s1.cuda_stream)
+    binding.no_eval(h, d_cfg.data_ptr(), 37, o2.data_ptr(), s2.cuda_stream)
+    torch.cuda.synchronize()
+    assert torch.equal(o1, ref) and torch.equal(o2, ref)         # bit-identical: fixed summation order
+    # host-buffer path
+    h_out = np.empty((37, 16, 16, 2))
+    binding.no_eval_host(h, cfg.ctypes.data, 37, h_out.ctypes.data, None)
+    assert np.array_equal(h_out, ref.cpu().numpy())
+    binding.no_eval_host(h, cfg.ctypes.data, 5, h_out.ctypes.data, s1.cuda_stream)   # smaller batch reuses scratch
+    assert np.array_equal(h_out[:5], ref[:5].cpu().numpy())
+    info = binding.no_kernel_info(h)
+    assert info["threads"] == 128 and info["cfg_per_cta"] == 4 and info["ctas_per_sm"] >= 1 and info["n_sm"] > 0
+    assert binding.no_evals_per_cfg(h) == 8 ** 3
+    binding.no_free(h)
+    check_parity(torch.view_as_complex(ref).cpu().numpy(), O.normal_order(cfg, **run.params()), "streams")
+    with pytest.raises(binding.NoError):
+        binding.no_init(device=99, **run.params())
+
+
+def test_fp64_probe_reports_a_sane_peak():
+    r = binding.no_probe_fp64_peak(0, 100)
+    assert r["n_sm"] > 0 and 1.0 < r["tflops"] < 100.0
+    print("FP64 DFMA probe:", r)
+
+
+def test_native_library_is_the_one_loaded():
+    maps = open(f"/proc/{os.getpid()}/maps").read()
+    assert "libno3n.so" in maps
