@@ -57,7 +57,8 @@ struct DevParams {
 
 // table layout of one pass: radial nodes as [n_r][4] = (r, r^2, w_r r^2/(2 pi)^3, 0), then
 // cos(theta)[n_cos], sin(theta)[n_cos], w_cos[n_cos], cos(phi)[n_phi], sin(phi)[n_phi], w_phi[n_phi]
-NO_HD int tab_pass_doubles(int n_r, int n_cos, int n_phi) { return 4 * n_r + 3 * n_cos + 3 * n_phi; }
+// (padded to a multiple of 4 doubles so that every pass's radial block stays 32-byte aligned)
+NO_HD int tab_pass_doubles(int n_r, int n_cos, int n_phi) { return (4 * n_r + 3 * n_cos + 3 * n_phi + 3) & ~3; }
 
 // second-level accumulator rows
 template <bool C4> struct Layout {

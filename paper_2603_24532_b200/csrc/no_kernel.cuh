@@ -55,7 +55,7 @@ inline size_t smem_bytes(int tab_doubles, int warps) {
 template <int NREG, bool C4, int WARPS, int MINB>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
 no3n_kernel(const DevParams P, const double* __restrict__ cfg, long long n_cfg, double* __restrict__ out) {
-  extern __shared__ __align__(16) double smem[];
+  extern __shared__ __align__(128) double smem[];
   using L = Layout<C4>;
   double* s_tab = smem;
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem + P.tab_doubles);

@@ -44,8 +44,8 @@ def test_plan_passes_variants_and_tables():
     base = dict(PHYS, n_r=3, n_cos=4, n_phi=5)
     p = emu.emu_plan(kf_n=1.2, kf_p=0.9, **base)
     assert (p["n_pass"], p["nreg_variant"], p["has_c4"], p["evals_per_cfg"]) == (2, 4, 0, 2 * 60)
-    per = 4 * 3 + 3 * 4 + 3 * 5
-    assert p["tab_doubles"] == 2 * per + (2 * per) % 2
+    per = (4 * 3 + 3 * 4 + 3 * 5 + 3) // 4 * 4          # each pass padded to 32 bytes
+    assert p["tab_doubles"] == 2 * per
     r, wr = O.gauss_legendre(3, 0.0, 0.9)               # pass 0 = protons
     t = p["tab"]
     assert np.allclose(t[0:12:4], r, rtol=0, atol=3e-16)
