@@ -28,7 +28,8 @@ int cuda_fail(cudaError_t e, const char* where) {
     if (e_ != cudaSuccess) return cuda_fail(e_, #call); \
   } while (0)
 
-constexpr int kWarps = 4;   // configurations per CTA
+constexpr int kWarps = 2;       // configurations per CTA
+constexpr int kMinBlocks = 6;   // resident CTAs per SM the register allocation must allow
 
 typedef void (*KernelFn)(const DevParams, const double*, long long, double*);
 
@@ -38,22 +39,22 @@ struct Variant {
 };
 
 template <int NREG, bool C4>
-Variant make_variant(int tab_doubles) {
+Variant make_variant(int tab_doubles, int n_r_pad) {
   Variant v;
-  v.fn = no3n_kernel<NREG, C4, kWarps, C4 ? 2 : 3>;
-  v.smem = smem_bytes<C4>(tab_doubles, kWarps);
+  v.fn = no3n_kernel<NREG, C4, kWarps, kMinBlocks>;
+  v.smem = smem_bytes<C4>(tab_doubles, n_r_pad, kWarps);
   return v;
 }
 
 template <bool C4>
-Variant pick_nreg(int nreg, int tab_doubles) {
+Variant pick_nreg(int nreg, int tab_doubles, int n_r_pad) {
   switch (nreg) {
-    case -1: return make_variant<-1, C4>(tab_doubles);
-    case 1: return make_variant<1, C4>(tab_doubles);
-    case 2: return make_variant<2, C4>(tab_doubles);
-    case 3: return make_variant<3, C4>(tab_doubles);
-    case 4: return make_variant<4, C4>(tab_doubles);
-    default: return make_variant<0, C4>(tab_doubles);
+    case -1: return make_variant<-1, C4>(tab_doubles, n_r_pad);
+    case 1: return make_variant<1, C4>(tab_doubles, n_r_pad);
+    case 2: return make_variant<2, C4>(tab_doubles, n_r_pad);
+    case 3: return make_variant<3, C4>(tab_doubles, n_r_pad);
+    case 4: return make_variant<4, C4>(tab_doubles, n_r_pad);
+    default: return make_variant<0, C4>(tab_doubles, n_r_pad);
   }
 }
 
@@ -111,8 +112,8 @@ int no_init(no_handle** out, const no_params* p) {
   h->device = p->device;
   DeviceGuard guard(h->device);
   if (!guard.ok) { delete h; return cuda_fail(cudaGetLastError(), "cudaSetDevice"); }
-  h->var = h->plan.has_c4 ? pick_nreg<true>(h->plan.nreg_variant, h->plan.dp.tab_doubles)
-                          : pick_nreg<false>(h->plan.nreg_variant, h->plan.dp.tab_doubles);
+  h->var = h->plan.has_c4 ? pick_nreg<true>(h->plan.nreg_variant, h->plan.dp.tab_doubles, h->plan.dp.n_r_pad)
+                          : pick_nreg<false>(h->plan.nreg_variant, h->plan.dp.tab_doubles, h->plan.dp.n_r_pad);
   e = cudaFuncSetAttribute((const void*)h->var.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->var.smem);
   if (e != cudaSuccess) { delete h; return cuda_fail(e, "cudaFuncSetAttribute(smem)"); }
   const size_t bytes = sizeof(double) * (size_t)(h->plan.dp.tab_doubles > 0 ? h->plan.dp.tab_doubles : 2);

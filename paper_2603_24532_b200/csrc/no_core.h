@@ -7,23 +7,31 @@
 //     M(p,p',P) = G(p,p',P) - P12 G(p,-p',P),      G = T_id - T_13 - T_23,
 // and every traced term is expanded in Pauli operators of the two external nucleons.  All k3
 // dependence sits in a few scalar "moments"; with k3 = r u (u = unit direction) and the four
-// legs x_l = k3 - kappa_l (kappa = k1, k2, k1', k2'), D_l = x_l^2 + mpi^2:
-//     first level (one direction, sum over radial nodes, registers):
-//        R0 = sum wF,  S_l^k = sum wF r^k / D_l (k=0,1,2),
-//        pair (x,y):  g = wF/(D_x D_y), a.b = -x.y = c_xy - (D_x+D_y)/2, h = g (al + be a.b)
-//                     HAB = sum h a.b, H0 = sum h, H1 = sum h r
-//     second level (sum over directions with angular weight, lane-private shared memory):
+// legs x_l = k3 - kappa_l (kappa = k1, k2, k1', k2'), D_l = x_l^2 + mpi^2 = r^2 + bet_l r + gam_l:
+//     first level (one direction, sum over the radial nodes, 17 registers):
+//        R0 = sum wF,   S_l^k = sum wF r^k / D_l   (k = 0,1; 4 legs),
+//        G_t^k = sum wF r^k / (D_x D_y)             (k = 0,1; 4 exchange pairs t = (x,y))
+//     per direction, from those:  S_l^2 = sum wF r^2/D_l = R0 - bet_l S_l^1 - gam_l S_l^0
+//                                 (c4 only) G_t^2 = S_y^0 - bet_x G_t^1 - gam_x G_t^0
+//     second level (sum over directions with the angular weight, lane-private shared memory):
 //        A0 = sum S^0, A1 = sum S^1 u, A2 = sum S^2 u u^T   (per leg)
-//        BS = sum HAB, B0 = sum H0, B1 = sum H1 u           (per pair)
-// from which  sum wF x/D = A1 - kappa A0,  sum wF x x^T/D = A2 - sym(A1 kappa^T) + kappa kappa^T A0, ...
+//        Gm0 = sum G^0, Gm1 = sum G^1 u  [, Gm2 = sum G^2 u u^T]   (per pair)
+//     epilogue: with a.b = -x_x.x_y = c_xy - (D_x + D_y)/2 every moment of g (a.b)^j, g = wF/(D_x D_y),
+//        follows from the ones above (phase1_job), e.g.
+//        sum g a.b = c Gm0 - (A0_x + A0_y)/2,
+//        sum g (a.b)^2 = c^2 Gm0 - c (A0_x + A0_y) + R0 + [(gam_x-gam_y)(A0_y-A0_x) - 2 (kappa_x-kappa_y).(A1_y-A1_x)]/4,
+//        sum wF x/D = A1 - kappa A0,  sum wF x x^T/D = A2 - A1 kappa^T - kappa (A1 - kappa A0)^T, ...
 // The regulator is evaluated as F = exp(-E0) exp(-dE(d^2)), E0 = (p^2/L^2)^n + (p'^2/L^2)^n the
 // k3-independent part of the exponent, dE a degree-n polynomial in d^2 = |k3 - P/2|^2 without a
 // constant term: identical to Eq. (13) applied to the in- and outgoing triples (R5), but the
 // node-dependent rounding error scales with dE (O(1) where the integrand is large) instead of
-// with the full exponent.
+// with the full exponent.  exp(-dE) is a branch-free 2^(s/64), s = -64 log2(e) dE: 64-entry table
+// of 2^(j/64), degree-5 polynomial on the remainder, exponent added as an integer.
 #pragma once
 
 #include <math.h>
+#include <stdint.h>
+#include <string.h>
 
 #ifdef __CUDACC__
 #define NO_HD __host__ __device__ __forceinline__
@@ -35,13 +43,16 @@ namespace no3n {
 
 constexpr int kLanes = 32;
 constexpr int kMaxRegPoly = 12;   // largest regulator exponent of the generic path
+constexpr int kExpTab = 64;       // entries of the 2^(j/64) table at the start of the device tables
+constexpr int kNodesPerTrip = 4;  // radial nodes per trip of the hot loop (n_r is padded to a multiple)
 
 // kernel-wide constants, all in fm units
 struct DevParams {
   const double* tab;      // device tables, see table layout below
   int n_r, n_cos, n_phi;
+  int n_r_pad;            // n_r rounded up to a multiple of kNodesPerTrip; padding nodes have weight 0
   int n_pass;             // number of Fermi spheres to integrate (1 or 2)
-  int tab_doubles;        // doubles to stage into shared memory (all passes), multiple of 2
+  int tab_doubles;        // doubles to stage into shared memory (exp table + all passes), multiple of 2
   int pass_off[2];        // offset (in doubles) of each pass's tables inside tab
   double nsp[2];          // sum over the species of this pass of 1     (1, or 2 for fused SNM)
   double esum[2];         // sum over the species of this pass of tau_z (+1 proton, -1 neutron, 0 fused)
@@ -55,18 +66,17 @@ struct DevParams {
   int n_reg;              // regulator exponent (generic path)
 };
 
-// table layout of one pass: radial nodes as [n_r][4] = (r, r^2, w_r r^2/(2 pi)^3, 0), then
-// cos(theta)[n_cos], sin(theta)[n_cos], w_cos[n_cos], cos(phi)[n_phi], sin(phi)[n_phi], w_phi[n_phi]
-// (padded to a multiple of 4 doubles so that every pass's radial block stays 32-byte aligned)
-NO_HD int tab_pass_doubles(int n_r, int n_cos, int n_phi) { return (4 * n_r + 3 * n_cos + 3 * n_phi + 3) & ~3; }
+// table layout: tab[0..64) = 2^(j/64); then for each pass: radial nodes as [n_r_pad][2] =
+// (r, w_r r^2/(2 pi)^3), then cos(theta)[n_cos], sin(theta)[n_cos], w_cos[n_cos], cos(phi)[n_phi],
+// sin(phi)[n_phi], w_phi[n_phi] (padded to a multiple of 4 doubles: every radial block 32-byte aligned)
+NO_HD int tab_pass_doubles(int n_r_pad, int n_cos, int n_phi) { return (2 * n_r_pad + 3 * n_cos + 3 * n_phi + 3) & ~3; }
 
 // second-level accumulator rows
 template <bool C4> struct Layout {
-  static constexpr int kPairFirst = C4 ? 6 : 3;     // first-level sums per pair
-  static constexpr int kPairRows = C4 ? 15 : 5;     // second-level rows per pair
-  static constexpr int kRowLeg = 1;                 // row 0 is R0; leg l at 1 + 10 l
+  static constexpr int kPairRows = C4 ? 10 : 4;     // Gm0, Gm1[3] (, Gm2[6])
+  static constexpr int kRowLeg = 1;                 // row 0 is R0; leg l at 1 + 10 l: A0, A1[3], A2[6]
   static constexpr int kRowPair = 41;
-  static constexpr int kRows = 41 + 4 * kPairRows;  // 61 or 101
+  static constexpr int kRows = 41 + 4 * kPairRows;  // 57 or 81
 };
 
 // legs of the four exchange terms.  pair t uses x-leg kPairX[t] (incoming) and y-leg kPairY[t] (outgoing)
@@ -75,6 +85,7 @@ template <bool C4> struct Layout {
 #define NO_PAIR_X(t) ((t) & 1)
 #define NO_PAIR_Y(t) (2 + (((t) & 1) ^ ((t) >> 1)))
 
+// per-configuration constants; the kernel keeps one copy per warp in shared memory
 struct CfgConst {
   double kap[4][3];   // k1, k2, k1', k2'
   double gam[4];      // |kappa_l|^2 + mpi^2
@@ -82,8 +93,11 @@ struct CfgConst {
   double gamd;        // |P/2|^2
   double cpair[4];    // |kappa_x - kappa_y|^2/2 + mpi^2
   double E0;          // k3-independent part of the regulator exponent
-  double rc[kMaxRegPoly];  // dE = sum_k rc[k-1] (d^2)^k, k = 1..n
+  double rs[kMaxRegPoly];  // s = -64 log2(e) dE = sum_k rs[k-1] (d^2)^k, k = 1..n
+  double pad_[3];     // 40 doubles: keeps what follows in shared memory 32-byte aligned
 };
+constexpr int kCfgDoubles = sizeof(CfgConst) / sizeof(double);
+static_assert(kCfgDoubles == 40, "CfgConst layout");
 
 template <int NREG>
 NO_HD void cfg_setup(const DevParams& P, const double* cfg, CfgConst& c) {
@@ -113,7 +127,8 @@ NO_HD void cfg_setup(const DevParams& P, const double* cfg, CfgConst& c) {
   }
   // regulator: (X0 + s3 d2)^n + (X1 + s3 d2)^n = E0 + sum_{k=1..n} C(n,k) (X0^(n-k) + X1^(n-k)) s3^k d2^k
   c.E0 = 0;
-  for (int k = 0; k < kMaxRegPoly; ++k) c.rc[k] = 0;
+  for (int k = 0; k < kMaxRegPoly; ++k) c.rs[k] = 0;
+  for (int k = 0; k < 3; ++k) c.pad_[k] = 0;
   if (NREG >= 0) {
     const int n = NREG > 0 ? NREG : P.n_reg;
     const double X0 = p2 * P.inv_L2, X1 = pp2 * P.inv_L2, s3 = P.inv_L2 * (1.0 / 3.0);
@@ -124,25 +139,89 @@ NO_HD void cfg_setup(const DevParams& P, const double* cfg, CfgConst& c) {
       px1[j] = px1[j - 1] * X1;
       ps3[j] = ps3[j - 1] * s3;
     }
+    const double scale = -92.33248261689366;   // -64 log2(e)
     double binom = 1.0;                       // C(n, k), exact in double
     for (int k = 1; k <= n; ++k) {
       binom = binom * (double)(n - k + 1) / (double)k;
-      c.rc[k - 1] = binom * (px0[n - k] + px1[n - k]) * ps3[k];
+      c.rs[k - 1] = scale * (binom * (px0[n - k] + px1[n - k]) * ps3[k]);
     }
     c.E0 = px0[n] + px1[n];
   }
 }
 
-// dE(d2) = d2 (rc0 + d2 (rc1 + ...)), no constant term
+// ---- bit access to doubles ----
+NO_HD int hi32(double x) {
+#ifdef __CUDA_ARCH__
+  return __double2hiint(x);
+#else
+  uint64_t u; memcpy(&u, &x, 8); return (int)(uint32_t)(u >> 32);
+#endif
+}
+NO_HD int lo32(double x) {
+#ifdef __CUDA_ARCH__
+  return __double2loint(x);
+#else
+  uint64_t u; memcpy(&u, &x, 8); return (int)(uint32_t)u;
+#endif
+}
+NO_HD double hilo(int hi, int lo) {
+#ifdef __CUDA_ARCH__
+  return __hiloint2double(hi, lo);
+#else
+  const uint64_t u = ((uint64_t)(uint32_t)hi << 32) | (uint32_t)lo; double x; memcpy(&x, &u, 8); return x;
+#endif
+}
+
+// exp(-dE(d2)) = 2^(s/64), s = d2 * h(d2) <= 0, h = rs0 + d2 (rs1 + ...).  Branch free:
+//   tm = s + 1.5 2^52 holds round(s) in its low mantissa bits, f = s - round(s) in [-1/2, 1/2],
+//   2^(s/64) = 2^(ky >> 6) * tab[ky & 63] * exp(f ln2/64)  (degree-5 Taylor, |error| < 4e-17).
+// Below s = -65000 (exp(-dE) < 1e-305) the result is replaced by a subnormal (< 3e-308), i.e. zero.
+// The stages are separate functions so that the W nodes of one trip can be interleaved.
 template <int NREG>
-NO_HD double reg_poly(const DevParams& P, const CfgConst& c, double d2) {
-  if (NREG == 1) return d2 * c.rc[0];
-  if (NREG == 2) return d2 * fma(d2, c.rc[1], c.rc[0]);
-  if (NREG == 3) return d2 * fma(d2, fma(d2, c.rc[2], c.rc[1]), c.rc[0]);
-  if (NREG == 4) return d2 * fma(d2, fma(d2, fma(d2, c.rc[3], c.rc[2]), c.rc[1]), c.rc[0]);
-  double s = 0;
-  for (int k = P.n_reg - 1; k >= 0; --k) s = fma(d2, s, c.rc[k]);
-  return d2 * s;
+NO_HD double reg_h(const double* rs, int n_reg, double d2) {
+  if (NREG == 1) return rs[0];
+  if (NREG == 2) return fma(d2, rs[1], rs[0]);
+  if (NREG == 3) return fma(d2, fma(d2, rs[2], rs[1]), rs[0]);
+  if (NREG == 4) return fma(d2, fma(d2, fma(d2, rs[3], rs[2]), rs[1]), rs[0]);
+  double h = rs[n_reg - 1];
+  for (int k = n_reg - 2; k >= 0; --k) h = fma(d2, h, rs[k]);
+  return h;
+}
+
+constexpr double kMagic = 6755399441055744.0;             // 1.5 * 2^52
+
+// scaled table value 2^(ky/64) from tm = s + kMagic and kf = round(s)
+NO_HD double exp2_table(double tm, double kf, const double* e2tab) {
+  const int ky = lo32(tm);
+  const double T = e2tab[ky & (kExpTab - 1)];
+  int hiT = hi32(T) + (ky >> 6) * 1048576;                // exponent field += floor(ky / 64)
+  hiT = (uint32_t)hi32(kf) > 0xC0EFBD00u ? 0 : hiT;       // kf < -65000 (or not finite): flush
+  return hilo(hiT, lo32(T));
+}
+
+// exp(f ln2/64), |f| <= 1/2
+NO_HD double exp2_poly(double f) {
+  const double c1 = 0.010830424696249145;                 // (ln2/64)^m / m!
+  const double c2 = 5.86490495505617e-05;
+  const double c3 = 2.1173137155464776e-07;
+  const double c4 = 5.732851688640402e-10;
+  const double c5 = 1.2417843701716925e-12;
+  double p = fma(f, c5, c4);
+  p = fma(f, p, c3);
+  p = fma(f, p, c2);
+  p = fma(f, p, c1);
+  return fma(f, p, 1.0);
+}
+
+// hardware seed of 1/x (relative error <= 2^-20, measured), x normal and positive
+NO_HD double rcp_seed(double d) {
+#ifdef __CUDA_ARCH__
+  double x;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(d));
+  return x;
+#else
+  return hilo(hi32(1.0 / hilo(hi32(d), 0)), 0);           // emulation of the seed: high word only
+#endif
 }
 
 // per-direction constants
@@ -158,123 +237,167 @@ NO_HD void dir_setup(const CfgConst& c, double ux, double uy, double uz, DirCons
   d.betd = -2.0 * fma(ux, c.hP[0], fma(uy, c.hP[1], uz * c.hP[2]));
 }
 
-template <bool C4> struct First {
+// first-level sums of one direction
+struct First {
   double R0;
-  double S[4][3];
-  double Pr[4][Layout<C4>::kPairFirst];   // !C4: HAB, H0, H1      C4: G0, G1, G2, GA0, GA1, GAA0
+  double S[4][2];
+  double G[4][2];
 };
 
-template <bool C4> NO_HD void first_zero(First<C4>& f) {
+NO_HD void first_zero(First& f) {
   f.R0 = 0;
-  for (int l = 0; l < 4; ++l) for (int k = 0; k < 3; ++k) f.S[l][k] = 0;
-  for (int t = 0; t < 4; ++t) for (int k = 0; k < Layout<C4>::kPairFirst; ++k) f.Pr[t][k] = 0;
+  for (int l = 0; l < 4; ++l) f.S[l][0] = f.S[l][1] = 0;
+  for (int t = 0; t < 4; ++t) f.G[t][0] = f.G[t][1] = 0;
 }
 
-NO_HD double no_exp_neg(double e) {   // exp(-e), e >= 0
-  return exp(-e);
+// per-warp radial table entry (shared memory): r^2 + |P/2|^2, r^2 + gam_l (l = 0..3), pad
+constexpr int kRadT = 6;
+
+NO_HD void radial_entry(const CfgConst& c, double r, double* T) {
+  T[0] = fma(r, r, c.gamd);
+  for (int l = 0; l < 4; ++l) T[1 + l] = fma(r, r, c.gam[l]);
+  T[5] = 0.0;
 }
 
-NO_HD double no_rcp(double x) { return 1.0 / x; }
-
-// one k3 node: r, r2 = r^2, wr = w_r r^2/(2 pi)^3   (the HOT loop body)
-template <int NREG, bool C4>
-NO_HD void node(const DevParams& P, const CfgConst& c, const DirConst& d, double r, double r2, double wr,
-                First<C4>& f) {
-  double wf = wr;
+// W k3 nodes of one direction at once (the HOT loop body): r, wr = w_r r^2/(2 pi)^3,
+// T = radial_entry.  Every step is written for all W nodes before the next one, so that the W
+// independent dependency chains interleave in the instruction stream (FP64 latency is 8 cycles at
+// one instruction per 2 cycles).
+template <int NREG, int W>
+NO_HD void nodes(const double* rs, int n_reg, const double* e2tab, const DirConst& d, const double* r,
+                 const double* wr, const double (*T)[5], First& f) {
+  double F[W], D0[W], D1[W], D2[W], D3[W], p01[W], p23[W], den[W], x[W];
+#pragma unroll
+  for (int k = 0; k < W; ++k) {
+    D0[k] = fma(r[k], d.bet[0], T[k][1]);
+    D1[k] = fma(r[k], d.bet[1], T[k][2]);
+    D2[k] = fma(r[k], d.bet[2], T[k][3]);
+    D3[k] = fma(r[k], d.bet[3], T[k][4]);
+  }
+#pragma unroll
+  for (int k = 0; k < W; ++k) { p01[k] = D0[k] * D1[k]; p23[k] = D2[k] * D3[k]; }
+#pragma unroll
+  for (int k = 0; k < W; ++k) den[k] = p01[k] * p23[k];
+#pragma unroll
+  for (int k = 0; k < W; ++k) x[k] = rcp_seed(den[k]);
   if (NREG >= 0) {
-    const double d2 = fma(r, r + d.betd, c.gamd);
-    wf = wr * no_exp_neg(reg_poly<NREG>(P, c, d2));
+    double d2[W], h[W], tm[W], kf[W], fr[W], Ts[W];
+#pragma unroll
+    for (int k = 0; k < W; ++k) d2[k] = fma(r[k], d.betd, T[k][0]);
+#pragma unroll
+    for (int k = 0; k < W; ++k) h[k] = reg_h<NREG>(rs, n_reg, d2[k]);
+#pragma unroll
+    for (int k = 0; k < W; ++k) tm[k] = fma(d2[k], h[k], kMagic);
+#pragma unroll
+    for (int k = 0; k < W; ++k) kf[k] = tm[k] - kMagic;                 // round(s), exact
+#pragma unroll
+    for (int k = 0; k < W; ++k) fr[k] = fma(d2[k], h[k], -kf[k]);       // s - round(s), one rounding
+#pragma unroll
+    for (int k = 0; k < W; ++k) Ts[k] = exp2_table(tm[k], kf[k], e2tab);
+#pragma unroll
+    for (int k = 0; k < W; ++k) F[k] = exp2_poly(fr[k]);
+#pragma unroll
+    for (int k = 0; k < W; ++k) F[k] *= Ts[k];
+  } else {
+#pragma unroll
+    for (int k = 0; k < W; ++k) F[k] = 1.0;
   }
-  double D[4];
-  for (int l = 0; l < 4; ++l) D[l] = fma(r, r + d.bet[l], c.gam[l]);
-  // four reciprocals from one division
-  const double p01 = D[0] * D[1], p23 = D[2] * D[3];
-  const double inv = no_rcp(p01 * p23);
-  const double i01 = inv * p23, i23 = inv * p01;
-  double iD[4];
-  iD[0] = i01 * D[1];
-  iD[1] = i01 * D[0];
-  iD[2] = i23 * D[3];
-  iD[3] = i23 * D[2];
-  const double wf1 = wf * r, wf2 = wf * r2;
-  f.R0 += wf;
-  for (int l = 0; l < 4; ++l) {
-    f.S[l][0] = fma(wf, iD[l], f.S[l][0]);
-    f.S[l][1] = fma(wf1, iD[l], f.S[l][1]);
-    f.S[l][2] = fma(wf2, iD[l], f.S[l][2]);
+  // 1/den: seed and one cubic step, x (1 + e + e^2), e = 1 - den x (relative error 2^-60 + rounding)
+  double e[W];
+#pragma unroll
+  for (int k = 0; k < W; ++k) e[k] = fma(-den[k], x[k], 1.0);
+#pragma unroll
+  for (int k = 0; k < W; ++k) e[k] = fma(e[k], e[k], e[k]);
+#pragma unroll
+  for (int k = 0; k < W; ++k) x[k] = fma(x[k], e[k], x[k]);
+  // four reciprocals from one
+  double i01[W], i23[W], iD0[W], iD1[W], iD2[W], iD3[W], g0[W], g1[W], g2[W], g3[W], wf[W], wf1[W];
+#pragma unroll
+  for (int k = 0; k < W; ++k) { i01[k] = x[k] * p23[k]; i23[k] = x[k] * p01[k]; }
+#pragma unroll
+  for (int k = 0; k < W; ++k) {
+    iD0[k] = i01[k] * D1[k]; iD1[k] = i01[k] * D0[k];
+    iD2[k] = i23[k] * D3[k]; iD3[k] = i23[k] * D2[k];
   }
-  const double wi0 = wf * iD[0], wi1 = wf * iD[1];
-  for (int t = 0; t < 4; ++t) {
-    const int x = NO_PAIR_X(t), y = NO_PAIR_Y(t);
-    const double g = (x == 0 ? wi0 : wi1) * iD[y];
-    const double ab = fma(-0.5, D[x] + D[y], c.cpair[t]);
-    if (!C4) {
-      const double h = g * fma(P.be, ab, P.al);
-      f.Pr[t][0] = fma(h, ab, f.Pr[t][0]);
-      f.Pr[t][1] += h;
-      f.Pr[t][2] = fma(h, r, f.Pr[t][2]);
-    } else {
-      const double ga = g * ab;
-      f.Pr[t][0] += g;
-      f.Pr[t][1] = fma(g, r, f.Pr[t][1]);
-      f.Pr[t][2] = fma(g, r2, f.Pr[t][2]);
-      f.Pr[t][3] += ga;
-      f.Pr[t][4] = fma(ga, r, f.Pr[t][4]);
-      f.Pr[t][5] = fma(ga, ab, f.Pr[t][5]);
-    }
+#pragma unroll
+  for (int k = 0; k < W; ++k) {
+    g0[k] = iD0[k] * iD2[k];   // pair 0 = legs (0, 2)
+    g1[k] = iD1[k] * iD3[k];   // pair 1 = legs (1, 3)
+    g2[k] = iD0[k] * iD3[k];   // pair 2 = legs (0, 3)
+    g3[k] = iD1[k] * iD2[k];   // pair 3 = legs (1, 2)
+  }
+#pragma unroll
+  for (int k = 0; k < W; ++k) { wf[k] = wr[k] * F[k]; }
+#pragma unroll
+  for (int k = 0; k < W; ++k) { wf1[k] = wf[k] * r[k]; }
+#pragma unroll
+  for (int k = 0; k < W; ++k) {
+    f.R0 = fma(wr[k], F[k], f.R0);
+    f.S[0][0] = fma(wf[k], iD0[k], f.S[0][0]);
+    f.S[1][0] = fma(wf[k], iD1[k], f.S[1][0]);
+    f.S[2][0] = fma(wf[k], iD2[k], f.S[2][0]);
+    f.S[3][0] = fma(wf[k], iD3[k], f.S[3][0]);
+    f.G[0][0] = fma(wf[k], g0[k], f.G[0][0]);
+    f.G[1][0] = fma(wf[k], g1[k], f.G[1][0]);
+    f.G[2][0] = fma(wf[k], g2[k], f.G[2][0]);
+    f.G[3][0] = fma(wf[k], g3[k], f.G[3][0]);
+    f.S[0][1] = fma(wf1[k], iD0[k], f.S[0][1]);
+    f.S[1][1] = fma(wf1[k], iD1[k], f.S[1][1]);
+    f.S[2][1] = fma(wf1[k], iD2[k], f.S[2][1]);
+    f.S[3][1] = fma(wf1[k], iD3[k], f.S[3][1]);
+    f.G[0][1] = fma(wf1[k], g0[k], f.G[0][1]);
+    f.G[1][1] = fma(wf1[k], g1[k], f.G[1][1]);
+    f.G[2][1] = fma(wf1[k], g2[k], f.G[2][1]);
+    f.G[3][1] = fma(wf1[k], g3[k], f.G[3][1]);
   }
 }
 
 // second level: acc[row * kLanes + lane] += w_ang * (first-level sum) * (1 | u | u u^T)
+// The rows are updated in groups (all loads of a group, then the FMAs, then the stores) so that the
+// shared-memory latency is paid once per group; the compiler fences at both ends keep it from
+// carrying the rows in registers across the direction loop.
+#define NO_FENCE() asm volatile("" ::: "memory")
+
+NO_HD void rmw_rank012(double* a /* 10 rows: 1 | u | u u^T */, const double* wt, double s0, double s1, double s2) {
+  double v[10];
+  for (int k = 0; k < 10; ++k) v[k] = a[k * kLanes];
+  v[0] = fma(wt[0], s0, v[0]);
+  for (int k = 1; k < 4; ++k) v[k] = fma(wt[k], s1, v[k]);
+  for (int k = 4; k < 10; ++k) v[k] = fma(wt[k], s2, v[k]);
+  for (int k = 0; k < 10; ++k) a[k * kLanes] = v[k];
+}
+
 template <bool C4>
-NO_HD void second_level(const First<C4>& f, const DirConst& d, double w, volatile double* acc /* + lane */) {
-  // `volatile`: every row is read, updated and written back in shared memory right here; without it
-  // the compiler keeps all rows live in registers across the direction loop and spills them
+NO_HD void second_level(const First& f, const DirConst& d, const double* gam, double w, double* acc /* + lane */) {
   const double ux = d.u[0], uy = d.u[1], uz = d.u[2];
-  const double wx = w * ux, wy = w * uy, wz = w * uz;
-  const double wxx = wx * ux, wxy = wx * uy, wxz = wx * uz, wyy = wy * uy, wyz = wy * uz, wzz = wz * uz;
-#define NO_ACCW(row, wgt, val) acc[(row) * kLanes] = fma((wgt), (val), acc[(row) * kLanes])
-  NO_ACCW(0, w, f.R0);
+  double wt[10];      // w * (1, ux, uy, uz, ux ux, ux uy, ux uz, uy uy, uy uz, uz uz)
+  wt[0] = w; wt[1] = w * ux; wt[2] = w * uy; wt[3] = w * uz;
+  wt[4] = wt[1] * ux; wt[5] = wt[1] * uy; wt[6] = wt[1] * uz; wt[7] = wt[2] * uy; wt[8] = wt[2] * uz; wt[9] = wt[3] * uz;
+  NO_FENCE();
   for (int l = 0; l < 4; ++l) {
-    const int b = Layout<C4>::kRowLeg + 10 * l;
-    NO_ACCW(b + 0, w, f.S[l][0]);
-    NO_ACCW(b + 1, wx, f.S[l][1]);
-    NO_ACCW(b + 2, wy, f.S[l][1]);
-    NO_ACCW(b + 3, wz, f.S[l][1]);
-    NO_ACCW(b + 4, wxx, f.S[l][2]);
-    NO_ACCW(b + 5, wxy, f.S[l][2]);
-    NO_ACCW(b + 6, wxz, f.S[l][2]);
-    NO_ACCW(b + 7, wyy, f.S[l][2]);
-    NO_ACCW(b + 8, wyz, f.S[l][2]);
-    NO_ACCW(b + 9, wzz, f.S[l][2]);
+    const double S2 = fma(-gam[l], f.S[l][0], fma(-d.bet[l], f.S[l][1], f.R0));   // sum wF r^2 / D_l
+    rmw_rank012(acc + (Layout<C4>::kRowLeg + 10 * l) * kLanes, wt, f.S[l][0], f.S[l][1], S2);
   }
-  for (int t = 0; t < 4; ++t) {
-    const int b = Layout<C4>::kRowPair + Layout<C4>::kPairRows * t;
-    if (!C4) {
-      NO_ACCW(b + 0, w, f.Pr[t][0]);    // BS
-      NO_ACCW(b + 1, w, f.Pr[t][1]);    // B0
-      NO_ACCW(b + 2, wx, f.Pr[t][2]);   // B1
-      NO_ACCW(b + 3, wy, f.Pr[t][2]);
-      NO_ACCW(b + 4, wz, f.Pr[t][2]);
-    } else {
-      NO_ACCW(b + 0, w, f.Pr[t][0]);    // G0
-      NO_ACCW(b + 1, wx, f.Pr[t][1]);   // G1 u
-      NO_ACCW(b + 2, wy, f.Pr[t][1]);
-      NO_ACCW(b + 3, wz, f.Pr[t][1]);
-      NO_ACCW(b + 4, wxx, f.Pr[t][2]);  // G2 u u^T
-      NO_ACCW(b + 5, wxy, f.Pr[t][2]);
-      NO_ACCW(b + 6, wxz, f.Pr[t][2]);
-      NO_ACCW(b + 7, wyy, f.Pr[t][2]);
-      NO_ACCW(b + 8, wyz, f.Pr[t][2]);
-      NO_ACCW(b + 9, wzz, f.Pr[t][2]);
-      NO_ACCW(b + 10, w, f.Pr[t][3]);   // GA0
-      NO_ACCW(b + 11, wx, f.Pr[t][4]);  // GA1 u
-      NO_ACCW(b + 12, wy, f.Pr[t][4]);
-      NO_ACCW(b + 13, wz, f.Pr[t][4]);
-      NO_ACCW(b + 14, w, f.Pr[t][5]);   // GAA0
+  if (C4) {
+    for (int t = 0; t < 4; ++t) {
+      const int x = NO_PAIR_X(t), y = NO_PAIR_Y(t);
+      const double G2 = fma(-gam[x], f.G[t][0], fma(-d.bet[x], f.G[t][1], f.S[y][0]));   // sum wF r^2/(D_x D_y)
+      rmw_rank012(acc + (Layout<C4>::kRowPair + 10 * t) * kLanes, wt, f.G[t][0], f.G[t][1], G2);   // Gm0, Gm1, Gm2
     }
+    acc[0] = fma(w, f.R0, acc[0]);
+  } else {
+    double v[17];     // R0 and Gm0, Gm1[3] of the four pairs
+    v[0] = acc[0];
+    for (int k = 0; k < 16; ++k) v[1 + k] = acc[(Layout<C4>::kRowPair + k) * kLanes];
+    v[0] = fma(w, f.R0, v[0]);
+    for (int t = 0; t < 4; ++t) {
+      v[1 + 4 * t] = fma(wt[0], f.G[t][0], v[1 + 4 * t]);
+      for (int k = 1; k < 4; ++k) v[1 + 4 * t + k] = fma(wt[k], f.G[t][1], v[1 + 4 * t + k]);
+    }
+    acc[0] = v[0];
+    for (int k = 0; k < 16; ++k) acc[(Layout<C4>::kRowPair + k) * kLanes] = v[1 + k];
   }
-#undef NO_ACCW
+  NO_FENCE();
 }
 
 // ------------------------------------------------------------------------------------------
@@ -328,15 +451,22 @@ NO_HD void phase1_job(const DevParams& P, const CfgConst& c, const double* mom, 
     const double Dc = fma(cv[0], cv[0], fma(cv[1], cv[1], fma(cv[2], cv[2], P.m2)));
     const double iDc = 1.0 / Dc;
     const int pb = Layout<C4>::kRowPair + Layout<C4>::kPairRows * t;
-    double BS, B0, B1[3];
-    if (!C4) {
-      BS = mom[pb]; B0 = mom[pb + 1];
-      for (int a = 0; a < 3; ++a) B1[a] = mom[pb + 2 + a];
-    } else {
-      BS = P.al * mom[pb + 10] + P.be * mom[pb + 14];
-      B0 = P.al * mom[pb] + P.be * mom[pb + 10];
-      for (int a = 0; a < 3; ++a) B1[a] = P.al * mom[pb + 1 + a] + P.be * mom[pb + 11 + a];
+    // moments of g (a.b)^j, g = wF/(D_x D_y), a.b = c_xy - (D_x + D_y)/2, from Gm0, Gm1 and the leg moments
+    const int lx = Layout<C4>::kRowLeg + 10 * x, ly = Layout<C4>::kRowLeg + 10 * y;
+    const double Gm0 = mom[pb], ct = c.cpair[t];
+    const double sA0 = mom[lx] + mom[ly], dA0 = mom[ly] - mom[lx];
+    const double GA0 = fma(ct, Gm0, -0.5 * sA0);                       // sum g a.b
+    double GA1[3], dkA1 = 0;                                           // sum g a.b r u
+    for (int a = 0; a < 3; ++a) {
+      GA1[a] = fma(ct, mom[pb + 1 + a], -0.5 * (mom[lx + 1 + a] + mom[ly + 1 + a]));
+      dkA1 = fma(kx[a] - ky[a], mom[ly + 1 + a] - mom[lx + 1 + a], dkA1);
     }
+    const double gx = x == 0 ? c.gam[0] : c.gam[1], gy = y == 2 ? c.gam[2] : c.gam[3];
+    const double GAA0 = fma(ct, GA0 - 0.5 * sA0, R0) + 0.25 * fma(gx - gy, dA0, -2.0 * dkA1);   // sum g (a.b)^2
+    const double BS = fma(P.al, GA0, P.be * GAA0);                     // sum h a.b, h = g (al + be a.b)
+    const double B0 = fma(P.al, Gm0, P.be * GA0);                      // sum h
+    double B1[3];                                                      // sum h r u
+    for (int a = 0; a < 3; ++a) B1[a] = fma(P.al, mom[pb + 1 + a], P.be * GA1[a]);
     double hab[3];
     for (int a = 0; a < 3; ++a) hab[a] = fma(-kx[a], B0, B1[a]);
     double va[3], vb[3], Tac[3], Tbc[3];
@@ -361,10 +491,9 @@ NO_HD void phase1_job(const DevParams& P, const CfgConst& c, const double* mom, 
     for (int a = 0; a < 12; ++a) o[23 + a] = 0;  // T4[9], n4[3] (c4 topology)
     if (C4) {
       // Ga = sum g a, GAa = sum g (a.b) a, Gaa = sum g a a^T   (a = r u - kappa_x)
-      double G0, Ga[3], Gaa[6], GA0, GAa[3];
+      double G0, Ga[3], Gaa[6], GAa[3];
       leg_moments(mom, pb, kx, G0, Ga, Gaa);
-      GA0 = mom[pb + 10];
-      for (int a = 0; a < 3; ++a) GAa[a] = fma(-kx[a], GA0, mom[pb + 11 + a]);
+      for (int a = 0; a < 3; ++a) GAa[a] = fma(-kx[a], GA0, GA1[a]);
       (void)G0; (void)Ga;
       double v12[3];
       for (int a = 0; a < 3; ++a) v12[a] = cv[a] * (trA + trB) - (Tac[a] + Tbc[a]);

@@ -124,29 +124,30 @@ inline int build_plan(const no_params* p, HostPlan& plan) {
   plan.n_sph = d.n_pass;
   plan.evals_per_cfg = (long long)p->n_r * p->n_cos * p->n_phi * d.n_pass;
 
-  const int per = tab_pass_doubles(p->n_r, p->n_cos, p->n_phi);
-  int total = per * d.n_pass;
+  d.n_r_pad = (p->n_r + kNodesPerTrip - 1) / kNodesPerTrip * kNodesPerTrip;
+  const int per = tab_pass_doubles(d.n_r_pad, p->n_cos, p->n_phi);
+  int total = kExpTab + per * d.n_pass;
   total = (total + 1) & ~1;               // 16-byte granularity of the bulk copy
   d.tab_doubles = total;
   plan.tab.assign(total, 0.0);
+  for (int j = 0; j < kExpTab; ++j) plan.tab[j] = (double)exp2l((long double)j / kExpTab);   // 2^(j/64)
   const double pi = 3.14159265358979323846;
   const double norm = 1.0 / (8.0 * pi * pi * pi);
   std::vector<double> xr, wr, xc, wc, xp, wp;
   gl_rule(p->n_cos, -1.0, 1.0, xc, wc);
   gl_rule(p->n_phi, 0.0, 2.0 * pi, xp, wp);
   for (int s = 0; s < d.n_pass; ++s) {
-    d.pass_off[s] = per * s;
+    d.pass_off[s] = kExpTab + per * s;
     d.nsp[s] = passes[s].nsp;
     d.esum[s] = passes[s].esum;
-    double* T = plan.tab.data() + per * s;
+    double* T = plan.tab.data() + d.pass_off[s];
     gl_rule(p->n_r, 0.0, passes[s].kf, xr, wr);
-    for (int i = 0; i < p->n_r; ++i) {
-      T[4 * i + 0] = xr[i];
-      T[4 * i + 1] = xr[i] * xr[i];
-      T[4 * i + 2] = wr[i] * xr[i] * xr[i] * norm;
-      T[4 * i + 3] = 0.0;
+    for (int i = 0; i < d.n_r_pad; ++i) {
+      const int k = i < p->n_r ? i : p->n_r - 1;        // padding node: a valid radius with weight 0
+      T[2 * i + 0] = xr[k];
+      T[2 * i + 1] = i < p->n_r ? wr[k] * xr[k] * xr[k] * norm : 0.0;
     }
-    double* A = T + 4 * p->n_r;
+    double* A = T + 2 * d.n_r_pad;
     for (int j = 0; j < p->n_cos; ++j) {
       A[j] = xc[j];
       A[p->n_cos + j] = std::sqrt((1.0 - xc[j]) * (1.0 + xc[j]));

@@ -1,12 +1,13 @@
 // no_kernel.cuh -- the sm_100a kernel of the 3N normal ordering.
 //
 // One warp integrates one configuration (p, p', P): lanes stride over the angular directions
-// of the k3 grid, every lane runs the radial loop of its direction with all sums in registers
-// (no3n::node, the hot loop), folds them into lane-private shared-memory accumulators
-// (no3n::second_level), then the warp reduces the 61 (101 with c4) moments, turns them into
-// Pauli-operator coefficients and writes the 16x16 complex matrix.  A CTA holds WARPS warps;
-// the quadrature tables of every Fermi sphere are staged once per CTA into shared memory with
-// one TMA bulk copy (cp.async.bulk + mbarrier).
+// of the k3 grid, every lane runs the radial loop of its direction, two nodes per trip, with the
+// 17 first-level sums in registers (no3n::node, the hot loop, branch free), folds them into
+// lane-private shared-memory accumulators (no3n::second_level), then the warp reduces the 57
+// (81 with c4) moments, turns them into Pauli-operator coefficients and writes the 16x16 complex
+// matrix.  A CTA holds WARPS warps; the 2^(j/64) table and the quadrature tables of every Fermi
+// sphere are staged once per CTA into shared memory with one TMA bulk copy (cp.async.bulk +
+// mbarrier); r^2 + gam_l of the configuration is tabulated per warp.
 #pragma once
 
 #include <cuda_runtime.h>
@@ -44,12 +45,17 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t phase) {
   }
 }
 
-// shared memory per CTA, in doubles: tables | mbarrier (2) | mom[WARPS][rows_pad] | acc[WARPS][rows][32]
+// shared memory per CTA, in doubles:
+//   tables | mbarrier (2) | per warp: CfgConst (40) | radial table [n_r_pad][6] | mom[rows_pad] | acc[rows][32]
 template <bool C4> __host__ __device__ constexpr int rows_pad() { return (Layout<C4>::kRows + 3) & ~3; }
 
+template <bool C4> __host__ __device__ inline int warp_doubles(int n_r_pad) {
+  return kCfgDoubles + kRadT * n_r_pad + rows_pad<C4>() + Layout<C4>::kRows * kLanes;
+}
+
 template <bool C4>
-inline size_t smem_bytes(int tab_doubles, int warps) {
-  return sizeof(double) * (size_t)(tab_doubles + 2 + warps * (rows_pad<C4>() + Layout<C4>::kRows * kLanes));
+inline size_t smem_bytes(int tab_doubles, int n_r_pad, int warps) {
+  return sizeof(double) * (size_t)(tab_doubles + 2 + warps * warp_doubles<C4>(n_r_pad));
 }
 
 template <int NREG, bool C4, int WARPS, int MINB>
@@ -60,61 +66,82 @@ no3n_kernel(const DevParams P, const double* __restrict__ cfg, long long n_cfg, 
   double* s_tab = smem;
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem + P.tab_doubles);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  double* mom = smem + P.tab_doubles + 2 + warp * rows_pad<C4>();
-  double* acc = smem + P.tab_doubles + 2 + WARPS * rows_pad<C4>() + warp * (L::kRows * kLanes);
+  double* wbase = smem + P.tab_doubles + 2 + warp * warp_doubles<C4>(P.n_r_pad);
+  CfgConst* cc = reinterpret_cast<CfgConst*>(wbase);
+  double* ttab = wbase + kCfgDoubles;
+  double* mom = ttab + kRadT * P.n_r_pad;
+  double* acc = mom + rows_pad<C4>();
 
-  // ---- a0: stage the quadrature tables (TMA bulk copy, one per CTA) ----
-  if (threadIdx.x == 0) mbar_init(bar, 1);
-  __syncthreads();
-  if (threadIdx.x == 0 && P.tab_doubles > 0) {
+  // ---- a0: stage the exp table and the quadrature tables (TMA bulk copy, one per CTA) ----
+  if (threadIdx.x == 0) {
+    mbar_init(bar, 1);
     const uint32_t bytes = (uint32_t)P.tab_doubles * 8u;
     mbar_expect_tx(bar, bytes);
     tma_bulk_g2s(s_tab, P.tab, bytes, bar);
   }
+  __syncthreads();
 
   const long long ic = (long long)blockIdx.x * WARPS + warp;
   if (ic >= n_cfg) return;
 
-  // ---- a1: per-configuration constants (every lane holds them) ----
-  CfgConst c;
+  // ---- a1: per-configuration constants, one copy per warp in shared memory ----
   {
     double q[9];
 #pragma unroll
     for (int a = 0; a < 9; ++a) q[a] = __ldg(cfg + ic * 9 + a);
+    CfgConst c;
     cfg_setup<NREG>(P, q, c);
+    if (lane == 0) *cc = c;
   }
-  if (P.tab_doubles > 0) mbar_wait(bar, 0);
+  __syncwarp();
+  double rs[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) rs[k] = cc->rs[k];
+  const double* rsp = NREG >= 1 ? rs : cc->rs;     // unrolled exponents keep the coefficients in registers
+  mbar_wait(bar, 0);
+  const double* e2tab = s_tab;
 
   double blk[6] = {0, 0, 0, 0, 0, 0};
   for (int pass = 0; pass < P.n_pass; ++pass) {
     const double* rad = s_tab + P.pass_off[pass];
-    const double* ct = rad + 4 * P.n_r;
+    const double* ct = rad + 2 * P.n_r_pad;
     const double* st = ct + P.n_cos;
     const double* wc = st + P.n_cos;
     const double* cph = wc + P.n_cos;
     const double* sph = cph + P.n_phi;
     const double* wph = sph + P.n_phi;
+    for (int i = lane; i < P.n_r_pad; i += kLanes) radial_entry(*cc, rad[2 * i], ttab + kRadT * i);
 #pragma unroll 1
     for (int row = 0; row < L::kRows; ++row) acc[row * kLanes + lane] = 0.0;
+    __syncwarp();
 
     // ---- a2 + a3: hot loop over the k3 nodes of this sphere ----
     const int n_dir = P.n_cos * P.n_phi;
+    const double2* rad2 = reinterpret_cast<const double2*>(rad);
+    const double2* tt2 = reinterpret_cast<const double2*>(ttab);
 #pragma unroll 1
     for (int m = lane; m < n_dir; m += kLanes) {
       const int j = m / P.n_phi, l = m - j * P.n_phi;
       const double sj = st[j];
       DirConst d;
-      dir_setup(c, sj * cph[l], sj * sph[l], ct[j], d);
+      dir_setup(*cc, sj * cph[l], sj * sph[l], ct[j], d);
       const double w = wc[j] * wph[l];
-      First<C4> f;
-      first_zero<C4>(f);
-      const double4* rad4 = reinterpret_cast<const double4*>(rad);
-#pragma unroll 2
-      for (int i = 0; i < P.n_r; ++i) {
-        const double4 q = rad4[i];
-        node<NREG, C4>(P, c, d, q.x, q.y, q.z, f);
+      First f;
+      first_zero(f);
+#pragma unroll 1
+      for (int i = 0; i < P.n_r_pad; i += kNodesPerTrip) {     // kNodesPerTrip independent nodes per trip
+        double r[kNodesPerTrip], wr[kNodesPerTrip], T[kNodesPerTrip][5];
+#pragma unroll
+        for (int k = 0; k < kNodesPerTrip; ++k) {
+          const double2 a = rad2[i + k];
+          const double2 t0 = tt2[3 * (i + k)], t1 = tt2[3 * (i + k) + 1];
+          const double t2 = ttab[kRadT * (i + k) + 4];
+          r[k] = a.x; wr[k] = a.y;
+          T[k][0] = t0.x; T[k][1] = t0.y; T[k][2] = t1.x; T[k][3] = t1.y; T[k][4] = t2;
+        }
+        nodes<NREG, kNodesPerTrip>(rsp, P.n_reg, e2tab, d, r, wr, T, f);
       }
-      second_level<C4>(f, d, w, acc + lane);
+      second_level<C4>(f, d, cc->gam, w, acc + lane);
     }
     __syncwarp();
 
@@ -129,9 +156,9 @@ no3n_kernel(const DevParams P, const double* __restrict__ cfg, long long n_cfg, 
 
     // ---- a4: epilogue, phases 1 and 2 (records live in the dead accumulator area) ----
     double* rec = acc;
-    if (lane < 6) phase1_job<C4>(P, c, mom, lane, rec);
+    if (lane < 6) phase1_job<C4>(P, *cc, mom, lane, rec);
     __syncwarp();
-    phase2_lane(rec, lane, P.nsp[pass], P.esum[pass], NREG >= 0 ? exp(-c.E0) : 1.0, blk);
+    phase2_lane(rec, lane, P.nsp[pass], P.esum[pass], NREG >= 0 ? exp(-cc->E0) : 1.0, blk);
     __syncwarp();
   }
 

@@ -12,6 +12,19 @@
 
 using namespace no3n;
 
+// one trip of the hot loop: the kernel's load pattern followed by no3n::nodes
+template <int NREG>
+static void trip(const double* rs, int n_reg, const double* e2tab, const DirConst& d, const double* rad,
+                 const double* ttab, int i, First& f) {
+  double r[kNodesPerTrip], wr[kNodesPerTrip], T[kNodesPerTrip][5];
+  for (int k = 0; k < kNodesPerTrip; ++k) {
+    r[k] = rad[2 * (i + k)];
+    wr[k] = rad[2 * (i + k) + 1];
+    for (int q = 0; q < 5; ++q) T[k][q] = ttab[kRadT * (i + k) + q];
+  }
+  nodes<NREG, kNodesPerTrip>(rs, n_reg, e2tab, d, r, wr, T, f);
+}
+
 template <int NREG, bool C4>
 static void emu_cfg(const HostPlan& plan, const double* cfg, double* out /*[512]*/) {
   using L = Layout<C4>;
@@ -19,9 +32,12 @@ static void emu_cfg(const HostPlan& plan, const double* cfg, double* out /*[512]
   CfgConst c;
   cfg_setup<NREG>(P, cfg, c);
   std::vector<double> acc(L::kRows * kLanes), mom(L::kRows), rec(kRecDoubles), coef(32 * 6, 0.0);
+  std::vector<double> ttab(kRadT * P.n_r_pad);
+  const double* e2tab = plan.tab.data();
   for (int pass = 0; pass < P.n_pass; ++pass) {
     const double* rad = plan.tab.data() + P.pass_off[pass];
-    const double* ct = rad + 4 * P.n_r;
+    for (int i = 0; i < P.n_r_pad; ++i) radial_entry(c, rad[2 * i], &ttab[kRadT * i]);
+    const double* ct = rad + 2 * P.n_r_pad;
     const double* st = ct + P.n_cos;
     const double* wc = st + P.n_cos;
     const double* cph = wc + P.n_cos;
@@ -35,10 +51,10 @@ static void emu_cfg(const HostPlan& plan, const double* cfg, double* out /*[512]
         DirConst d;
         dir_setup(c, st[j] * cph[l], st[j] * sph[l], ct[j], d);
         const double w = wc[j] * wph[l];
-        First<C4> f;
-        first_zero<C4>(f);
-        for (int i = 0; i < P.n_r; ++i) node<NREG, C4>(P, c, d, rad[4 * i], rad[4 * i + 1], rad[4 * i + 2], f);
-        second_level<C4>(f, d, w, acc.data() + lane);
+        First f;
+        first_zero(f);
+        for (int i = 0; i < P.n_r_pad; i += kNodesPerTrip) trip<NREG>(c.rs, P.n_reg, e2tab, d, rad, ttab.data(), i, f);
+        second_level<C4>(f, d, c.gam, w, acc.data() + lane);
       }
     }
     for (int lane = 0; lane < kLanes; ++lane)
@@ -120,7 +136,9 @@ extern "C" int emu_moments(const no_params* p, const double* cfg, int pass, doub
   cfg_setup<-1>(P, cfg, c);
   std::vector<double> acc(L::kRows * kLanes, 0.0);
   const double* rad = plan.tab.data() + P.pass_off[pass];
-  const double* ct = rad + 4 * P.n_r;
+  std::vector<double> ttab(kRadT * P.n_r_pad);
+  for (int i = 0; i < P.n_r_pad; ++i) radial_entry(c, rad[2 * i], &ttab[kRadT * i]);
+  const double* ct = rad + 2 * P.n_r_pad;
   const double* st = ct + P.n_cos;
   const double* wc = st + P.n_cos;
   const double* cph = wc + P.n_cos;
@@ -130,10 +148,10 @@ extern "C" int emu_moments(const no_params* p, const double* cfg, int pass, doub
     const int j = m / P.n_phi, l = m - j * P.n_phi;
     DirConst d;
     dir_setup(c, st[j] * cph[l], st[j] * sph[l], ct[j], d);
-    First<false> f;
-    first_zero<false>(f);
-    for (int i = 0; i < P.n_r; ++i) node<-1, false>(P, c, d, rad[4 * i], rad[4 * i + 1], rad[4 * i + 2], f);
-    second_level<false>(f, d, wc[j] * wph[l], acc.data() + (m & 31));
+    First f;
+    first_zero(f);
+    for (int i = 0; i < P.n_r_pad; i += kNodesPerTrip) trip<-1>(c.rs, P.n_reg, plan.tab.data(), d, rad, ttab.data(), i, f);
+    second_level<false>(f, d, c.gam, wc[j] * wph[l], acc.data() + (m & 31));
   }
   for (int row = 0; row < L::kRows; ++row) {
     double s = 0;

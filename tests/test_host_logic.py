@@ -44,21 +44,24 @@ def test_plan_passes_variants_and_tables():
     base = dict(PHYS, n_r=3, n_cos=4, n_phi=5)
     p = emu.emu_plan(kf_n=1.2, kf_p=0.9, **base)
     assert (p["n_pass"], p["nreg_variant"], p["has_c4"], p["evals_per_cfg"]) == (2, 4, 0, 2 * 60)
-    per = (4 * 3 + 3 * 4 + 3 * 5 + 3) // 4 * 4          # each pass padded to 32 bytes
-    assert p["tab_doubles"] == 2 * per
-    r, wr = O.gauss_legendre(3, 0.0, 0.9)               # pass 0 = protons
+    n_pad = 4                                           # n_r = 3 padded to a multiple of 4 with zero-weight nodes
+    per = (2 * n_pad + 3 * 4 + 3 * 5 + 3) // 4 * 4      # each pass padded to 32 bytes
+    assert p["tab_doubles"] == 64 + 2 * per
     t = p["tab"]
-    assert np.allclose(t[0:12:4], r, rtol=0, atol=3e-16)
-    assert np.allclose(t[1:12:4], r * r, rtol=1e-15)
-    assert np.allclose(t[2:12:4], wr * r * r / (2 * math.pi) ** 3, rtol=1e-14)
+    assert t[0] == 1.0 and np.abs(t[:64] - 2.0 ** (np.arange(64) / 64.0)).max() < 2.3e-16   # 2^(j/64)
+    t = t[64:]
+    r, wr = O.gauss_legendre(3, 0.0, 0.9)               # pass 0 = protons
+    assert np.allclose(t[0:6:2], r, rtol=0, atol=3e-16)
+    assert np.allclose(t[1:6:2], wr * r * r / (2 * math.pi) ** 3, rtol=1e-14)
+    assert t[6] == t[4] and t[7] == 0.0                 # padding node: valid radius, weight 0
     x, wx = O.gauss_legendre(4, -1.0, 1.0)
-    assert np.allclose(t[12:16], x, atol=3e-16) and np.allclose(t[16:20], np.sqrt(1 - x * x), atol=3e-16)
-    assert np.allclose(t[20:24], wx, rtol=1e-14)
+    assert np.allclose(t[8:12], x, atol=3e-16) and np.allclose(t[12:16], np.sqrt(1 - x * x), atol=3e-16)
+    assert np.allclose(t[16:20], wx, rtol=1e-14)
     ph, wp = O.gauss_legendre(5, 0.0, 2 * math.pi)
-    assert np.allclose(t[24:29], np.cos(ph), atol=1e-15) and np.allclose(t[29:34], np.sin(ph), atol=1e-15)
-    assert np.allclose(t[34:39], wp, rtol=1e-14)
+    assert np.allclose(t[20:25], np.cos(ph), atol=1e-15) and np.allclose(t[25:30], np.sin(ph), atol=1e-15)
+    assert np.allclose(t[30:35], wp, rtol=1e-14)
     rn, _ = O.gauss_legendre(3, 0.0, 1.2)               # pass 1 = neutrons
-    assert np.allclose(t[per:per + 12:4], rn, atol=3e-16)
+    assert np.allclose(t[per:per + 6:2], rn, atol=3e-16)
     # equal Fermi momenta share one grid; empty spheres are skipped; regulator variants
     assert emu.emu_plan(kf_n=1.3, kf_p=1.3, **base)["n_pass"] == 1
     assert emu.emu_plan(kf_n=1.3, kf_p=1.3, **base)["evals_per_cfg"] == 60

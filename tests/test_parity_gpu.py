@@ -225,7 +225,7 @@ def test_abi_pointer_checks_streams_and_host_path():
     binding.no_eval_host(h, cfg.ctypes.data, 5, h_out.ctypes.data, s1.cuda_stream)   # smaller batch reuses scratch
     assert np.array_equal(h_out[:5], ref[:5].cpu().numpy())
     info = binding.no_kernel_info(h)
-    assert info["threads"] == 128 and info["cfg_per_cta"] == 4 and info["ctas_per_sm"] >= 1 and info["n_sm"] > 0
+    assert info["threads"] == 32 * info["cfg_per_cta"] and info["cfg_per_cta"] in (1, 2, 4) and info["ctas_per_sm"] >= 1 and info["n_sm"] > 0
     assert binding.no_evals_per_cfg(h) == 8 ** 3
     binding.no_free(h)
     check_parity(torch.view_as_complex(ref).cpu().numpy(), O.normal_order(cfg, **run.params()), "streams")
