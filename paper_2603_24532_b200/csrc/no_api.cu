@@ -28,8 +28,14 @@ int cuda_fail(cudaError_t e, const char* where) {
     if (e_ != cudaSuccess) return cuda_fail(e_, #call); \
   } while (0)
 
-constexpr int kWarps = 2;       // configurations per CTA
-constexpr int kMinBlocks = 6;   // resident CTAs per SM the register allocation must allow
+#ifndef NO_WARPS
+#define NO_WARPS 2
+#endif
+#ifndef NO_MINB
+#define NO_MINB 6
+#endif
+constexpr int kWarps = NO_WARPS;       // configurations per CTA
+constexpr int kMinBlocks = NO_MINB;   // resident CTAs per SM the register allocation must allow
 
 typedef void (*KernelFn)(const DevParams, const double*, long long, double*);
 

@@ -43,8 +43,13 @@ namespace no3n {
 
 constexpr int kLanes = 32;
 constexpr int kMaxRegPoly = 12;   // largest regulator exponent of the generic path
+constexpr int kMaxNr = 128;      // largest radial order (n_r_pad <= kMaxNr)
 constexpr int kExpTab = 64;       // entries of the 2^(j/64) table at the start of the device tables
-constexpr int kNodesPerTrip = 4;  // radial nodes per trip of the hot loop (n_r is padded to a multiple)
+#ifndef NO_NPT
+#define NO_NPT 4
+#endif
+constexpr int kNodesPerTrip = NO_NPT;
+static_assert(128 % NO_NPT == 0, "n_r_pad must not exceed kMaxNr");  // radial nodes per trip of the hot loop (n_r is padded to a multiple)
 
 // kernel-wide constants, all in fm units
 struct DevParams {
@@ -64,6 +69,8 @@ struct DevParams {
   double gE2;             // cE/(fpi^4 Lchi)
   double g4;              // G2 c4/fpi^2
   int n_reg;              // regulator exponent (generic path)
+  double radk[2][kMaxNr][2];  // per pass: (r_i, w_i r_i^2/(2 pi)^3), i < n_r_pad (weight 0 on the padding):
+                              // read in the hot loop through the constant bank (uniform operands)
 };
 
 // table layout: tab[0..64) = 2^(j/64); then for each pass: radial nodes as [n_r_pad][2] =
@@ -259,31 +266,39 @@ NO_HD void radial_entry(const CfgConst& c, double r, double* T) {
   T[5] = 0.0;
 }
 
-// W k3 nodes of one direction at once (the HOT loop body): r, wr = w_r r^2/(2 pi)^3,
-// T = radial_entry.  Every step is written for all W nodes before the next one, so that the W
+// W k3 nodes of one direction at once (the HOT loop body): r, wr = w_r r^2/(2 pi)^3
+// (the same for every lane: the kernel passes them from the constant bank, i.e. as uniform-register
+// operands), T = radial_entry.  Every step is written for all W nodes before the next one, so that the W
 // independent dependency chains interleave in the instruction stream (FP64 latency is 8 cycles at
 // one instruction per 2 cycles).
+//
+// An FP64 instruction with three distinct 64-bit REGISTER operands occupies the pipe for 3 cycles
+// instead of 2 (profiles/r01b.md), so the body is arranged to need at most two: the weight wF is
+// folded into the shared reciprocal, y = wF/(D0 D1 D2 D3), the pair and leg terms are products of y
+// with the D's, the k = 0 sums are plain additions and the k = 1 sums are FMAs with the uniform r.
 template <int NREG, int W>
 NO_HD void nodes(const double* rs, int n_reg, const double* e2tab, const DirConst& d, const double* r,
                  const double* wr, const double (*T)[5], First& f) {
-  double F[W], D0[W], D1[W], D2[W], D3[W], p01[W], p23[W], den[W], x[W];
+  double F[W], D0[W], D1[W], D2[W], D3[W], q02[W], q13[W], q03[W], q12[W], den[W], x[W];
 #pragma unroll
   for (int k = 0; k < W; ++k) {
-    D0[k] = fma(r[k], d.bet[0], T[k][1]);
-    D1[k] = fma(r[k], d.bet[1], T[k][2]);
-    D2[k] = fma(r[k], d.bet[2], T[k][3]);
-    D3[k] = fma(r[k], d.bet[3], T[k][4]);
+    D0[k] = fma(d.bet[0], r[k], T[k][1]);
+    D1[k] = fma(d.bet[1], r[k], T[k][2]);
+    D2[k] = fma(d.bet[2], r[k], T[k][3]);
+    D3[k] = fma(d.bet[3], r[k], T[k][4]);
   }
 #pragma unroll
-  for (int k = 0; k < W; ++k) { p01[k] = D0[k] * D1[k]; p23[k] = D2[k] * D3[k]; }
+  for (int k = 0; k < W; ++k) { q02[k] = D0[k] * D2[k]; q13[k] = D1[k] * D3[k]; }
 #pragma unroll
-  for (int k = 0; k < W; ++k) den[k] = p01[k] * p23[k];
+  for (int k = 0; k < W; ++k) den[k] = q02[k] * q13[k];
 #pragma unroll
   for (int k = 0; k < W; ++k) x[k] = rcp_seed(den[k]);
+#pragma unroll
+  for (int k = 0; k < W; ++k) { q03[k] = D0[k] * D3[k]; q12[k] = D1[k] * D2[k]; }
   if (NREG >= 0) {
     double d2[W], h[W], tm[W], kf[W], fr[W], Ts[W];
 #pragma unroll
-    for (int k = 0; k < W; ++k) d2[k] = fma(r[k], d.betd, T[k][0]);
+    for (int k = 0; k < W; ++k) d2[k] = fma(d.betd, r[k], T[k][0]);
 #pragma unroll
     for (int k = 0; k < W; ++k) h[k] = reg_h<NREG>(rs, n_reg, d2[k]);
 #pragma unroll
@@ -310,45 +325,44 @@ NO_HD void nodes(const double* rs, int n_reg, const double* e2tab, const DirCons
   for (int k = 0; k < W; ++k) e[k] = fma(e[k], e[k], e[k]);
 #pragma unroll
   for (int k = 0; k < W; ++k) x[k] = fma(x[k], e[k], x[k]);
-  // four reciprocals from one
-  double i01[W], i23[W], iD0[W], iD1[W], iD2[W], iD3[W], g0[W], g1[W], g2[W], g3[W], wf[W], wf1[W];
+  double wf[W], y[W], g0[W], g1[W], g2[W], g3[W], i0[W], i1[W], i2[W], i3[W];
 #pragma unroll
-  for (int k = 0; k < W; ++k) { i01[k] = x[k] * p23[k]; i23[k] = x[k] * p01[k]; }
+  for (int k = 0; k < W; ++k) wf[k] = F[k] * wr[k];
+#pragma unroll
+  for (int k = 0; k < W; ++k) y[k] = x[k] * wf[k];
 #pragma unroll
   for (int k = 0; k < W; ++k) {
-    iD0[k] = i01[k] * D1[k]; iD1[k] = i01[k] * D0[k];
-    iD2[k] = i23[k] * D3[k]; iD3[k] = i23[k] * D2[k];
+    g0[k] = y[k] * q13[k];   // wF/(D0 D2): pair 0 = legs (0, 2)
+    g1[k] = y[k] * q02[k];   // wF/(D1 D3): pair 1 = legs (1, 3)
+    g2[k] = y[k] * q12[k];   // wF/(D0 D3): pair 2 = legs (0, 3)
+    g3[k] = y[k] * q03[k];   // wF/(D1 D2): pair 3 = legs (1, 2)
   }
 #pragma unroll
   for (int k = 0; k < W; ++k) {
-    g0[k] = iD0[k] * iD2[k];   // pair 0 = legs (0, 2)
-    g1[k] = iD1[k] * iD3[k];   // pair 1 = legs (1, 3)
-    g2[k] = iD0[k] * iD3[k];   // pair 2 = legs (0, 3)
-    g3[k] = iD1[k] * iD2[k];   // pair 3 = legs (1, 2)
+    i0[k] = g0[k] * D2[k];   // wF/D0
+    i2[k] = g0[k] * D0[k];   // wF/D2
+    i1[k] = g1[k] * D3[k];   // wF/D1
+    i3[k] = g1[k] * D1[k];   // wF/D3
   }
 #pragma unroll
-  for (int k = 0; k < W; ++k) { wf[k] = wr[k] * F[k]; }
-#pragma unroll
-  for (int k = 0; k < W; ++k) { wf1[k] = wf[k] * r[k]; }
-#pragma unroll
   for (int k = 0; k < W; ++k) {
-    f.R0 = fma(wr[k], F[k], f.R0);
-    f.S[0][0] = fma(wf[k], iD0[k], f.S[0][0]);
-    f.S[1][0] = fma(wf[k], iD1[k], f.S[1][0]);
-    f.S[2][0] = fma(wf[k], iD2[k], f.S[2][0]);
-    f.S[3][0] = fma(wf[k], iD3[k], f.S[3][0]);
-    f.G[0][0] = fma(wf[k], g0[k], f.G[0][0]);
-    f.G[1][0] = fma(wf[k], g1[k], f.G[1][0]);
-    f.G[2][0] = fma(wf[k], g2[k], f.G[2][0]);
-    f.G[3][0] = fma(wf[k], g3[k], f.G[3][0]);
-    f.S[0][1] = fma(wf1[k], iD0[k], f.S[0][1]);
-    f.S[1][1] = fma(wf1[k], iD1[k], f.S[1][1]);
-    f.S[2][1] = fma(wf1[k], iD2[k], f.S[2][1]);
-    f.S[3][1] = fma(wf1[k], iD3[k], f.S[3][1]);
-    f.G[0][1] = fma(wf1[k], g0[k], f.G[0][1]);
-    f.G[1][1] = fma(wf1[k], g1[k], f.G[1][1]);
-    f.G[2][1] = fma(wf1[k], g2[k], f.G[2][1]);
-    f.G[3][1] = fma(wf1[k], g3[k], f.G[3][1]);
+    f.R0 += wf[k];
+    f.S[0][0] += i0[k];
+    f.S[1][0] += i1[k];
+    f.S[2][0] += i2[k];
+    f.S[3][0] += i3[k];
+    f.G[0][0] += g0[k];
+    f.G[1][0] += g1[k];
+    f.G[2][0] += g2[k];
+    f.G[3][0] += g3[k];
+    f.S[0][1] = fma(i0[k], r[k], f.S[0][1]);
+    f.S[1][1] = fma(i1[k], r[k], f.S[1][1]);
+    f.S[2][1] = fma(i2[k], r[k], f.S[2][1]);
+    f.S[3][1] = fma(i3[k], r[k], f.S[3][1]);
+    f.G[0][1] = fma(g0[k], r[k], f.G[0][1]);
+    f.G[1][1] = fma(g1[k], r[k], f.G[1][1]);
+    f.G[2][1] = fma(g2[k], r[k], f.G[2][1]);
+    f.G[3][1] = fma(g3[k], r[k], f.G[3][1]);
   }
 }
 

@@ -146,6 +146,8 @@ inline int build_plan(const no_params* p, HostPlan& plan) {
       const int k = i < p->n_r ? i : p->n_r - 1;        // padding node: a valid radius with weight 0
       T[2 * i + 0] = xr[k];
       T[2 * i + 1] = i < p->n_r ? wr[k] * xr[k] * xr[k] * norm : 0.0;
+      d.radk[s][i][0] = T[2 * i + 0];
+      d.radk[s][i][1] = T[2 * i + 1];
     }
     double* A = T + 2 * d.n_r_pad;
     for (int j = 0; j < p->n_cos; ++j) {

@@ -1,8 +1,9 @@
 // no_kernel.cuh -- the sm_100a kernel of the 3N normal ordering.
 //
 // One warp integrates one configuration (p, p', P): lanes stride over the angular directions
-// of the k3 grid, every lane runs the radial loop of its direction, two nodes per trip, with the
-// 17 first-level sums in registers (no3n::node, the hot loop, branch free), folds them into
+// of the k3 grid, every lane runs the radial loop of its direction, kNodesPerTrip nodes per trip, with
+// the 17 first-level sums in registers (no3n::nodes, the hot loop, branch free; the radial nodes and
+// weights are read from the kernel-parameter block, i.e. as uniform-register operands), folds them into
 // lane-private shared-memory accumulators (no3n::second_level), then the warp reduces the 57
 // (81 with c4) moments, turns them into Pauli-operator coefficients and writes the 16x16 complex
 // matrix.  A CTA holds WARPS warps; the 2^(j/64) table and the quadrature tables of every Fermi
@@ -60,7 +61,7 @@ inline size_t smem_bytes(int tab_doubles, int n_r_pad, int warps) {
 
 template <int NREG, bool C4, int WARPS, int MINB>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
-no3n_kernel(const DevParams P, const double* __restrict__ cfg, long long n_cfg, double* __restrict__ out) {
+no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg, long long n_cfg, double* __restrict__ out) {
   extern __shared__ __align__(128) double smem[];
   using L = Layout<C4>;
   double* s_tab = smem;
@@ -117,7 +118,6 @@ no3n_kernel(const DevParams P, const double* __restrict__ cfg, long long n_cfg, 
 
     // ---- a2 + a3: hot loop over the k3 nodes of this sphere ----
     const int n_dir = P.n_cos * P.n_phi;
-    const double2* rad2 = reinterpret_cast<const double2*>(rad);
     const double2* tt2 = reinterpret_cast<const double2*>(ttab);
 #pragma unroll 1
     for (int m = lane; m < n_dir; m += kLanes) {
@@ -133,13 +133,12 @@ no3n_kernel(const DevParams P, const double* __restrict__ cfg, long long n_cfg, 
         double r[kNodesPerTrip], wr[kNodesPerTrip], T[kNodesPerTrip][5];
 #pragma unroll
         for (int k = 0; k < kNodesPerTrip; ++k) {
-          const double2 a = rad2[i + k];
           const double2 t0 = tt2[3 * (i + k)], t1 = tt2[3 * (i + k) + 1];
           const double t2 = ttab[kRadT * (i + k) + 4];
-          r[k] = a.x; wr[k] = a.y;
+          r[k] = P.radk[pass][i + k][0]; wr[k] = P.radk[pass][i + k][1];
           T[k][0] = t0.x; T[k][1] = t0.y; T[k][2] = t1.x; T[k][3] = t1.y; T[k][4] = t2;
         }
-        nodes<NREG, kNodesPerTrip>(rsp, P.n_reg, e2tab, d, r, wr, T, f);
+nodes<NREG, kNodesPerTrip>(rsp, P.n_reg, e2tab, d, r, wr, T, f);
       }
       second_level<C4>(f, d, cc->gam, w, acc + lane);
     }
