@@ -69,6 +69,7 @@ struct DevParams {
   double gE2;             // cE/(fpi^4 Lchi)
   double g4;              // G2 c4/fpi^2
   int n_reg;              // regulator exponent (generic path)
+  double kf_max;          // largest Fermi momentum of the passes
   double radk[2][kMaxNr][2];  // per pass: (r_i, w_i r_i^2/(2 pi)^3), i < n_r_pad (weight 0 on the padding):
                               // read in the hot loop through the constant bank (uniform operands)
 };
@@ -81,9 +82,14 @@ NO_HD int tab_pass_doubles(int n_r_pad, int n_cos, int n_phi) { return (2 * n_r_
 // second-level accumulator rows
 template <bool C4> struct Layout {
   static constexpr int kPairRows = C4 ? 10 : 4;     // Gm0, Gm1[3] (, Gm2[6])
-  static constexpr int kRowLeg = 1;                 // row 0 is R0; leg l at 1 + 10 l: A0, A1[3], A2[6]
-  static constexpr int kRowPair = 41;
-  static constexpr int kRows = 41 + 4 * kPairRows;  // 57 or 81
+  static constexpr int kRowLeg = 0;                 // leg l at 10 l: A0, A1[3], A2[6]
+  static constexpr int kRowPair = 40;               // pair t at 40 + kPairRows t
+  static constexpr int kRowR0 = 40 + 4 * kPairRows; // R0 is the last row
+  static constexpr int kRows = kRowR0 + 1;          // 57 or 81
+  // the accumulators are lane-major in shared memory, acc[lane * kStride + row], and are read and
+  // written as 16-byte pairs; kStride / 2 is odd, so the eight lanes of a quarter warp hit eight
+  // different 16-byte bank groups
+  static constexpr int kStride = kRows + 1;         // 58 or 82
 };
 
 // legs of the four exchange terms.  pair t uses x-leg kPairX[t] (incoming) and y-leg kPairY[t] (outgoing)
@@ -101,7 +107,8 @@ struct CfgConst {
   double cpair[4];    // |kappa_x - kappa_y|^2/2 + mpi^2
   double E0;          // k3-independent part of the regulator exponent
   double rs[kMaxRegPoly];  // s = -64 log2(e) dE = sum_k rs[k-1] (d^2)^k, k = 1..n
-  double pad_[3];     // 40 doubles: keeps what follows in shared memory 32-byte aligned
+  double smin;        // lower bound of s over the Fermi spheres (s at d^2 = (kF_max + |P/2|)^2); NaN if cfg is not finite
+  double pad_[2];     // 40 doubles: keeps what follows in shared memory 32-byte aligned
 };
 constexpr int kCfgDoubles = sizeof(CfgConst) / sizeof(double);
 static_assert(kCfgDoubles == 40, "CfgConst layout");
@@ -135,7 +142,8 @@ NO_HD void cfg_setup(const DevParams& P, const double* cfg, CfgConst& c) {
   // regulator: (X0 + s3 d2)^n + (X1 + s3 d2)^n = E0 + sum_{k=1..n} C(n,k) (X0^(n-k) + X1^(n-k)) s3^k d2^k
   c.E0 = 0;
   for (int k = 0; k < kMaxRegPoly; ++k) c.rs[k] = 0;
-  for (int k = 0; k < 3; ++k) c.pad_[k] = 0;
+  for (int k = 0; k < 2; ++k) c.pad_[k] = 0;
+  c.smin = 0;
   if (NREG >= 0) {
     const int n = NREG > 0 ? NREG : P.n_reg;
     const double X0 = p2 * P.inv_L2, X1 = pp2 * P.inv_L2, s3 = P.inv_L2 * (1.0 / 3.0);
@@ -153,8 +161,17 @@ NO_HD void cfg_setup(const DevParams& P, const double* cfg, CfgConst& c) {
       c.rs[k - 1] = scale * (binom * (px0[n - k] + px1[n - k]) * ps3[k]);
     }
     c.E0 = px0[n] + px1[n];
+    // s = d2 h(d2) decreases with d2 (all rs <= 0); d2 = |k3 - P/2|^2 <= (kF_max + |P/2|)^2
+    const double dmax = P.kf_max + sqrt(c.gamd), d2max = dmax * dmax;
+    double h = c.rs[n - 1];
+    for (int k = n - 2; k >= 0; --k) h = fma(d2max, h, c.rs[k]);
+    c.smin = d2max * h;
   }
 }
+
+// the hot loop may skip the underflow guard of exp2_table when s >= kFlushBelow at every node
+constexpr double kFlushBelow = -65000.0;
+NO_HD bool needs_flush(const CfgConst& c) { return !(c.smin > kFlushBelow); }
 
 // ---- bit access to doubles ----
 NO_HD int hi32(double x) {
@@ -182,7 +199,8 @@ NO_HD double hilo(int hi, int lo) {
 // exp(-dE(d2)) = 2^(s/64), s = d2 * h(d2) <= 0, h = rs0 + d2 (rs1 + ...).  Branch free:
 //   tm = s + 1.5 2^52 holds round(s) in its low mantissa bits, f = s - round(s) in [-1/2, 1/2],
 //   2^(s/64) = 2^(ky >> 6) * tab[ky & 63] * exp(f ln2/64)  (degree-5 Taylor, |error| < 4e-17).
-// Below s = -65000 (exp(-dE) < 1e-305) the result is replaced by a subnormal (< 3e-308), i.e. zero.
+// Below s = -65000 (exp(-dE) < 1e-305) the result is replaced by a subnormal (< 3e-308), i.e. zero
+// (FLUSH); configurations whose bound smin shows that no node gets there run without that guard.
 // The stages are separate functions so that the W nodes of one trip can be interleaved.
 template <int NREG>
 NO_HD double reg_h(const double* rs, int n_reg, double d2) {
@@ -197,12 +215,24 @@ NO_HD double reg_h(const double* rs, int n_reg, double d2) {
 
 constexpr double kMagic = 6755399441055744.0;             // 1.5 * 2^52
 
-// scaled table value 2^(ky/64) from tm = s + kMagic and kf = round(s)
+// scaled table value 2^(ky/64) from tm = s + kMagic and kf = round(s).  Index and exponent are taken
+// with multiply-adds only (n = floor(ky/64) as the high word of ky 2^26): on B200 the logic/shift
+// pipe shares issue bandwidth with the FP64 pipe, the integer multiply-add pipe does not.
+NO_HD int mulhi32(int a, int b) {
+#ifdef __CUDA_ARCH__
+  return __mulhi(a, b);
+#else
+  return (int)(((long long)a * (long long)b) >> 32);
+#endif
+}
+
+template <bool FLUSH>
 NO_HD double exp2_table(double tm, double kf, const double* e2tab) {
   const int ky = lo32(tm);
-  const double T = e2tab[ky & (kExpTab - 1)];
-  int hiT = hi32(T) + (ky >> 6) * 1048576;                // exponent field += floor(ky / 64)
-  hiT = (uint32_t)hi32(kf) > 0xC0EFBD00u ? 0 : hiT;       // kf < -65000 (or not finite): flush
+  const int n = mulhi32(ky, 1 << 26);                     // floor(ky / 64)
+  const double T = e2tab[ky - 64 * n];                    // ky mod 64 in [0, 64)
+  int hiT = hi32(T) + n * 1048576;                        // exponent field += n
+  if (FLUSH) hiT = (uint32_t)hi32(kf) > 0xC0EFBD00u ? 0 : hiT;   // kf < -65000 (or not finite): flush
   return hilo(hiT, lo32(T));
 }
 
@@ -276,7 +306,7 @@ NO_HD void radial_entry(const CfgConst& c, double r, double* T) {
 // instead of 2 (profiles/r01b.md), so the body is arranged to need at most two: the weight wF is
 // folded into the shared reciprocal, y = wF/(D0 D1 D2 D3), the pair and leg terms are products of y
 // with the D's, the k = 0 sums are plain additions and the k = 1 sums are FMAs with the uniform r.
-template <int NREG, int W>
+template <int NREG, int W, bool FLUSH>
 NO_HD void nodes(const double* rs, int n_reg, const double* e2tab, const DirConst& d, const double* r,
                  const double* wr, const double (*T)[5], First& f) {
   double F[W], D0[W], D1[W], D2[W], D3[W], q02[W], q13[W], q03[W], q12[W], den[W], x[W];
@@ -308,7 +338,7 @@ NO_HD void nodes(const double* rs, int n_reg, const double* e2tab, const DirCons
 #pragma unroll
     for (int k = 0; k < W; ++k) fr[k] = fma(d2[k], h[k], -kf[k]);       // s - round(s), one rounding
 #pragma unroll
-    for (int k = 0; k < W; ++k) Ts[k] = exp2_table(tm[k], kf[k], e2tab);
+    for (int k = 0; k < W; ++k) Ts[k] = exp2_table<FLUSH>(tm[k], kf[k], e2tab);
 #pragma unroll
     for (int k = 0; k < W; ++k) F[k] = exp2_poly(fr[k]);
 #pragma unroll
@@ -366,23 +396,29 @@ NO_HD void nodes(const double* rs, int n_reg, const double* e2tab, const DirCons
   }
 }
 
-// second level: acc[row * kLanes + lane] += w_ang * (first-level sum) * (1 | u | u u^T)
+// second level: acc[lane * kStride + row] += w_ang * (first-level sum) * (1 | u | u u^T)
 // The rows are updated in groups (all loads of a group, then the FMAs, then the stores) so that the
 // shared-memory latency is paid once per group; the compiler fences at both ends keep it from
 // carrying the rows in registers across the direction loop.
 #define NO_FENCE() asm volatile("" ::: "memory")
 
-NO_HD void rmw_rank012(double* a /* 10 rows: 1 | u | u u^T */, const double* wt, double s0, double s1, double s2) {
-  double v[10];
-  for (int k = 0; k < 10; ++k) v[k] = a[k * kLanes];
-  v[0] = fma(wt[0], s0, v[0]);
-  for (int k = 1; k < 4; ++k) v[k] = fma(wt[k], s1, v[k]);
-  for (int k = 4; k < 10; ++k) v[k] = fma(wt[k], s2, v[k]);
-  for (int k = 0; k < 10; ++k) a[k * kLanes] = v[k];
+struct alignas(16) Pair { double x, y; };
+
+// a: 10 consecutive rows of one lane (16-byte aligned): 1 | u | u u^T
+NO_HD void rmw_rank012(double* a, const double* wt, double s0, double s1, double s2) {
+  Pair* p = reinterpret_cast<Pair*>(a);
+  Pair v[5];
+  for (int k = 0; k < 5; ++k) v[k] = p[k];
+  v[0].x = fma(wt[0], s0, v[0].x); v[0].y = fma(wt[1], s1, v[0].y);
+  v[1].x = fma(wt[2], s1, v[1].x); v[1].y = fma(wt[3], s1, v[1].y);
+  v[2].x = fma(wt[4], s2, v[2].x); v[2].y = fma(wt[5], s2, v[2].y);
+  v[3].x = fma(wt[6], s2, v[3].x); v[3].y = fma(wt[7], s2, v[3].y);
+  v[4].x = fma(wt[8], s2, v[4].x); v[4].y = fma(wt[9], s2, v[4].y);
+  for (int k = 0; k < 5; ++k) p[k] = v[k];
 }
 
 template <bool C4>
-NO_HD void second_level(const First& f, const DirConst& d, const double* gam, double w, double* acc /* + lane */) {
+NO_HD void second_level(const First& f, const DirConst& d, const double* gam, double w, double* acc /* this lane's rows */) {
   const double ux = d.u[0], uy = d.u[1], uz = d.u[2];
   double wt[10];      // w * (1, ux, uy, uz, ux ux, ux uy, ux uz, uy uy, uy uz, uz uz)
   wt[0] = w; wt[1] = w * ux; wt[2] = w * uy; wt[3] = w * uz;
@@ -390,27 +426,27 @@ NO_HD void second_level(const First& f, const DirConst& d, const double* gam, do
   NO_FENCE();
   for (int l = 0; l < 4; ++l) {
     const double S2 = fma(-gam[l], f.S[l][0], fma(-d.bet[l], f.S[l][1], f.R0));   // sum wF r^2 / D_l
-    rmw_rank012(acc + (Layout<C4>::kRowLeg + 10 * l) * kLanes, wt, f.S[l][0], f.S[l][1], S2);
+    rmw_rank012(acc + Layout<C4>::kRowLeg + 10 * l, wt, f.S[l][0], f.S[l][1], S2);
   }
   if (C4) {
     for (int t = 0; t < 4; ++t) {
       const int x = NO_PAIR_X(t), y = NO_PAIR_Y(t);
       const double G2 = fma(-gam[x], f.G[t][0], fma(-d.bet[x], f.G[t][1], f.S[y][0]));   // sum wF r^2/(D_x D_y)
-      rmw_rank012(acc + (Layout<C4>::kRowPair + 10 * t) * kLanes, wt, f.G[t][0], f.G[t][1], G2);   // Gm0, Gm1, Gm2
+      rmw_rank012(acc + Layout<C4>::kRowPair + 10 * t, wt, f.G[t][0], f.G[t][1], G2);     // Gm0, Gm1, Gm2
     }
-    acc[0] = fma(w, f.R0, acc[0]);
   } else {
-    double v[17];     // R0 and Gm0, Gm1[3] of the four pairs
-    v[0] = acc[0];
-    for (int k = 0; k < 16; ++k) v[1 + k] = acc[(Layout<C4>::kRowPair + k) * kLanes];
-    v[0] = fma(w, f.R0, v[0]);
+    Pair* p = reinterpret_cast<Pair*>(acc + Layout<C4>::kRowPair);   // Gm0, Gm1[3] of the four pairs
+    Pair v[8];
+    for (int k = 0; k < 8; ++k) v[k] = p[k];
     for (int t = 0; t < 4; ++t) {
-      v[1 + 4 * t] = fma(wt[0], f.G[t][0], v[1 + 4 * t]);
-      for (int k = 1; k < 4; ++k) v[1 + 4 * t + k] = fma(wt[k], f.G[t][1], v[1 + 4 * t + k]);
+      v[2 * t].x = fma(wt[0], f.G[t][0], v[2 * t].x);
+      v[2 * t].y = fma(wt[1], f.G[t][1], v[2 * t].y);
+      v[2 * t + 1].x = fma(wt[2], f.G[t][1], v[2 * t + 1].x);
+      v[2 * t + 1].y = fma(wt[3], f.G[t][1], v[2 * t + 1].y);
     }
-    acc[0] = v[0];
-    for (int k = 0; k < 16; ++k) acc[(Layout<C4>::kRowPair + k) * kLanes] = v[1 + k];
+    for (int k = 0; k < 8; ++k) p[k] = v[k];
   }
+  acc[Layout<C4>::kRowR0] = fma(w, f.R0, acc[Layout<C4>::kRowR0]);
   NO_FENCE();
 }
 
@@ -447,7 +483,7 @@ NO_HD void cross(const double* a, const double* b, double* c) {
 
 template <bool C4>
 NO_HD void phase1_job(const DevParams& P, const CfgConst& c, const double* mom, int job, double* rec) {
-  const double R0 = mom[0];
+  const double R0 = mom[Layout<C4>::kRowR0];
   if (job < 4) {
     const int t = job, x = NO_PAIR_X(t), y = NO_PAIR_Y(t);
     double* o = rec + kRecX * t;
@@ -599,30 +635,28 @@ NO_HD int iso_block(int to, int ti) {   // to, ti = 2 t1 + t2; -1 if charge is n
   return -1;
 }
 
-// <a| sigma^mu |b> = (re + i im); returns false if zero
-NO_HD bool pauli_elem(int mu, int a, int b, double& re, double& im) {
+// sum_{mu,nu} coef[g][mu][nu][blk] <ao|sigma^mu|ai> <bo|sigma^nu|bi>, times i for the vector coefficients
+// (exactly one of mu, nu zero).  For given spin projections only two mu contribute: (0, 3) on the
+// diagonal, (1, 2) off it, with <a|1|a> = <a|sigma_x|b> = 1, <a|sigma_z|a> = +1/-1 and
+// <0|sigma_y|1> = -i, <1|sigma_y|0> = +i; every term is coef * i^k, k = ka + kb + kv (mod 4).
+NO_HD void spin_elem(const double* coef, int g, int blk, int ao, int bo, int ai, int bi, double& re, double& im) {
+  const int da = ao ^ ai, db = bo ^ bi;
+  const int mu[2] = {da, 3 - da}, nu[2] = {db, 3 - db};
+  const int ka[2] = {0, da ? (ao ? 1 : 3) : (ao ? 2 : 0)};
+  const int kb[2] = {0, db ? (bo ? 1 : 3) : (bo ? 2 : 0)};
   re = 0; im = 0;
-  if (mu == 0) { if (a != b) return false; re = 1; return true; }
-  if (mu == 3) { if (a != b) return false; re = a == 0 ? 1.0 : -1.0; return true; }
-  if (a == b) return false;
-  if (mu == 1) { re = 1; return true; }
-  im = a == 0 ? -1.0 : 1.0;             // sigma_y[0][1] = -i, [1][0] = +i
-  return true;
-}
-
-NO_HD void spin_elem(const double* coef, int g, int blk, int s1o, int s2o, int s1i, int s2i, double& re, double& im) {
-  re = 0; im = 0;
-  for (int mu = 0; mu < 4; ++mu) {
-    double ar, ai;
-    if (!pauli_elem(mu, s1o, s1i, ar, ai)) continue;
-    for (int nu = 0; nu < 4; ++nu) {
-      double br, bi;
-      if (!pauli_elem(nu, s2o, s2i, br, bi)) continue;
-      const double cf = coef[(16 * g + 4 * mu + nu) * 6 + blk];
-      double pr = ar * br - ai * bi, pi = ar * bi + ai * br;
-      if ((mu == 0) != (nu == 0)) { const double t = pr; pr = -pi; pi = t; }   // vector coefficient: times i
-      re = fma(cf, pr, re);
-      im = fma(cf, pi, im);
+#ifdef __CUDA_ARCH__
+#pragma unroll
+#endif
+  for (int x = 0; x < 2; ++x) {
+#ifdef __CUDA_ARCH__
+#pragma unroll
+#endif
+    for (int y = 0; y < 2; ++y) {
+      const double cf = coef[(16 * g + 4 * mu[x] + nu[y]) * 6 + blk];
+      const int k = ka[x] + kb[y] + (((mu[x] == 0) != (nu[y] == 0)) ? 1 : 0);
+      const double v = (k & 2) ? -cf : cf;
+      if (k & 1) im += v; else re += v;
     }
   }
 }

@@ -121,6 +121,8 @@ inline int build_plan(const no_params* p, HostPlan& plan) {
     if (p->kf_n > 0) passes.push_back({p->kf_n, 1.0, -1.0});
   }
   d.n_pass = (int)passes.size();
+  d.kf_max = 0.0;
+  for (const Pass& q : passes) d.kf_max = q.kf > d.kf_max ? q.kf : d.kf_max;
   plan.n_sph = d.n_pass;
   plan.evals_per_cfg = (long long)p->n_r * p->n_cos * p->n_phi * d.n_pass;
 

@@ -51,12 +51,30 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t phase) {
 template <bool C4> __host__ __device__ constexpr int rows_pad() { return (Layout<C4>::kRows + 3) & ~3; }
 
 template <bool C4> __host__ __device__ inline int warp_doubles(int n_r_pad) {
-  return kCfgDoubles + kRadT * n_r_pad + rows_pad<C4>() + Layout<C4>::kRows * kLanes;
+  return kCfgDoubles + kRadT * n_r_pad + rows_pad<C4>() + Layout<C4>::kStride * kLanes;
 }
 
 template <bool C4>
 inline size_t smem_bytes(int tab_doubles, int n_r_pad, int warps) {
   return sizeof(double) * (size_t)(tab_doubles + 2 + warps * warp_doubles<C4>(n_r_pad));
+}
+
+// radial loop of one direction: kNodesPerTrip independent nodes per trip
+template <int NREG, bool FLUSH>
+__device__ __forceinline__ void radial_loop(const DevParams& P, int pass, const double* rsp, const double* e2tab,
+                                            const DirConst& d, const double2* tt2, const double* ttab, First& f) {
+#pragma unroll 1
+  for (int i = 0; i < P.n_r_pad; i += kNodesPerTrip) {
+    double r[kNodesPerTrip], wr[kNodesPerTrip], T[kNodesPerTrip][5];
+#pragma unroll
+    for (int k = 0; k < kNodesPerTrip; ++k) {
+      const double2 t0 = tt2[3 * (i + k)], t1 = tt2[3 * (i + k) + 1];
+      const double t2 = ttab[kRadT * (i + k) + 4];
+      r[k] = P.radk[pass][i + k][0]; wr[k] = P.radk[pass][i + k][1];
+      T[k][0] = t0.x; T[k][1] = t0.y; T[k][2] = t1.x; T[k][3] = t1.y; T[k][4] = t2;
+    }
+    nodes<NREG, kNodesPerTrip, FLUSH>(rsp, P.n_reg, e2tab, d, r, wr, T, f);
+  }
 }
 
 template <int NREG, bool C4, int WARPS, int MINB>
@@ -99,6 +117,7 @@ no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg,
 #pragma unroll
   for (int k = 0; k < 4; ++k) rs[k] = cc->rs[k];
   const double* rsp = NREG >= 1 ? rs : cc->rs;     // unrolled exponents keep the coefficients in registers
+  const bool flush = NREG >= 0 && needs_flush(*cc);   // warp uniform
   mbar_wait(bar, 0);
   const double* e2tab = s_tab;
 
@@ -112,35 +131,31 @@ no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg,
     const double* sph = cph + P.n_phi;
     const double* wph = sph + P.n_phi;
     for (int i = lane; i < P.n_r_pad; i += kLanes) radial_entry(*cc, rad[2 * i], ttab + kRadT * i);
+    {
+      Pair* z = reinterpret_cast<Pair*>(acc + lane * L::kStride);
 #pragma unroll 1
-    for (int row = 0; row < L::kRows; ++row) acc[row * kLanes + lane] = 0.0;
+      for (int k = 0; k < L::kStride / 2; ++k) z[k] = Pair{0.0, 0.0};
+    }
     __syncwarp();
 
     // ---- a2 + a3: hot loop over the k3 nodes of this sphere ----
     const int n_dir = P.n_cos * P.n_phi;
+    const int dj = kLanes / P.n_phi, dl = kLanes - dj * P.n_phi;   // (j, l) advance by 32 directions per trip
+    int j = lane / P.n_phi, l = lane - j * P.n_phi;
     const double2* tt2 = reinterpret_cast<const double2*>(ttab);
 #pragma unroll 1
     for (int m = lane; m < n_dir; m += kLanes) {
-      const int j = m / P.n_phi, l = m - j * P.n_phi;
       const double sj = st[j];
       DirConst d;
       dir_setup(*cc, sj * cph[l], sj * sph[l], ct[j], d);
       const double w = wc[j] * wph[l];
       First f;
       first_zero(f);
-#pragma unroll 1
-      for (int i = 0; i < P.n_r_pad; i += kNodesPerTrip) {     // kNodesPerTrip independent nodes per trip
-        double r[kNodesPerTrip], wr[kNodesPerTrip], T[kNodesPerTrip][5];
-#pragma unroll
-        for (int k = 0; k < kNodesPerTrip; ++k) {
-          const double2 t0 = tt2[3 * (i + k)], t1 = tt2[3 * (i + k) + 1];
-          const double t2 = ttab[kRadT * (i + k) + 4];
-          r[k] = P.radk[pass][i + k][0]; wr[k] = P.radk[pass][i + k][1];
-          T[k][0] = t0.x; T[k][1] = t0.y; T[k][2] = t1.x; T[k][3] = t1.y; T[k][4] = t2;
-        }
-nodes<NREG, kNodesPerTrip>(rsp, P.n_reg, e2tab, d, r, wr, T, f);
-      }
-      second_level<C4>(f, d, cc->gam, w, acc + lane);
+      if (flush) radial_loop<NREG, true>(P, pass, rsp, e2tab, d, tt2, ttab, f);
+      else radial_loop<NREG, false>(P, pass, rsp, e2tab, d, tt2, ttab, f);
+      second_level<C4>(f, d, cc->gam, w, acc + lane * L::kStride);
+      j += dj; l += dl;
+      if (l >= P.n_phi) { l -= P.n_phi; ++j; }
     }
     __syncwarp();
 
@@ -148,7 +163,7 @@ nodes<NREG, kNodesPerTrip>(rsp, P.n_reg, e2tab, d, r, wr, T, f);
     for (int row = lane; row < L::kRows; row += kLanes) {
       double s = 0.0;
 #pragma unroll 8
-      for (int t = 0; t < kLanes; ++t) s += acc[row * kLanes + ((lane + t) & 31)];
+      for (int t = 0; t < kLanes; ++t) s += acc[((lane + t) & 31) * L::kStride + row];
       mom[row] = s;
     }
     __syncwarp();

@@ -6,6 +6,7 @@
 // CPU path.  It lets the host logic (tables, kernel-variant choice, moment algebra, epilogue) be
 // checked against the oracle on a machine without a GPU.
 #include <cstring>
+#include <cstdint>
 #include <vector>
 
 #include "../paper_2603_24532_b200/csrc/no_host.h"
@@ -15,14 +16,15 @@ using namespace no3n;
 // one trip of the hot loop: the kernel's load pattern followed by no3n::nodes
 template <int NREG>
 static void trip(const double* rs, int n_reg, const double* e2tab, const DirConst& d, const double* rad,
-                 const double* ttab, int i, First& f) {
+                 const double* ttab, int i, First& f, bool flush) {
   double r[kNodesPerTrip], wr[kNodesPerTrip], T[kNodesPerTrip][5];
   for (int k = 0; k < kNodesPerTrip; ++k) {
     r[k] = rad[2 * (i + k)];
     wr[k] = rad[2 * (i + k) + 1];
     for (int q = 0; q < 5; ++q) T[k][q] = ttab[kRadT * (i + k) + q];
   }
-  nodes<NREG, kNodesPerTrip>(rs, n_reg, e2tab, d, r, wr, T, f);
+  if (flush) nodes<NREG, kNodesPerTrip, true>(rs, n_reg, e2tab, d, r, wr, T, f);
+  else nodes<NREG, kNodesPerTrip, false>(rs, n_reg, e2tab, d, r, wr, T, f);
 }
 
 template <int NREG, bool C4>
@@ -31,7 +33,8 @@ static void emu_cfg(const HostPlan& plan, const double* cfg, double* out /*[512]
   const DevParams& P = plan.dp;
   CfgConst c;
   cfg_setup<NREG>(P, cfg, c);
-  std::vector<double> acc(L::kRows * kLanes), mom(L::kRows), rec(kRecDoubles), coef(32 * 6, 0.0);
+  std::vector<double> acc(L::kStride * kLanes + 2), mom(L::kRows), rec(kRecDoubles), coef(32 * 6, 0.0);
+  double* acc16 = acc.data() + ((reinterpret_cast<uintptr_t>(acc.data()) & 15) ? 1 : 0);   // 16-byte aligned rows
   std::vector<double> ttab(kRadT * P.n_r_pad);
   const double* e2tab = plan.tab.data();
   for (int pass = 0; pass < P.n_pass; ++pass) {
@@ -53,14 +56,14 @@ static void emu_cfg(const HostPlan& plan, const double* cfg, double* out /*[512]
         const double w = wc[j] * wph[l];
         First f;
         first_zero(f);
-        for (int i = 0; i < P.n_r_pad; i += kNodesPerTrip) trip<NREG>(c.rs, P.n_reg, e2tab, d, rad, ttab.data(), i, f);
-        second_level<C4>(f, d, c.gam, w, acc.data() + lane);
+        for (int i = 0; i < P.n_r_pad; i += kNodesPerTrip) trip<NREG>(c.rs, P.n_reg, e2tab, d, rad, ttab.data(), i, f, NREG >= 0 && needs_flush(c));
+        second_level<C4>(f, d, c.gam, w, acc16 + lane * L::kStride);
       }
     }
     for (int lane = 0; lane < kLanes; ++lane)
       for (int row = lane; row < L::kRows; row += kLanes) {
         double s = 0.0;
-        for (int t = 0; t < kLanes; ++t) s += acc[row * kLanes + ((lane + t) & 31)];
+        for (int t = 0; t < kLanes; ++t) s += acc16[((lane + t) & 31) * L::kStride + row];
         mom[row] = s;
       }
     for (int lane = 0; lane < 6; ++lane) phase1_job<C4>(P, c, mom.data(), lane, rec.data());
@@ -134,7 +137,8 @@ extern "C" int emu_moments(const no_params* p, const double* cfg, int pass, doub
   const DevParams& P = plan.dp;
   CfgConst c;
   cfg_setup<-1>(P, cfg, c);
-  std::vector<double> acc(L::kRows * kLanes, 0.0);
+  std::vector<double> acc(L::kStride * kLanes + 2, 0.0);
+  double* acc16 = acc.data() + ((reinterpret_cast<uintptr_t>(acc.data()) & 15) ? 1 : 0);
   const double* rad = plan.tab.data() + P.pass_off[pass];
   std::vector<double> ttab(kRadT * P.n_r_pad);
   for (int i = 0; i < P.n_r_pad; ++i) radial_entry(c, rad[2 * i], &ttab[kRadT * i]);
@@ -150,12 +154,12 @@ extern "C" int emu_moments(const no_params* p, const double* cfg, int pass, doub
     dir_setup(c, st[j] * cph[l], st[j] * sph[l], ct[j], d);
     First f;
     first_zero(f);
-    for (int i = 0; i < P.n_r_pad; i += kNodesPerTrip) trip<-1>(c.rs, P.n_reg, plan.tab.data(), d, rad, ttab.data(), i, f);
-    second_level<false>(f, d, c.gam, wc[j] * wph[l], acc.data() + (m & 31));
+    for (int i = 0; i < P.n_r_pad; i += kNodesPerTrip) trip<-1>(c.rs, P.n_reg, plan.tab.data(), d, rad, ttab.data(), i, f, false);
+    second_level<false>(f, d, c.gam, wc[j] * wph[l], acc16 + (m & 31) * L::kStride);
   }
   for (int row = 0; row < L::kRows; ++row) {
     double s = 0;
-    for (int t = 0; t < kLanes; ++t) s += acc[row * kLanes + t];
+    for (int t = 0; t < kLanes; ++t) s += acc16[t * L::kStride + row];
     mom_out[row] = s;
   }
   return NO_OK;

@@ -100,6 +100,20 @@ def test_kernel_arithmetic_on_the_cfg1_distribution():
     check_parity(emu.emu_eval(cfg, **run.params()), want)
 
 
+def test_underflow_guard_path_strong_regulator():
+    """Lambda = 100 MeV: at the far nodes the regulator exponent exceeds 704 (exp(-dE) below the double
+    range) while the near nodes are O(1): the configurations take the guarded (FLUSH) hot loop; a
+    configuration with a mild exponent in the same batch takes the unguarded one."""
+    kw = dict(PHYS, c4=0.0, kf_n=1.4, kf_p=0.8, n_r=6, n_cos=7, n_phi=8)
+    kw.update(Lambda=100.0, n_reg=4)
+    cfg = np.array([[0.05, -0.02, 0.03, -0.04, 0.06, 0.01, 0.6, 0.8, 1.0],
+                    [0.10, 0.05, -0.05, 0.02, -0.08, 0.04, -0.9, 0.5, 0.7],
+                    [0.02, 0.01, 0.03, 0.01, -0.02, 0.02, 0.05, 0.02, -0.03]])
+    want = O.normal_order(cfg, **kw)
+    assert np.abs(want).max(axis=(1, 2)).min() > 1e-30            # the matrices themselves are representable
+    check_parity(emu.emu_eval(cfg, **kw), want)
+
+
 def test_empty_fermi_sea_gives_zero():
     out = emu.emu_eval(np.ones((2, 9)), kf_n=0.0, kf_p=0.0, n_r=2, n_cos=2, n_phi=2, **PHYS)
     assert np.count_nonzero(out) == 0

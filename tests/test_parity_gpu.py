@@ -168,6 +168,24 @@ def test_every_kernel_variant(geo, c4):
     check_parity(gpu_eval(cfg, **kw), O.normal_order(cfg, **kw), f"{geo} c4={c4}")
 
 
+def test_underflow_guard_path_strong_regulator():
+    """Lambda = 100 MeV: far nodes have exp(-dE) below the double range (guarded hot loop, chosen per
+    configuration from a bound on the exponent), near nodes are O(1); mixed with mild configurations."""
+    kw = dict(PHYS, kf_n=1.4, kf_p=0.8, n_r=6, n_cos=7, n_phi=8)
+    kw.update(Lambda=100.0, n_reg=4)
+    cfg = np.array([[0.05, -0.02, 0.03, -0.04, 0.06, 0.01, 0.6, 0.8, 1.0],
+                    [0.02, 0.01, 0.03, 0.01, -0.02, 0.02, 0.05, 0.02, -0.03],
+                    [0.10, 0.05, -0.05, 0.02, -0.08, 0.04, -0.9, 0.5, 0.7],
+                    [0.02, 0.01, 0.03, 0.01, -0.02, 0.02, 0.05, 0.02, -0.03],
+                    [0.01, 0.00, 0.02, 0.00, 0.03, -0.01, 1.2, -1.1, 0.9]])
+    want = O.normal_order(cfg, **kw)
+    assert np.abs(want).max(axis=(1, 2)).min() > 1e-30
+    check_parity(gpu_eval(cfg, **kw), want, "guarded hot loop")
+    # generic exponent, extreme: everything underflows to exactly zero instead of garbage
+    out = gpu_eval(np.full((2, 9), 3.0), **dict(kw, Lambda=50.0, n_reg=12))
+    assert np.count_nonzero(out) == 0
+
+
 def test_degenerate_inputs():
     kw = dict(PHYS, kf_n=1.2, kf_p=0.9, n_r=4, n_cos=4, n_phi=4)
     # empty Fermi sea: exactly zero
