@@ -78,6 +78,24 @@ int no_eval(const no_handle *h, const double *d_cfg, long long n_cfg, double *d_
  * measurement. */
 int no_eval_host(no_handle *h, const double *h_cfg, long long n_cfg, double *h_out, void *cuda_stream);
 
+/* Spin-traced diagonal of the normal-ordered matrix, reduced inside the kernel (the 16x16 matrix is
+ * never written): the integrand of the Hartree-Fock contractions Eq. (1) and Eq. (9),
+ * obtained "by repeatedly normal ordering".  Same arguments as no_eval except
+ *   d_out : DEVICE, [n_cfg][4] doubles, d_out[c][2 t1 + t2] = sum_{s1,s2} Re M_c[a, a],
+ *           a = (s1, s2, t1, t2), t = 0 proton / 1 neutron; 8-byte aligned, dense, caller-owned.
+ * The configurations are arbitrary (for p' = p the diagonal is real by Hermiticity). */
+int no_eval_diag(const no_handle *h, const double *d_cfg, long long n_cfg, double *d_out, void *cuda_stream);
+
+/* 3N Hartree-Fock energy per volume (fm^-4; multiply by hbar c for MeV fm^-3),
+ *   E/V = (1/6) sum_{123} n_1 n_2 n_3 <123| A_123 V_3N |123>        (xi-weights of Eq. (10))
+ * by a second Fermi-sea quadrature over no_eval_diag: particles 1 and 2 run over Gauss-Legendre product
+ * grids (n_r x n_cos x n_phi per Fermi sphere of the handle, fixed lab frame), particle 3 over the
+ * handle's own k3 grid; configuration (p, p', P) = ((k1-k2)/2, (k1-k2)/2, k1+k2).  On the same grids this
+ * equals the brute-force 9-dimensional sum exactly (pin P8).  Generates the pair configurations on the
+ * device in chunks, enqueues on `cuda_stream`, SYNCHRONISES it, and writes the result to the HOST
+ * double *e_over_v.  Allocates and frees its own device scratch. */
+int no_hf_energy(const no_handle *h, int n_r, int n_cos, int n_phi, double *e_over_v, void *cuda_stream);
+
 /* Release the handle and everything it owns.  NULL is a no-op. */
 int no_free(no_handle *h);
 

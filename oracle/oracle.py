@@ -115,6 +115,55 @@ def hf3n_bruteforce(**params) -> float:
     return float(_load().oracle_hf3n_bruteforce(ctypes.byref(_params(params))))
 
 
+def diag_trace(cfg, **params) -> np.ndarray:
+    """D[n_cfg,4]: D[c, 2 t1 + t2] = sum_{s1,s2} Re M_c[a,a], a = 8 s1 + 4 s2 + 2 t1 + t2 (the integrand
+    of the Hartree-Fock contractions Eq. (1), (9)): the definition, from normal_order."""
+    M = normal_order(cfg, **params)
+    D = np.zeros((M.shape[0], 4))
+    for s1 in range(2):
+        for s2 in range(2):
+            for t in range(4):
+                a = 8 * s1 + 4 * s2 + t
+                D[:, t] += M[:, a, a].real
+    return D
+
+
+def sphere_nodes(n_r: int, n_cos: int, n_phi: int, kf: float):
+    """Product Gauss-Legendre grid of one Fermi sphere (fixed lab frame): k[n,3], W[n] = r^2 w_r w_c w_phi/(2 pi)^3."""
+    r, wr = gauss_legendre(n_r, 0.0, kf)
+    x, wx = gauss_legendre(n_cos, -1.0, 1.0)
+    ph, wp = gauss_legendre(n_phi, 0.0, 2.0 * np.pi)
+    k, w = [], []
+    for i in range(n_r):
+        for j in range(n_cos):
+            for l in range(n_phi):
+                st = np.sqrt(1.0 - x[j] ** 2)
+                k.append(r[i] * np.array([st * np.cos(ph[l]), st * np.sin(ph[l]), x[j]]))
+                w.append(r[i] ** 2 * wr[i] * wx[j] * wp[l] / (2.0 * np.pi) ** 3)
+    return np.array(k), np.array(w)
+
+
+def hf_energy(n_r12: int, n_cos12: int, n_phi12: int, **params) -> float:
+    """3N Hartree-Fock energy per volume (fm^-4) by repeated normal ordering:
+    E/V = (1/6) sum_{t1 t2} sum_{k1 in S(t1)} sum_{k2 in S(t2)} W1 W2 sum_{s1 s2} M(p=(k1-k2)/2, p'=p, P=k1+k2)[a,a],
+    particles 1, 2 on n_r12 x n_cos12 x n_phi12 grids, particle 3 inside M on the grid of `params`."""
+    kf = {0: params.get("kf_p", 0.0), 1: params.get("kf_n", 0.0)}
+    e = 0.0
+    for t1 in (0, 1):
+        for t2 in (0, 1):
+            if kf[t1] <= 0 or kf[t2] <= 0:
+                continue
+            k1, w1 = sphere_nodes(n_r12, n_cos12, n_phi12, kf[t1])
+            k2, w2 = sphere_nodes(n_r12, n_cos12, n_phi12, kf[t2])
+            cfg = np.empty((len(k1), len(k2), 9))
+            cfg[:, :, 0:3] = (k1[:, None, :] - k2[None, :, :]) / 2
+            cfg[:, :, 3:6] = cfg[:, :, 0:3]
+            cfg[:, :, 6:9] = k1[:, None, :] + k2[None, :, :]
+            D = diag_trace(cfg.reshape(-1, 9), **params)[:, 2 * t1 + t2]
+            e += float(np.sum((w1[:, None] * w2[None, :]).reshape(-1) * D))
+    return e / 6.0
+
+
 def num_threads() -> int:
     return int(_load().oracle_num_threads())
 

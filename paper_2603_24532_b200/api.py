@@ -47,6 +47,19 @@ class NormalOrdering:
         s = stream if stream is not None else torch.cuda.current_stream(cfg.device)
         binding.no_eval(self._h, cfg.data_ptr(), n, out.data_ptr(), s.cuda_stream)
 
+    def diag(self, cfg: torch.Tensor) -> torch.Tensor:
+        """no_eval_diag: spin-traced diagonal per isospin pair, float64 [n, 4] (pp, pn, np, nn) on the device."""
+        assert cfg.is_cuda
+        cfg = cfg.to(torch.float64).contiguous().reshape(-1, 9)
+        n = cfg.shape[0]
+        out = torch.empty((n, 4), dtype=torch.float64, device=cfg.device)
+        binding.no_eval_diag(self._h, cfg.data_ptr(), n, out.data_ptr(), torch.cuda.current_stream(cfg.device).cuda_stream)
+        return out
+
+    def hf_energy(self, n_r: int, n_cos: int, n_phi: int) -> float:
+        """no_hf_energy: 3N Hartree-Fock energy per volume (fm^-4) on the given grids for particles 1 and 2."""
+        return binding.no_hf_energy(self._h, n_r, n_cos, n_phi, torch.cuda.current_stream(self.device).cuda_stream)
+
     def __call__(self, cfg: torch.Tensor) -> torch.Tensor:
         cfg = cfg.to(torch.float64).contiguous().reshape(-1, 9)
         n = cfg.shape[0]

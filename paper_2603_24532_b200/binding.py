@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libno3n.so")
 
 NO_OK, NO_ERR_INVALID, NO_ERR_CUDA, NO_ERR_ALLOC = 0, 1, 2, 3
 
-EXPORTS = ("no_init", "no_eval", "no_eval_host", "no_free", "no_strerror", "no_last_cuda_error",
+EXPORTS = ("no_init", "no_eval", "no_eval_host", "no_eval_diag", "no_hf_energy", "no_free", "no_strerror", "no_last_cuda_error",
            "no_kernel_info", "no_evals_per_cfg", "no_probe_fp64_peak")
 
 
@@ -50,6 +50,9 @@ def load() -> ctypes.CDLL:
         lib.no_init.argtypes = [ctypes.POINTER(H), ctypes.POINTER(no_params)]
         lib.no_eval.argtypes = [H, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]
         lib.no_eval_host.argtypes = [H, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]
+        lib.no_eval_diag.argtypes = [H, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]
+        lib.no_hf_energy.argtypes = [H, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double),
+                                     ctypes.c_void_p]
         lib.no_free.argtypes = [H]
         lib.no_strerror.argtypes = [ctypes.c_int]
         lib.no_strerror.restype = ctypes.c_char_p
@@ -60,7 +63,8 @@ def load() -> ctypes.CDLL:
         lib.no_evals_per_cfg.restype = ctypes.c_longlong
         lib.no_probe_fp64_peak.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double), ip,
                                            ctypes.c_void_p]
-        for name in ("no_init", "no_eval", "no_eval_host", "no_free", "no_kernel_info", "no_probe_fp64_peak"):
+        for name in ("no_init", "no_eval", "no_eval_host", "no_eval_diag", "no_hf_energy", "no_free", "no_kernel_info",
+                     "no_probe_fp64_peak"):
             getattr(lib, name).restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -90,6 +94,23 @@ def no_eval_host(h, h_cfg_ptr: int, n_cfg: int, h_out_ptr: int, stream_ptr: Opti
                              ctypes.c_void_p(stream_ptr or 0))
     if rc != NO_OK:
         raise NoError(rc, "no_eval_host")
+
+
+def no_eval_diag(h, d_cfg_ptr: int, n_cfg: int, d_out_ptr: int, stream_ptr: Optional[int] = None) -> None:
+    """no_eval_diag with raw DEVICE pointers: d_out is [n_cfg][4] doubles."""
+    rc = load().no_eval_diag(h, ctypes.c_void_p(d_cfg_ptr), n_cfg, ctypes.c_void_p(d_out_ptr),
+                             ctypes.c_void_p(stream_ptr or 0))
+    if rc != NO_OK:
+        raise NoError(rc, "no_eval_diag")
+
+
+def no_hf_energy(h, n_r: int, n_cos: int, n_phi: int, stream_ptr: Optional[int] = None) -> float:
+    """no_hf_energy: 3N Hartree-Fock energy per volume in fm^-4 (synchronises the stream)."""
+    e = ctypes.c_double(0.0)
+    rc = load().no_hf_energy(h, n_r, n_cos, n_phi, ctypes.byref(e), ctypes.c_void_p(stream_ptr or 0))
+    if rc != NO_OK:
+        raise NoError(rc, "no_hf_energy")
+    return float(e.value)
 
 
 def no_free(h) -> None:

@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "../../include/no.h"
 #include "no_host.h"
@@ -37,7 +38,7 @@ int cuda_fail(cudaError_t e, const char* where) {
 constexpr int kWarps = NO_WARPS;       // configurations per CTA
 constexpr int kMinBlocks = NO_MINB;   // resident CTAs per SM the register allocation must allow
 
-typedef void (*KernelFn)(const DevParams, const double*, long long, double*);
+typedef void (*KernelFn)(const DevParams, const double*, long long, double*, int);
 
 struct Variant {
   KernelFn fn;
@@ -92,10 +93,11 @@ struct DeviceGuard {
   }
 };
 
-int launch(const no_handle* h, const double* d_cfg, long long n_cfg, double* d_out, cudaStream_t s) {
+int launch(const no_handle* h, const double* d_cfg, long long n_cfg, double* d_out, cudaStream_t s,
+           int mode = kModeFull) {
   const long long blocks = (n_cfg + kWarps - 1) / kWarps;
   if (blocks > 2147483647LL) return NO_ERR_INVALID;
-  h->var.fn<<<(unsigned)blocks, kWarps * 32, h->var.smem, s>>>(h->plan.dp, d_cfg, n_cfg, d_out);
+  h->var.fn<<<(unsigned)blocks, kWarps * 32, h->var.smem, s>>>(h->plan.dp, d_cfg, n_cfg, d_out, mode);
   NO_CUDA(cudaGetLastError());
   return NO_OK;
 }
@@ -120,7 +122,13 @@ int no_init(no_handle** out, const no_params* p) {
   if (!guard.ok) { delete h; return cuda_fail(cudaGetLastError(), "cudaSetDevice"); }
   h->var = h->plan.has_c4 ? pick_nreg<true>(h->plan.nreg_variant, h->plan.dp.tab_doubles, h->plan.dp.n_r_pad)
                           : pick_nreg<false>(h->plan.nreg_variant, h->plan.dp.tab_doubles, h->plan.dp.n_r_pad);
-  e = cudaFuncSetAttribute((const void*)h->var.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->var.smem);
+  // the limit is a property of the kernel, shared by every handle that uses the same variant: raise it
+  // to the device maximum once, so that handles with different table sizes never lower it for each other
+  int smem_optin = 0;
+  e = cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->device);
+  if (e != cudaSuccess) { delete h; return cuda_fail(e, "cudaDeviceGetAttribute(smem optin)"); }
+  if (h->var.smem > (size_t)smem_optin) { delete h; return NO_ERR_INVALID; }
+  e = cudaFuncSetAttribute((const void*)h->var.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
   if (e != cudaSuccess) { delete h; return cuda_fail(e, "cudaFuncSetAttribute(smem)"); }
   const size_t bytes = sizeof(double) * (size_t)(h->plan.dp.tab_doubles > 0 ? h->plan.dp.tab_doubles : 2);
   e = cudaMalloc((void**)&h->d_tab, bytes);
@@ -142,6 +150,72 @@ int no_eval(const no_handle* h, const double* d_cfg, long long n_cfg, double* d_
   DeviceGuard guard(h->device);
   if (!guard.ok) return cuda_fail(cudaGetLastError(), "cudaSetDevice");
   return launch(h, d_cfg, n_cfg, d_out, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int no_eval_diag(const no_handle* h, const double* d_cfg, long long n_cfg, double* d_out, void* cuda_stream) {
+  if (!h || n_cfg < 0) return NO_ERR_INVALID;
+  if (n_cfg == 0) return NO_OK;
+  if (!d_cfg || !d_out) return NO_ERR_INVALID;
+  if ((reinterpret_cast<uintptr_t>(d_cfg) & 7u) || (reinterpret_cast<uintptr_t>(d_out) & 7u)) return NO_ERR_INVALID;
+  DeviceGuard guard(h->device);
+  if (!guard.ok) return cuda_fail(cudaGetLastError(), "cudaSetDevice");
+  return launch(h, d_cfg, n_cfg, d_out, static_cast<cudaStream_t>(cuda_stream), kModeDiag);
+}
+
+int no_hf_energy(const no_handle* h, int n_r, int n_cos, int n_phi, double* e_over_v, void* cuda_stream) {
+  if (!h || !e_over_v) return NO_ERR_INVALID;
+  if (n_r < 1 || n_r > kMaxOrder || n_cos < 1 || n_cos > kMaxOrder || n_phi < 1 || n_phi > kMaxOrder) return NO_ERR_INVALID;
+  DeviceGuard guard(h->device);
+  if (!guard.ok) return cuda_fail(cudaGetLastError(), "cudaSetDevice");
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  // single-particle grids of the two species (t = 0 proton, 1 neutron), [n][4] = (kx, ky, kz, W)
+  const double kf[2] = {h->plan.kf_p, h->plan.kf_n};
+  std::vector<double> nodes[2];
+  for (int t = 0; t < 2; ++t)
+    if (kf[t] > 0) sphere_nodes(n_r, n_cos, n_phi, kf[t], nodes[t]);
+  const long long n1 = (long long)n_r * n_cos * n_phi;
+  const long long chunk = n1 * n1 < (1LL << 20) ? n1 * n1 : (1LL << 20);
+  double *d_nodes[2] = {nullptr, nullptr}, *d_cfg = nullptr, *d_w = nullptr, *d_diag = nullptr, *d_acc = nullptr;
+  int rc = NO_OK;
+  cudaError_t e = cudaSuccess;
+  auto cleanup = [&]() {
+    for (int t = 0; t < 2; ++t) if (d_nodes[t]) cudaFree(d_nodes[t]);
+    if (d_cfg) cudaFree(d_cfg);
+    if (d_w) cudaFree(d_w);
+    if (d_diag) cudaFree(d_diag);
+    if (d_acc) cudaFree(d_acc);
+  };
+#define NO_HF_CUDA(call) do { e = (call); if (e != cudaSuccess) { rc = cuda_fail(e, #call); cleanup(); return rc; } } while (0)
+  for (int t = 0; t < 2; ++t)
+    if (kf[t] > 0) {
+      NO_HF_CUDA(cudaMalloc((void**)&d_nodes[t], sizeof(double) * 4 * (size_t)n1));
+      NO_HF_CUDA(cudaMemcpyAsync(d_nodes[t], nodes[t].data(), sizeof(double) * 4 * (size_t)n1, cudaMemcpyHostToDevice, s));
+    }
+  NO_HF_CUDA(cudaMalloc((void**)&d_cfg, sizeof(double) * 9 * (size_t)chunk));
+  NO_HF_CUDA(cudaMalloc((void**)&d_w, sizeof(double) * (size_t)chunk));
+  NO_HF_CUDA(cudaMalloc((void**)&d_diag, sizeof(double) * 4 * (size_t)chunk));
+  NO_HF_CUDA(cudaMalloc((void**)&d_acc, sizeof(double)));
+  NO_HF_CUDA(cudaMemsetAsync(d_acc, 0, sizeof(double), s));
+  for (int t1 = 0; t1 < 2; ++t1)
+    for (int t2 = 0; t2 < 2; ++t2) {
+      if (!(kf[t1] > 0) || !(kf[t2] > 0)) continue;
+      for (long long c0 = 0; c0 < n1 * n1; c0 += chunk) {
+        const long long count = n1 * n1 - c0 < chunk ? n1 * n1 - c0 : chunk;
+        hf_pairs_kernel<<<(unsigned)((count + 255) / 256), 256, 0, s>>>(d_nodes[t1], d_nodes[t2], n1, c0, count, d_cfg, d_w);
+        NO_HF_CUDA(cudaGetLastError());
+        rc = launch(h, d_cfg, count, d_diag, s, kModeDiag);
+        if (rc != NO_OK) { cleanup(); return rc; }
+        hf_reduce_kernel<<<1, 1024, 0, s>>>(d_diag, d_w, count, 2 * t1 + t2, d_acc);
+        NO_HF_CUDA(cudaGetLastError());
+      }
+    }
+  double acc = 0.0;
+  NO_HF_CUDA(cudaMemcpyAsync(&acc, d_acc, sizeof(double), cudaMemcpyDeviceToHost, s));
+  NO_HF_CUDA(cudaStreamSynchronize(s));
+#undef NO_HF_CUDA
+  cleanup();
+  *e_over_v = acc / 6.0;
+  return NO_OK;
 }
 
 int no_eval_host(no_handle* h, const double* h_cfg, long long n_cfg, double* h_out, void* cuda_stream) {

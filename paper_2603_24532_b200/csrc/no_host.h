@@ -73,8 +73,31 @@ struct HostPlan {
   int nreg_variant;           // -1 unregulated, 0 generic, 1..4 unrolled
   bool has_c4;
   int n_sph;                  // distinct non-zero Fermi momenta
+  double kf_n, kf_p;          // Fermi momenta as given (fm^-1)
   long long evals_per_cfg;
 };
+
+// product Gauss-Legendre grid of one Fermi sphere, [n_r n_cos n_phi][4] = (kx, ky, kz, W),
+// W = r^2 w_r w_cos w_phi / (2 pi)^3 (hole sum Eq. (6), fixed lab frame: readings R7, R11, R13)
+inline void sphere_nodes(int n_r, int n_cos, int n_phi, double kf, std::vector<double>& out) {
+  const double pi = 3.14159265358979323846;
+  const double norm = 1.0 / (8.0 * pi * pi * pi);
+  std::vector<double> xr, wr, xc, wc, xp, wp;
+  gl_rule(n_r, 0.0, kf, xr, wr);
+  gl_rule(n_cos, -1.0, 1.0, xc, wc);
+  gl_rule(n_phi, 0.0, 2.0 * pi, xp, wp);
+  out.resize(4 * (size_t)n_r * n_cos * n_phi);
+  size_t m = 0;
+  for (int i = 0; i < n_r; ++i)
+    for (int j = 0; j < n_cos; ++j)
+      for (int l = 0; l < n_phi; ++l, ++m) {
+        const double st = std::sqrt((1.0 - xc[j]) * (1.0 + xc[j]));
+        out[4 * m + 0] = xr[i] * st * std::cos(xp[l]);
+        out[4 * m + 1] = xr[i] * st * std::sin(xp[l]);
+        out[4 * m + 2] = xr[i] * xc[j];
+        out[4 * m + 3] = xr[i] * xr[i] * wr[i] * wc[j] * wp[l] * norm;
+      }
+}
 
 inline bool finite_all(const no_params& p) {
   const double v[] = {p.kf_n, p.kf_p, p.c1, p.c3, p.c4, p.cD, p.cE, p.gA, p.fpi, p.mpi, p.lambda_chi, p.Lambda};
@@ -120,6 +143,8 @@ inline int build_plan(const no_params* p, HostPlan& plan) {
     if (p->kf_p > 0) passes.push_back({p->kf_p, 1.0, +1.0});
     if (p->kf_n > 0) passes.push_back({p->kf_n, 1.0, -1.0});
   }
+  plan.kf_n = p->kf_n;
+  plan.kf_p = p->kf_p;
   d.n_pass = (int)passes.size();
   d.kf_max = 0.0;
   for (const Pass& q : passes) d.kf_max = q.kf > d.kf_max ? q.kf : d.kf_max;

@@ -18,6 +18,9 @@
 
 namespace no3n {
 
+constexpr int kModeFull = 0;   // out[n_cfg][16][16][2]
+constexpr int kModeDiag = 1;   // out[n_cfg][4]
+
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return static_cast<uint32_t>(__cvta_generic_to_shared(p));
 }
@@ -79,7 +82,8 @@ __device__ __forceinline__ void radial_loop(const DevParams& P, int pass, const 
 
 template <int NREG, bool C4, int WARPS, int MINB>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
-no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg, long long n_cfg, double* __restrict__ out) {
+no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg, long long n_cfg, double* __restrict__ out,
+            int mode) {
   extern __shared__ __align__(128) double smem[];
   using L = Layout<C4>;
   double* s_tab = smem;
@@ -181,6 +185,16 @@ no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg,
 #pragma unroll
   for (int b = 0; b < 6; ++b) coef[lane * 6 + b] = blk[b];
   __syncwarp();
+  if (mode == kModeDiag) {
+    // spin-traced diagonal per isospin pair: out[ic][2 t1 + t2] = sum_{s1 s2} Re M[(s1 s2 t1 t2), (s1 s2 t1 t2)]
+    // (the input of the Hartree-Fock contraction, Eq. (1)/(9): the 16x16 matrix never leaves the SM)
+    double re = 0.0, im = 0.0;
+    if (lane < 16) phase3_elem(coef, lane, lane, re, im);
+    re += __shfl_xor_sync(0xffffffffu, re, 4);
+    re += __shfl_xor_sync(0xffffffffu, re, 8);
+    if (lane < 4) out[ic * 4 + lane] = re;
+    return;
+  }
   double2* o = reinterpret_cast<double2*>(out) + ic * 256;
 #pragma unroll 1
   for (int it = 0; it < 8; ++it) {
@@ -189,6 +203,41 @@ no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg,
     phase3_elem(coef, row, col, re, im);
     o[row * 16 + col] = make_double2(re, im);
   }
+}
+
+// ---- Hartree-Fock contraction helpers ----
+// configurations of the node pairs [c0, c0 + count) of two single-particle grids: pair c = i1 * n2 + i2,
+// (p, p', P) = ((k1 - k2)/2, (k1 - k2)/2, k1 + k2), weight W1 W2.  nodes: [n][4] = (kx, ky, kz, W).
+__global__ void hf_pairs_kernel(const double* __restrict__ nodes1, const double* __restrict__ nodes2, long long n2,
+                                long long c0, long long count, double* __restrict__ cfg, double* __restrict__ w) {
+  const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= count) return;
+  const long long pair = c0 + c, i1 = pair / n2, i2 = pair - i1 * n2;
+  const double* a = nodes1 + 4 * i1;
+  const double* b = nodes2 + 4 * i2;
+#pragma unroll
+  for (int x = 0; x < 3; ++x) {
+    const double p = 0.5 * (a[x] - b[x]);
+    cfg[9 * c + x] = p;
+    cfg[9 * c + 3 + x] = p;
+    cfg[9 * c + 6 + x] = a[x] + b[x];
+  }
+  w[c] = a[3] * b[3];
+}
+
+// acc[0] += sum_c w[c] diag[c][blk], one CTA, fixed summation order (bit reproducible)
+__global__ void __launch_bounds__(1024) hf_reduce_kernel(const double* __restrict__ diag, const double* __restrict__ w,
+                                                         long long count, int blk, double* __restrict__ acc) {
+  __shared__ double sh[1024];
+  double s = 0.0;
+  for (long long c = threadIdx.x; c < count; c += 1024) s = fma(w[c], diag[4 * c + blk], s);
+  sh[threadIdx.x] = s;
+  __syncthreads();
+  for (int half = 512; half > 0; half >>= 1) {
+    if ((int)threadIdx.x < half) sh[threadIdx.x] += sh[threadIdx.x + half];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) acc[0] += sh[0];
 }
 
 // ---- FP64 roofline probe: 16 independent DFMA chains per thread ----

@@ -420,3 +420,39 @@ def test_regulator_reduces_to_the_normal_ordering_form():
         want = math.exp(-((p @ p + d2 / 3) / L2) ** n - ((pp @ pp + d2 / 3) / L2) ** n)
         i = np.unravel_index(np.abs(bare).argmax(), bare.shape)
         assert (reg[i] / bare[i]).real == pytest.approx(want, rel=1e-14)
+
+
+# ----------------------------------------------------------------------------------------------
+# the Hartree-Fock contraction functions of the oracle against what fixes them
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("geo", [dict(kf_n=1.2, kf_p=0.9), dict(kf_n=0.0, kf_p=1.0), dict(kf_n=1.1, kf_p=1.1)])
+def test_hf_energy_function_equals_brute_force_on_equal_grids(geo):
+    """pin P8 for O.hf_energy: exact reordering of the 9-D sum when all three particles share the grid."""
+    kw = dict(PHYS, c4=5.4, n_r=2, n_cos=3, n_phi=2, **geo)
+    e_brute = O.hf3n_bruteforce(**kw)
+    e_no = O.hf_energy(2, 3, 2, **kw)
+    assert abs(e_brute) > 1e-8
+    assert e_no == pytest.approx(e_brute, rel=1e-12)
+
+
+def test_hf_energy_function_cE_closed_form():
+    """pin P2 for O.hf_energy: unregulated contact term in SNM, E/V = -(3/16) cE rho^3/(fpi^4 Lchi), any grids >= 2."""
+    kF = 1.33
+    kw = dict(kf_n=kF, kf_p=kF, cE=-0.5, gA=1.27, fpi=92.4, mpi=138.04, lambda_chi=700.0, Lambda=-1.0,
+              n_r=3, n_cos=2, n_phi=2)
+    hbarc = 197.3269804
+    rho = 2 * kF ** 3 / (3 * math.pi ** 2)
+    want = -(3.0 / 16.0) * (-0.5) * rho ** 3 / ((92.4 / hbarc) ** 4 * (700.0 / hbarc))
+    assert O.hf_energy(2, 2, 3, **kw) == pytest.approx(want, rel=1e-12)
+
+
+def test_diag_trace_is_the_spin_trace_of_the_diagonal():
+    kw = dict(PHYS, kf_n=1.2, kf_p=0.9, n_r=2, n_cos=2, n_phi=2)
+    cfg = RNG.uniform(-1, 1, (3, 9))
+    M = O.normal_order(cfg, **kw)
+    D = O.diag_trace(cfg, **kw)
+    for t1 in range(2):
+        for t2 in range(2):
+            want = sum(M[:, idx(s1, s2, t1, t2), idx(s1, s2, t1, t2)].real for s1 in range(2) for s2 in range(2))
+            assert np.allclose(D[:, 2 * t1 + t2], want, rtol=0, atol=1e-15)
+    assert np.abs(np.trace(M, axis1=1, axis2=2).real - D.sum(axis=1)).max() < 1e-14

@@ -251,6 +251,72 @@ def test_abi_pointer_checks_streams_and_host_path():
         binding.no_init(device=99, **run.params())
 
 
+def test_handles_with_different_shared_memory_sizes_coexist():
+    """Two handles on the same kernel variant, the larger table set created first: the dynamic shared
+    memory limit is a property of the kernel, not of the handle that set it last."""
+    kw2 = dict(PHYS, kf_n=1.4, kf_p=0.8, n_r=24, n_cos=20, n_phi=20)     # two spheres: larger tables
+    kw1 = dict(PHYS, kf_n=1.4, kf_p=0.0, n_r=4, n_cos=4, n_phi=4)
+    big, small = NormalOrdering(device=0, **kw2), NormalOrdering(device=0, **kw1)
+    cfg = W.momentum_configurations(6, 1, 3, 1.5, 2.0)
+    got = big(torch.from_numpy(cfg).cuda()).cpu().numpy()
+    torch.cuda.synchronize()
+    check_parity(got, O.normal_order(cfg, **kw2), "big handle after small init")
+    big.close(); small.close()
+
+
+# ----------------------------------------------------------------------------------------------
+# Hartree-Fock contraction on the device (SURVEY.md 8(f) f1)
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("geo", [dict(kf_n=1.3, kf_p=0.9), dict(kf_n=1.33, kf_p=1.33), dict(kf_n=1.2, kf_p=0.0)])
+def test_diag_trace_matches_oracle(geo):
+    kw = dict(PHYS, c4=5.4, n_r=6, n_cos=5, n_phi=7, **geo)
+    cfg = W.momentum_configurations(11, 2, 37, 1.5, 2.0)
+    cfg[:20, 3:6] = cfg[:20, 0:3]                               # forward configurations p' = p, and generic ones
+    no = NormalOrdering(device=0, **kw)
+    got = no.diag(torch.from_numpy(cfg).cuda()).cpu().numpy()
+    full = no(torch.from_numpy(cfg).cuda()).cpu().numpy()
+    no.close()
+    want = O.diag_trace(cfg, **kw)
+    scale = np.abs(O.normal_order(cfg, **kw)).max(axis=(1, 2))[:, None]
+    assert np.abs(got - want).max() / scale.max() < 1e-13
+    assert (np.abs(got - want) <= 1e-12 * scale).all()          # relative to each matrix maximum
+    mask = np.abs(want) > 1e-6 * scale
+    assert (np.abs(got - want)[mask] / np.abs(want)[mask]).max() < 1e-10
+    idx4 = [[8 * s1 + 4 * s2 + t for s1 in range(2) for s2 in range(2)] for t in range(4)]
+    from_full = np.stack([sum(full[:, a, a].real for a in idx4[t]) for t in range(4)], axis=1)
+    assert (np.abs(got - from_full) <= 1e-14 * scale).all()     # same kernel, same coefficients
+
+
+@pytest.mark.parametrize("geo", [dict(kf_n=1.2, kf_p=0.9), dict(kf_n=1.1, kf_p=1.1), dict(kf_n=0.0, kf_p=1.0)])
+def test_hf_energy_equals_brute_force_9d_sum(geo):
+    """pin P8 on the device: all three particles on the same tiny grids."""
+    kw = dict(PHYS, c4=5.4, n_r=2, n_cos=3, n_phi=2, **geo)
+    no = NormalOrdering(device=0, **kw)
+    got = no.hf_energy(2, 3, 2)
+    no.close()
+    want = O.hf3n_bruteforce(**kw)
+    assert abs(want) > 1e-8
+    assert got == pytest.approx(want, rel=1e-11)
+
+
+def test_hf_energy_matches_oracle_contraction_and_closed_form():
+    kw = dict(PHYS, kf_n=1.4, kf_p=1.0, n_r=5, n_cos=4, n_phi=6)
+    no = NormalOrdering(device=0, **kw)
+    got = no.hf_energy(3, 4, 3)                                 # grids of particles 1, 2 differ from the k3 grid
+    assert got == no.hf_energy(3, 4, 3)                         # fixed summation order: bit reproducible
+    no.close()
+    assert got == pytest.approx(O.hf_energy(3, 4, 3, **kw), rel=1e-11)
+    # P2: unregulated contact term in symmetric matter, E/V = -(3/16) cE rho^3 / (fpi^4 Lchi); chunked pair loop
+    kF, hbarc = 1.33, 197.3269804
+    kc = dict(kf_n=kF, kf_p=kF, c1=0.0, c3=0.0, c4=0.0, cD=0.0, cE=-0.5, gA=1.27, fpi=92.4, mpi=138.04,
+              lambda_chi=700.0, Lambda=-1.0, n_r=2, n_cos=2, n_phi=2)
+    rho = 2 * kF ** 3 / (3 * np.pi ** 2)
+    want = -(3.0 / 16.0) * (-0.5) * rho ** 3 / ((92.4 / hbarc) ** 4 * (700.0 / hbarc))
+    no = NormalOrdering(device=0, **kc)
+    assert no.hf_energy(12, 10, 10) == pytest.approx(want, rel=1e-11)      # 1200^2 pairs: two chunks of 2^20
+    no.close()
+
+
 def test_fp64_probe_reports_a_sane_peak():
     r = binding.no_probe_fp64_peak(0, 100)
     assert r["n_sm"] > 0 and 1.0 < r["tflops"] < 100.0
