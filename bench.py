@@ -168,7 +168,7 @@ def run_b200(args, workload):
     import torch
     import torch.distributed as dist
 
-    from paper_2603_24532_b200 import binding, build
+    from paper_2603_24532_b200 import binding, build, replicas
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -184,7 +184,7 @@ def run_b200(args, workload):
     stream = torch.cuda.current_stream(dev)
 
     # replicas only: every rank integrates the whole workload on its own GPU
-    runs = workload.runs
+    runs = replicas.replica_runs(workload)
     handles = [binding.no_init(device=local, **r.params()) for r in runs]
     h_cfg = [torch.from_numpy(r.configurations()).pin_memory() for r in runs]
     d_cfg = [c.to(dev, non_blocking=True) for c in h_cfg]
@@ -199,8 +199,7 @@ def run_b200(args, workload):
             binding.no_eval(h, c.data_ptr(), r.n_cfg, o.data_ptr(), stream.cuda_stream)
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        replicas.barrier()
         torch.cuda.synchronize(dev)
 
     for _ in range(max(args.warmup, 3)):
@@ -222,12 +221,8 @@ def run_b200(args, workload):
     t_wall = time.perf_counter() - t_wall0
     clocks = sampler.stop()
     step_ms = [a.elapsed_time(b) for a, b in ev]
-    t_dev = sum(step_ms) * 1e-3
-    if world > 1:
-        t = torch.tensor([t_dev], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        t_dev = float(t.item())
-    value = world * evals_step * args.steps / t_dev
+    t_dev = replicas.max_over_ranks(sum(step_ms) * 1e-3, dev)
+    value = replicas.whole_job_rate(evals_step, args.steps, t_dev)
     n_launch = len(runs) * args.steps
 
     # ---- end to end through the C ABI with HOST buffers (H2D + D2H inside the timed region) ----
@@ -246,11 +241,7 @@ def run_b200(args, workload):
         for _ in range(k):
             step_host()
         barrier()
-        t_e2e = (time.perf_counter() - t0) / k
-        if world > 1:
-            t = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            t_e2e = float(t.item())
+        t_e2e = replicas.max_over_ranks((time.perf_counter() - t0) / k, dev)
         chk = float(h_out[0][0].abs().sum())          # the step's result is read on the host
         e2e = {"value": world * evals_step / t_e2e, "unit": UNIT,
                "h2d_bytes_per_step": int(sum(c.numel() * 8 for c in h_cfg)),
