@@ -60,6 +60,17 @@ typedef struct no_params {
  * *h is written only on success.  HOST pointers. */
 int no_init(no_handle **h, const no_params *p);
 
+/* no_init with a caller-supplied ANGULAR rule instead of the cos(theta) x phi Gauss-Legendre grid:
+ * the paper's own quadrature is "Gauss-Legendre radial x Lebedev angular" (16 radial points, order-15
+ * Lebedev).  The k3 nodes of a sphere are r_i u_m, weights r_i^2 w_i w_m / (2 pi)^3.
+ *   h_dirs : HOST, const, [n_dir][4] doubles = (ux, uy, uz, w): unit vectors in the fixed lab frame and
+ *            weights with sum w = 4 pi (neither is checked; both are used as given), all finite
+ *   n_dir  : 1..4096 (NO_ERR_INVALID otherwise, or if the tables do not fit in shared memory)
+ * p->n_cos and p->n_phi must still be valid orders but are otherwise unused; no_evals_per_cfg is
+ * n_r * n_dir * (number of spheres).  h_dirs == NULL (with n_dir == 0) is no_init.  The array is
+ * copied; the caller keeps ownership. */
+int no_init_angular(no_handle **h, const no_params *p, const double *h_dirs, int n_dir);
+
 /* Enqueue the normal ordering of n_cfg configurations on `cuda_stream` (a cudaStream_t; NULL is
  * the default stream).  No synchronisation inside: the call returns as soon as the work is
  * enqueued ("asynchronous GPU transaction"); one handle may be used from several

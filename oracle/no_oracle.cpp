@@ -443,10 +443,43 @@ void normal_order_level0(const Params& p, const double* cfg, long long n_cfg, do
 // and, the isospin factor being the same at every node, the node sum is taken on the 4x4 spin
 // factor of each (permutation, term) first (linearity of the sum; nothing else is regrouped).
 // ---------------------------------------------------------------------------------------
+// One k3 node: momentum and full weight r^2 w_r w_ang / (2 pi)^3.
+template <class T> struct Node { T k3[3]; T W; };
+
+// Nodes of one Fermi sphere in summation order.  Default: the Gauss-Legendre product grid in
+// (r, cos theta, phi) of Params (BASELINE.json).  With a caller-supplied angular rule
+// dirs[n_dir][4] = (ux, uy, uz, w), sum w = 4 pi (e.g. a Lebedev rule, the paper's choice:
+// "Gauss-Legendre radial x Lebedev angular"), the angular part is that list.
 template <class T>
-void normal_order_level1(const Params& p, const double* cfg, long long n_cfg, double* out) {
-  Coup<T> c = couplings<T>(p);
+std::vector<Node<T>> sphere_nodes(const Params& p, T kf, const double* dirs, int n_dir) {
   const T norm = 1 / (8 * (T)PI_LD * (T)PI_LD * (T)PI_LD);
+  Grid<T> g = make_grid<T>(p, kf);
+  std::vector<Node<T>> nodes;
+  if (dirs) {
+    for (int i = 0; i < p.n_r; ++i) for (int m = 0; m < n_dir; ++m) {
+      Node<T> nd;
+      for (int a = 0; a < 3; ++a) nd.k3[a] = g.r[i] * (T)dirs[4 * m + a];
+      nd.W = g.r[i] * g.r[i] * g.wr[i] * (T)dirs[4 * m + 3] * norm;
+      nodes.push_back(nd);
+    }
+  } else {
+    for (int i = 0; i < p.n_r; ++i) for (int j = 0; j < p.n_cos; ++j) for (int l = 0; l < p.n_phi; ++l) {
+      T st = std::sqrt(1 - g.x[j] * g.x[j]);
+      Node<T> nd;
+      nd.k3[0] = g.r[i] * st * std::cos(g.phi[l]);
+      nd.k3[1] = g.r[i] * st * std::sin(g.phi[l]);
+      nd.k3[2] = g.r[i] * g.x[j];
+      nd.W = g.r[i] * g.r[i] * g.wr[i] * g.wx[j] * g.wphi[l] * norm;
+      nodes.push_back(nd);
+    }
+  }
+  return nodes;
+}
+
+template <class T>
+void normal_order_level1(const Params& p, const double* cfg, long long n_cfg, double* out,
+                         const double* dirs = nullptr, int n_dir = 0) {
+  Coup<T> c = couplings<T>(p);
   // constant isospin matrices of the two kinds for every ordered pair (i,j)
   M8<T> iso_tab[2][3][3];
   for (int kind = 0; kind < 2; ++kind) for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j)
@@ -458,14 +491,13 @@ void normal_order_level1(const Params& p, const double* cfg, long long n_cfg, do
     for (int tau3 = 0; tau3 < 2; ++tau3) {
       T kf = (T)species_kf(p, tau3);
       if (!(kf > 0)) continue;
-      Grid<T> g = make_grid<T>(p, kf);
+      const std::vector<Node<T>> nodes = sphere_nodes<T>(p, kf, dirs, n_dir);
       // node sums of the traced spin factors: [permutation][kind][i][j][4][4]
       cx<T> S4[6][2][3][3][4][4];
       for (auto& a : S4) for (auto& b : a) for (auto& d : b) for (auto& e : d) for (auto& f : e) for (auto& v : f) v = 0;
-      for (int i = 0; i < p.n_r; ++i) for (int j = 0; j < p.n_cos; ++j) for (int l = 0; l < p.n_phi; ++l) {
-        T st = std::sqrt(1 - g.x[j] * g.x[j]);
-        T k3[3] = {g.r[i] * st * std::cos(g.phi[l]), g.r[i] * st * std::sin(g.phi[l]), g.r[i] * g.x[j]};
-        T W = g.r[i] * g.r[i] * g.wr[i] * g.wx[j] * g.wphi[l] * norm;
+      for (const Node<T>& nd : nodes) {
+        const T* k3 = nd.k3;
+        const T W = nd.W;
         T kin[3][3], kout[3][3];
         kinematics<T>(cfg + 9 * ic, k3, kin, kout);
         T WF = W * regulator<T>(c, kin, kout);
@@ -593,6 +625,11 @@ void oracle_no_level1_ld(const Params* p, const double* cfg, long long n, double
 }
 void oracle_no_level1_f64(const Params* p, const double* cfg, long long n, double* out) {
   normal_order_level1<double>(*p, cfg, n, out);
+}
+// level 1 with a caller-supplied angular rule dirs[n_dir][4] = (ux, uy, uz, w) instead of the cos x phi grid
+void oracle_no_level1_dirs_ld(const Params* p, const double* cfg, long long n, const double* dirs, int n_dir,
+                              double* out) {
+  normal_order_level1<long double>(*p, cfg, n, out, dirs, n_dir);
 }
 double oracle_hf3n_bruteforce(const Params* p) { return hf3n_bruteforce<long double>(*p); }
 

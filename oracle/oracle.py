@@ -50,6 +50,8 @@ def _load():
         for name in ("oracle_no_level0_ld", "oracle_no_level1_ld", "oracle_no_level1_f64"):
             getattr(lib, name).argtypes = [pp, dp, ctypes.c_longlong, dp]
             getattr(lib, name).restype = None
+        lib.oracle_no_level1_dirs_ld.argtypes = [pp, dp, ctypes.c_longlong, dp, ctypes.c_int, dp]
+        lib.oracle_no_level1_dirs_ld.restype = None
         lib.oracle_hf3n_bruteforce.argtypes = [pp]
         lib.oracle_hf3n_bruteforce.restype = ctypes.c_double
         lib.oracle_num_threads.restype = ctypes.c_int
@@ -94,15 +96,24 @@ def av3n(kin, kout, **params) -> np.ndarray:
     return out[..., 0] + 1j * out[..., 1]
 
 
-def normal_order(cfg, level: int = 1, precision: str = "ld", **params) -> np.ndarray:
+def normal_order(cfg, level: int = 1, precision: str = "ld", dirs=None, **params) -> np.ndarray:
     """M[n_cfg,16,16] complex for configurations cfg[n_cfg,9] = (p, p', P) in fm^-1; output fm^2.
 
     level 0 = definition (64x64 per node); level 1 = spin and isospin traced separately.
     precision "ld" = long double arithmetic (parity reference), "f64" = double (level 1 only).
+    dirs: optional caller-supplied angular rule [n_dir,4] = (ux, uy, uz, w), sum w = 4 pi, used instead
+    of the cos(theta) x phi Gauss-Legendre grid (level 1, long double): radial GL x Lebedev.
     """
     cfg = np.ascontiguousarray(cfg, dtype=np.float64).reshape(-1, 9)
     n = cfg.shape[0]
     out = np.empty((n, 16, 16, 2))
+    if dirs is not None:
+        assert level == 1 and precision == "ld"
+        dirs = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 4)
+        if n:
+            _load().oracle_no_level1_dirs_ld(ctypes.byref(_params(params)), _dptr(cfg), n, _dptr(dirs),
+                                             dirs.shape[0], _dptr(out))
+        return out[..., 0] + 1j * out[..., 1]
     name = {(0, "ld"): "oracle_no_level0_ld", (1, "ld"): "oracle_no_level1_ld",
             (1, "f64"): "oracle_no_level1_f64"}[(level, precision)]
     if n:

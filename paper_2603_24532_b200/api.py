@@ -11,14 +11,16 @@ class NormalOrdering:
 
     cfg: float64 tensor [n, 9] = (p, p', P) in fm^-1.  A CUDA tensor goes through no_eval on the
     current stream (asynchronous); a CPU tensor goes through no_eval_host (copies inside, blocks).
+    angular: optional [n_dir, 4] array (ux, uy, uz, w) replacing the cos x phi grid (no_init_angular),
+    e.g. `angular_rules.octahedral_rule(15)` for the paper's 86-point Lebedev-type rule.
     """
 
-    def __init__(self, device: int = 0, **params):
+    def __init__(self, device: int = 0, angular=None, **params):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2603_24532_b200 needs a CUDA device (no CPU fallback)")
         self.device = device
         self.params = dict(params)
-        self._h = binding.no_init(device=device, **params)
+        self._h = binding.no_init(device=device, angular=angular, **params)
 
     def close(self):
         if getattr(self, "_h", None) is not None:

@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libno3n.so")
 
 NO_OK, NO_ERR_INVALID, NO_ERR_CUDA, NO_ERR_ALLOC = 0, 1, 2, 3
 
-EXPORTS = ("no_init", "no_eval", "no_eval_host", "no_eval_diag", "no_hf_energy", "no_free", "no_strerror", "no_last_cuda_error",
+EXPORTS = ("no_init", "no_init_angular", "no_eval", "no_eval_host", "no_eval_diag", "no_hf_energy", "no_free", "no_strerror", "no_last_cuda_error",
            "no_kernel_info", "no_evals_per_cfg", "no_probe_fp64_peak")
 
 
@@ -48,6 +48,7 @@ def load() -> ctypes.CDLL:
         lib = ctypes.CDLL(LIB_PATH)
         H = ctypes.c_void_p
         lib.no_init.argtypes = [ctypes.POINTER(H), ctypes.POINTER(no_params)]
+        lib.no_init_angular.argtypes = [ctypes.POINTER(H), ctypes.POINTER(no_params), ctypes.c_void_p, ctypes.c_int]
         lib.no_eval.argtypes = [H, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]
         lib.no_eval_host.argtypes = [H, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]
         lib.no_eval_diag.argtypes = [H, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]
@@ -63,20 +64,33 @@ def load() -> ctypes.CDLL:
         lib.no_evals_per_cfg.restype = ctypes.c_longlong
         lib.no_probe_fp64_peak.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double), ip,
                                            ctypes.c_void_p]
-        for name in ("no_init", "no_eval", "no_eval_host", "no_eval_diag", "no_hf_energy", "no_free", "no_kernel_info",
+        for name in ("no_init", "no_init_angular", "no_eval", "no_eval_host", "no_eval_diag", "no_hf_energy", "no_free", "no_kernel_info",
                      "no_probe_fp64_peak"):
             getattr(lib, name).restype = ctypes.c_int
         _lib = lib
     return _lib
 
 
-def no_init(device: int = 0, **params) -> ctypes.c_void_p:
-    """no_init: keyword arguments are the fields of struct no_params; returns the opaque handle."""
+def no_init(device: int = 0, angular=None, **params) -> ctypes.c_void_p:
+    """no_init: keyword arguments are the fields of struct no_params; returns the opaque handle.
+    angular: optional host array [n_dir, 4] = (ux, uy, uz, w) -> no_init_angular (n_cos, n_phi default to 1)."""
+    if angular is None:
+        p = no_params(device=device, **params)
+        h = ctypes.c_void_p()
+        rc = load().no_init(ctypes.byref(h), ctypes.byref(p))
+        if rc != NO_OK:
+            raise NoError(rc, "no_init")
+        return h
+    import numpy as np
+    dirs = np.ascontiguousarray(angular, dtype=np.float64).reshape(-1, 4)
+    params = dict(params)
+    params.setdefault("n_cos", 1)
+    params.setdefault("n_phi", 1)
     p = no_params(device=device, **params)
     h = ctypes.c_void_p()
-    rc = load().no_init(ctypes.byref(h), ctypes.byref(p))
+    rc = load().no_init_angular(ctypes.byref(h), ctypes.byref(p), ctypes.c_void_p(dirs.ctypes.data), dirs.shape[0])
     if rc != NO_OK:
-        raise NoError(rc, "no_init")
+        raise NoError(rc, "no_init_angular")
     return h
 
 

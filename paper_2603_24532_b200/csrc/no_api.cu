@@ -106,12 +106,15 @@ int launch(const no_handle* h, const double* d_cfg, long long n_cfg, double* d_o
 
 extern "C" {
 
-int no_init(no_handle** out, const no_params* p) {
+int no_init(no_handle** out, const no_params* p) { return no_init_angular(out, p, nullptr, 0); }
+
+int no_init_angular(no_handle** out, const no_params* p, const double* h_dirs, int n_dir) {
   if (!out || !p) return NO_ERR_INVALID;
+  if (!h_dirs && n_dir != 0) return NO_ERR_INVALID;
   no_handle* h = new (std::nothrow) no_handle();
   if (!h) return NO_ERR_ALLOC;
   h->d_tab = nullptr; h->d_cfg = nullptr; h->d_out = nullptr; h->scratch_cfg = 0;
-  int rc = build_plan(p, h->plan);
+  int rc = build_plan(p, h->plan, h_dirs, n_dir);
   if (rc != NO_OK) { delete h; return rc; }
   int n_dev = 0;
   cudaError_t e = cudaGetDeviceCount(&n_dev);

@@ -55,6 +55,7 @@ static_assert(128 % NO_NPT == 0, "n_r_pad must not exceed kMaxNr");  // radial n
 struct DevParams {
   const double* tab;      // device tables, see table layout below
   int n_r, n_cos, n_phi;
+  int n_list;             // > 0: caller-supplied angular rule of n_list directions replaces the cos x phi grid
   int n_r_pad;            // n_r rounded up to a multiple of kNodesPerTrip; padding nodes have weight 0
   int n_pass;             // number of Fermi spheres to integrate (1 or 2)
   int tab_doubles;        // doubles to stage into shared memory (exp table + all passes), multiple of 2
@@ -77,7 +78,10 @@ struct DevParams {
 // table layout: tab[0..64) = 2^(j/64); then for each pass: radial nodes as [n_r_pad][2] =
 // (r, w_r r^2/(2 pi)^3), then cos(theta)[n_cos], sin(theta)[n_cos], w_cos[n_cos], cos(phi)[n_phi],
 // sin(phi)[n_phi], w_phi[n_phi] (padded to a multiple of 4 doubles: every radial block 32-byte aligned)
-NO_HD int tab_pass_doubles(int n_r_pad, int n_cos, int n_phi) { return (2 * n_r_pad + 3 * n_cos + 3 * n_phi + 3) & ~3; }
+// (list mode: the six angular arrays are replaced by dirs[n_list][4] = (ux, uy, uz, w))
+NO_HD int tab_pass_doubles(int n_r_pad, int n_cos, int n_phi, int n_list) {
+  return n_list > 0 ? 2 * n_r_pad + 4 * n_list : (2 * n_r_pad + 3 * n_cos + 3 * n_phi + 3) & ~3;
+}
 
 // second-level accumulator rows
 template <bool C4> struct Layout {

@@ -105,12 +105,19 @@ inline bool finite_all(const no_params& p) {
   return true;
 }
 
-inline int build_plan(const no_params* p, HostPlan& plan) {
+constexpr int kMaxList = 4096;   // directions of a caller-supplied angular rule
+
+// dirs != nullptr: angular rule [n_dir][4] = (ux, uy, uz, w), sum w = 4 pi, instead of the cos x phi grid
+inline int build_plan(const no_params* p, HostPlan& plan, const double* dirs = nullptr, int n_dir = 0) {
   if (!p || !finite_all(*p)) return NO_ERR_INVALID;
   if (p->kf_n < 0 || p->kf_p < 0 || !(p->fpi > 0) || !(p->mpi > 0)) return NO_ERR_INVALID;
   if (p->n_r < 1 || p->n_r > kMaxOrder || p->n_cos < 1 || p->n_cos > kMaxOrder || p->n_phi < 1 ||
       p->n_phi > kMaxOrder)
     return NO_ERR_INVALID;
+  if (dirs) {
+    if (n_dir < 1 || n_dir > kMaxList) return NO_ERR_INVALID;
+    for (int i = 0; i < 4 * n_dir; ++i) if (!std::isfinite(dirs[i])) return NO_ERR_INVALID;
+  }
   const bool regulated = p->Lambda > 0;
   if (regulated && (p->n_reg < 1 || p->n_reg > kMaxRegPoly)) return NO_ERR_INVALID;
 
@@ -118,6 +125,7 @@ inline int build_plan(const no_params* p, HostPlan& plan) {
   d = DevParams();
   d.tab = nullptr;
   d.n_r = p->n_r; d.n_cos = p->n_cos; d.n_phi = p->n_phi;
+  d.n_list = dirs ? n_dir : 0;
   const double mpi = p->mpi / kHbarc, fpi = p->fpi / kHbarc;
   const double Lchi = (p->lambda_chi > 0 ? p->lambda_chi : 700.0) / kHbarc;
   const double c1 = p->c1 * 1e-3 * kHbarc, c3 = p->c3 * 1e-3 * kHbarc, c4 = p->c4 * 1e-3 * kHbarc;
@@ -149,10 +157,10 @@ inline int build_plan(const no_params* p, HostPlan& plan) {
   d.kf_max = 0.0;
   for (const Pass& q : passes) d.kf_max = q.kf > d.kf_max ? q.kf : d.kf_max;
   plan.n_sph = d.n_pass;
-  plan.evals_per_cfg = (long long)p->n_r * p->n_cos * p->n_phi * d.n_pass;
+  plan.evals_per_cfg = (long long)p->n_r * (dirs ? (long long)n_dir : (long long)p->n_cos * p->n_phi) * d.n_pass;
 
   d.n_r_pad = (p->n_r + kNodesPerTrip - 1) / kNodesPerTrip * kNodesPerTrip;
-  const int per = tab_pass_doubles(d.n_r_pad, p->n_cos, p->n_phi);
+  const int per = tab_pass_doubles(d.n_r_pad, p->n_cos, p->n_phi, d.n_list);
   int total = kExpTab + per * d.n_pass;
   total = (total + 1) & ~1;               // 16-byte granularity of the bulk copy
   d.tab_doubles = total;
@@ -177,6 +185,10 @@ inline int build_plan(const no_params* p, HostPlan& plan) {
       d.radk[s][i][1] = T[2 * i + 1];
     }
     double* A = T + 2 * d.n_r_pad;
+    if (dirs) {
+      for (int i = 0; i < 4 * n_dir; ++i) A[i] = dirs[i];
+      continue;
+    }
     for (int j = 0; j < p->n_cos; ++j) {
       A[j] = xc[j];
       A[p->n_cos + j] = std::sqrt((1.0 - xc[j]) * (1.0 + xc[j]));

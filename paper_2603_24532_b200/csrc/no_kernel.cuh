@@ -143,16 +143,24 @@ no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg,
     __syncwarp();
 
     // ---- a2 + a3: hot loop over the k3 nodes of this sphere ----
-    const int n_dir = P.n_cos * P.n_phi;
+    const int n_dir = P.n_list > 0 ? P.n_list : P.n_cos * P.n_phi;
     const int dj = kLanes / P.n_phi, dl = kLanes - dj * P.n_phi;   // (j, l) advance by 32 directions per trip
     int j = lane / P.n_phi, l = lane - j * P.n_phi;
+    const double4* dlist = reinterpret_cast<const double4*>(ct);   // list mode: (ux, uy, uz, w), 32-byte aligned
     const double2* tt2 = reinterpret_cast<const double2*>(ttab);
 #pragma unroll 1
     for (int m = lane; m < n_dir; m += kLanes) {
-      const double sj = st[j];
       DirConst d;
-      dir_setup(*cc, sj * cph[l], sj * sph[l], ct[j], d);
-      const double w = wc[j] * wph[l];
+      double w;
+      if (P.n_list > 0) {                                   // caller-supplied angular rule (e.g. Lebedev)
+        const double4 q = dlist[m];
+        dir_setup(*cc, q.x, q.y, q.z, d);
+        w = q.w;
+      } else {
+        const double sj = st[j];
+        dir_setup(*cc, sj * cph[l], sj * sph[l], ct[j], d);
+        w = wc[j] * wph[l];
+      }
       First f;
       first_zero(f);
       if (flush) radial_loop<NREG, true>(P, pass, rsp, e2tab, d, tt2, ttab, f);

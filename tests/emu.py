@@ -35,6 +35,22 @@ def emu_eval(cfg, **params):
     return out[..., 0] + 1j * out[..., 1]
 
 
+def emu_eval_angular(cfg, dirs, **params):
+    cfg = np.ascontiguousarray(cfg, dtype=np.float64).reshape(-1, 9)
+    dirs = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 4)
+    out = np.empty((cfg.shape[0], 16, 16, 2))
+    params = dict(params)
+    params.setdefault("n_cos", 1)
+    params.setdefault("n_phi", 1)
+    p = no_params(device=0, **params)
+    rc = load().emu_eval_angular(ctypes.byref(p), dirs.ctypes.data_as(ctypes.c_void_p), ctypes.c_int(dirs.shape[0]),
+                                 cfg.ctypes.data_as(ctypes.c_void_p), ctypes.c_longlong(cfg.shape[0]),
+                                 out.ctypes.data_as(ctypes.c_void_p))
+    if rc != 0:
+        raise ValueError(rc)
+    return out[..., 0] + 1j * out[..., 1]
+
+
 def emu_plan(**params):
     p = no_params(device=0, **params)
     n_pass, nreg, c4, tabn = ctypes.c_int(), ctypes.c_int(), ctypes.c_int(), ctypes.c_int()

@@ -47,13 +47,19 @@ static void emu_cfg(const HostPlan& plan, const double* cfg, double* out /*[512]
     const double* sph = cph + P.n_phi;
     const double* wph = sph + P.n_phi;
     std::fill(acc.begin(), acc.end(), 0.0);
-    const int n_dir = P.n_cos * P.n_phi;
+    const int n_dir = P.n_list > 0 ? P.n_list : P.n_cos * P.n_phi;
     for (int lane = 0; lane < kLanes; ++lane) {
       for (int m = lane; m < n_dir; m += kLanes) {
-        const int j = m / P.n_phi, l = m - j * P.n_phi;
         DirConst d;
-        dir_setup(c, st[j] * cph[l], st[j] * sph[l], ct[j], d);
-        const double w = wc[j] * wph[l];
+        double w;
+        if (P.n_list > 0) {
+          dir_setup(c, ct[4 * m], ct[4 * m + 1], ct[4 * m + 2], d);
+          w = ct[4 * m + 3];
+        } else {
+          const int j = m / P.n_phi, l = m - j * P.n_phi;
+          dir_setup(c, st[j] * cph[l], st[j] * sph[l], ct[j], d);
+          w = wc[j] * wph[l];
+        }
         First f;
         first_zero(f);
         for (int i = 0; i < P.n_r_pad; i += kNodesPerTrip) trip<NREG>(c.rs, P.n_reg, e2tab, d, rad, ttab.data(), i, f, NREG >= 0 && needs_flush(c));
@@ -93,6 +99,18 @@ static void emu_dispatch(const HostPlan& plan, const double* cfg, double* out) {
 }
 
 extern "C" {
+
+int emu_eval_angular(const no_params* p, const double* dirs, int n_dir, const double* cfg, long long n_cfg,
+                     double* out) {
+  HostPlan plan;
+  const int rc = build_plan(p, plan, dirs, n_dir);
+  if (rc != NO_OK) return rc;
+  for (long long i = 0; i < n_cfg; ++i) {
+    if (plan.has_c4) emu_dispatch<true>(plan, cfg + 9 * i, out + 512 * i);
+    else emu_dispatch<false>(plan, cfg + 9 * i, out + 512 * i);
+  }
+  return NO_OK;
+}
 
 int emu_eval(const no_params* p, const double* cfg, long long n_cfg, double* out) {
   HostPlan plan;

@@ -114,6 +114,63 @@ def test_underflow_guard_path_strong_regulator():
     check_parity(emu.emu_eval(cfg, **kw), want)
 
 
+# ----------------------------------------------------------------------------------------------
+# caller-supplied angular rules (Gauss-Legendre radial x Lebedev angular)
+# ----------------------------------------------------------------------------------------------
+def test_octahedral_rules_integrate_monomials_exactly():
+    from paper_2603_24532_b200 import angular_rules as A
+    for deg, n_pts in ((3, 6), (5, 14), (7, 26), (9, 38), (11, 50), (15, 86)):
+        d = A.octahedral_rule(deg)
+        assert d.shape == (n_pts, 4) and (d[:, 3] > 0).all()
+        assert np.abs(np.linalg.norm(d[:, :3], axis=1) - 1).max() < 1e-15
+        assert A.check_rule(d, deg) < 5e-14                      # every monomial up to the degree
+        assert A.check_rule(d, deg + 1) > 1e-6                   # and not beyond
+    # octahedral symmetry of the point set: invariant under x -> -x and x <-> y
+    d = A.octahedral_rule(15)
+    key = lambda a: sorted(map(tuple, np.round(a, 12)))
+    assert key(d * [-1, 1, 1, 1]) == key(d) and key(d[:, [1, 0, 2, 3]]) == key(d)
+    p = A.product_rule(4, 5)
+    assert p.shape == (20, 4) and abs(p[:, 3].sum() - 4 * np.pi) < 1e-14
+    for k in (2, 4, 6):                                        # Gauss-Legendre in cos(theta): z^k exact
+        assert abs(np.sum(p[:, 3] * p[:, 2] ** k) - 4 * np.pi / (k + 1)) < 1e-14
+
+
+def test_product_rule_as_a_list_reproduces_the_grid_path():
+    """the same nodes through the list path of the kernel arithmetic and through the cos x phi path."""
+    from paper_2603_24532_b200 import angular_rules as A
+    kw = dict(PHYS, c4=5.4, kf_n=1.3, kf_p=0.9, n_r=5)
+    cfg = np.random.default_rng(9).uniform(-1, 1, (3, 9)) * 1.5
+    grid = emu.emu_eval(cfg, n_cos=6, n_phi=7, **kw)
+    lst = emu.emu_eval_angular(cfg, A.product_rule(6, 7), **kw)
+    assert np.abs(grid - lst).max() < 1e-14 * np.abs(grid).max()
+    check_parity(lst, O.normal_order(cfg, n_cos=6, n_phi=7, **kw))
+
+
+@pytest.mark.parametrize("degree", [5, 15])
+def test_kernel_arithmetic_with_a_lebedev_type_rule_matches_oracle(degree):
+    from paper_2603_24532_b200 import angular_rules as A
+    dirs = A.octahedral_rule(degree)                             # 14 and 86 directions: ragged over 32 lanes
+    kw = dict(PHYS, c4=0.0, kf_n=1.3, kf_p=0.9, n_r=4)
+    cfg = np.random.default_rng(11).uniform(-1, 1, (2, 9)) * 1.5
+    want = O.normal_order(cfg, dirs=dirs, n_cos=1, n_phi=1, **kw)
+    check_parity(emu.emu_eval_angular(cfg, dirs, **kw), want)
+    assert emu.emu_eval_angular(cfg, dirs, **kw).shape == (2, 16, 16)
+
+
+def test_lebedev_rule_converges_to_the_product_grid_result():
+    """quadrature sanity (loose): 86 Lebedev-type directions and a 24 x 24 product grid agree to ~1e-4,
+    far better than the 10 x 9 product grid with about the same number of directions."""
+    from paper_2603_24532_b200 import angular_rules as A
+    kw = dict(PHYS, c4=0.0, kf_n=1.2, kf_p=0.0, n_r=8, Lambda=500.0)
+    cfg = np.array([[0.3, -0.2, 0.5, -0.1, 0.4, 0.2, 0.2, 0.1, -0.3]])
+    fine = emu.emu_eval(cfg, n_cos=24, n_phi=24, **kw)
+    leb = emu.emu_eval_angular(cfg, A.octahedral_rule(15), **kw)
+    coarse = emu.emu_eval(cfg, n_cos=10, n_phi=9, **kw)
+    e_leb = np.abs(leb - fine).max() / np.abs(fine).max()
+    e_coarse = np.abs(coarse - fine).max() / np.abs(fine).max()
+    assert e_leb < 1e-3 and e_leb < e_coarse
+
+
 def test_empty_fermi_sea_gives_zero():
     out = emu.emu_eval(np.ones((2, 9)), kf_n=0.0, kf_p=0.0, n_r=2, n_cos=2, n_phi=2, **PHYS)
     assert np.count_nonzero(out) == 0

@@ -456,3 +456,32 @@ def test_diag_trace_is_the_spin_trace_of_the_diagonal():
             want = sum(M[:, idx(s1, s2, t1, t2), idx(s1, s2, t1, t2)].real for s1 in range(2) for s2 in range(2))
             assert np.allclose(D[:, 2 * t1 + t2], want, rtol=0, atol=1e-15)
     assert np.abs(np.trace(M, axis1=1, axis2=2).real - D.sum(axis=1)).max() < 1e-14
+
+
+def test_oracle_direction_list_equals_the_product_grid():
+    """pin of the caller-supplied angular rule path of the oracle: the cos x phi Gauss-Legendre grid passed
+    as a list (built here with numpy's leggauss, not with the oracle's rule) gives the default result."""
+    kw = dict(PHYS, c4=5.4, kf_n=1.2, kf_p=0.9, n_r=3)
+    x, wx = np.polynomial.legendre.leggauss(4)
+    t, wt = np.polynomial.legendre.leggauss(5)
+    ph, wp = math.pi * (t + 1), math.pi * wt
+    dirs = np.array([[math.sqrt(1 - x[j] ** 2) * math.cos(ph[l]), math.sqrt(1 - x[j] ** 2) * math.sin(ph[l]), x[j],
+                      wx[j] * wp[l]] for j in range(4) for l in range(5)])
+    cfg = RNG.uniform(-1, 1, (2, 9))
+    a = O.normal_order(cfg, n_cos=4, n_phi=5, **kw)
+    b = O.normal_order(cfg, dirs=dirs, n_cos=1, n_phi=1, **kw)
+    assert np.abs(a - b).max() < 1e-14 * np.abs(a).max()
+
+
+def test_oracle_direction_list_cE_closed_form():
+    """P1 with an angular rule of 6 directions: the constant integrand only needs sum w = 4 pi."""
+    kF = 1.33
+    dirs = np.array([[1, 0, 0], [-1, 0, 0], [0, 1, 0], [0, -1, 0], [0, 0, 1], [0, 0, -1]], dtype=float)
+    dirs = np.column_stack([dirs, np.full(6, 4 * math.pi / 6)])
+    kw = dict(kf_n=kF, kf_p=kF, cE=-0.5, gA=1.27, fpi=92.4, mpi=138.04, lambda_chi=700.0, Lambda=-1.0, n_r=2,
+              n_cos=1, n_phi=1)
+    M = O.normal_order(np.zeros((1, 9)), dirs=dirs, **kw)[0]
+    hbarc = 197.3269804
+    pref = -(-0.5) * kF ** 3 / (math.pi ** 2 * (92.4 / hbarc) ** 4 * (700.0 / hbarc))
+    assert M[1, 1].real == pytest.approx(pref, rel=1e-13) and M[1, 2].real == pytest.approx(-pref, rel=1e-13)
+    assert abs(M[0, 0]) < 1e-15

@@ -317,6 +317,44 @@ def test_hf_energy_matches_oracle_contraction_and_closed_form():
     no.close()
 
 
+# ----------------------------------------------------------------------------------------------
+# caller-supplied angular rule: Gauss-Legendre radial x Lebedev-type angular
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("degree,geo", [(15, dict(kf_n=1.33, kf_p=1.33)), (15, dict(kf_n=1.4, kf_p=0.8, c4=5.4)),
+                                        (5, dict(kf_n=1.0, kf_p=0.0)), (17, dict(kf_n=1.4, kf_p=0.8))])
+def test_lebedev_type_rule_matches_oracle(degree, geo):
+    """the paper's production quadrature: 16 radial Gauss-Legendre points x the 86-point degree-15 rule
+    (and 14 / 110 directions: ragged over the 32 lanes)."""
+    from paper_2603_24532_b200 import angular_rules as A
+    dirs = A.octahedral_rule(degree)
+    kw = dict(PHYS, n_r=16)
+    kw.update(geo)
+    cfg = W.momentum_configurations(21, 3, 11, 1.5, 2.0)
+    no = NormalOrdering(device=0, angular=dirs, **kw)
+    assert no.evals_per_cfg == 16 * len(dirs) * (1 if kw["kf_p"] in (0.0, kw["kf_n"]) else 2)
+    got = no(torch.from_numpy(cfg).cuda()).cpu().numpy()
+    torch.cuda.synchronize()
+    no.close()
+    check_parity(got, O.normal_order(cfg, dirs=dirs, n_cos=1, n_phi=1, **kw), f"degree {degree}")
+
+
+def test_product_rule_as_list_equals_grid_path_and_bad_rules_are_refused():
+    from paper_2603_24532_b200 import angular_rules as A
+    kw = dict(PHYS, kf_n=1.3, kf_p=0.9, n_r=6)
+    cfg = W.momentum_configurations(2, 1, 5, 1.5, 2.0)
+    grid = gpu_eval(cfg, n_cos=7, n_phi=9, **kw)
+    no = NormalOrdering(device=0, angular=A.product_rule(7, 9), **kw)
+    lst = no(torch.from_numpy(cfg).cuda()).cpu().numpy()
+    no.close()
+    assert np.abs(grid - lst).max() <= 1e-13 * np.abs(grid).max()
+    bad = A.product_rule(2, 2)
+    bad[1, 2] = np.nan
+    with pytest.raises(binding.NoError):
+        binding.no_init(device=0, angular=bad, **kw)
+    with pytest.raises(binding.NoError):
+        binding.no_init(device=0, angular=np.zeros((5000, 4)), **kw)          # more than 4096 directions
+
+
 def test_fp64_probe_reports_a_sane_peak():
     r = binding.no_probe_fp64_peak(0, 100)
     assert r["n_sm"] > 0 and 1.0 < r["tflops"] < 100.0
