@@ -44,7 +44,7 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "c4"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "c4", "paper"])
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg")
@@ -123,12 +123,12 @@ def time_oracle(workload, n_sample: int):
     from oracle import oracle as O
     run, cfg, n = oracle_sample(workload, n_sample)
     t0 = time.perf_counter()
-    O.normal_order(cfg, level=1, precision="ld", **run.params())
+    O.normal_order(cfg, level=1, precision="ld", dirs=run.angular(), **run.params())
     dt = time.perf_counter() - t0
     evals = n * run.nodes_per_cfg
     return {"value": evals / dt, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
             "sample": f"first {n} configurations of run '{run.name}' of {workload.name} at the full "
-                      f"{run.n_quad}^3 x {run.n_sph} grid ({evals} evaluations, {dt:.1f} s, level-1 long double)"}, dt
+                      f"{run.nodes_per_cfg}-node grid ({evals} evaluations, {dt:.1f} s, level-1 long double)"}, dt
 
 
 def run_reference(args, workload):
@@ -141,14 +141,14 @@ def run_reference(args, workload):
     run, cfg, n = oracle_sample(workload, args.cpu_sample)
     evals = n * run.nodes_per_cfg
     for _ in range(args.warmup):
-        O.normal_order(cfg[:max(1, n // 8)], **run.params())
+        O.normal_order(cfg[:max(1, n // 8)], dirs=run.angular(), **run.params())
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        O.normal_order(cfg, level=1, precision="ld", **run.params())
+        O.normal_order(cfg, level=1, precision="ld", dirs=run.angular(), **run.params())
     dt = (time.perf_counter() - t0) / args.steps
     value = evals / dt
     sample = (f"first {n} configurations of run '{run.name}' of {workload.name} at the full "
-              f"{run.n_quad}^3 x {run.n_sph} grid ({evals} evaluations per step)")
+              f"{run.nodes_per_cfg}-node grid ({evals} evaluations per step)")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -185,7 +185,7 @@ def run_b200(args, workload):
 
     # replicas only: every rank integrates the whole workload on its own GPU
     runs = replicas.replica_runs(workload)
-    handles = [binding.no_init(device=local, **r.params()) for r in runs]
+    handles = [binding.no_init(device=local, angular=r.angular(), **r.params()) for r in runs]
     h_cfg = [torch.from_numpy(r.configurations()).pin_memory() for r in runs]
     d_cfg = [c.to(dev, non_blocking=True) for c in h_cfg]
     d_out = [torch.empty((r.n_cfg, 16, 16, 2), dtype=torch.float64, device=dev) for r in runs]

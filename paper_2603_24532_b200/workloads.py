@@ -119,6 +119,7 @@ class Run:
     seed: int = 0
     stream: int = 0              # run index of the sweep
     r_p: float = 4.0             # fm^-1
+    angular_degree: int = 0      # > 0: n_quad radial points x the octahedral rule of that degree
 
     @property
     def n_sph(self) -> int:
@@ -128,7 +129,16 @@ class Run:
 
     @property
     def nodes_per_cfg(self) -> int:
+        if self.angular_degree:
+            return self.n_quad * len(self.angular()) * self.n_sph
         return self.n_quad ** 3 * self.n_sph
+
+    def angular(self):
+        """Direction list [n,4] for no_init_angular / the oracle's `dirs`, or None for the product grid."""
+        if not self.angular_degree:
+            return None
+        from . import angular_rules
+        return angular_rules.octahedral_rule(self.angular_degree)
 
     @property
     def evals(self) -> int:
@@ -204,7 +214,13 @@ def workload(name: str) -> Workload:
         # R2: the c4 part of the two-pion-exchange topology, exercised in one extra SNM case
         return Workload(name, "SNM kF=1.33 with c4=+5.4 GeV^-1 (extra parity case, R2)",
                         [Run("snm_kf1.33_c4", 1.33, 1.33, 1024, 24, c4=5.4, stream=7)])
+    if name == "paper":
+        # the paper's own production quadrature: 16 Gauss-Legendre radial points x the
+        # order-15, 86-point Lebedev-type angular rule; SNM at n = 0.16 fm^-3
+        return Workload(name, "SNM kF=1.33, 2^20 configurations, 16 radial x 86-point degree-15 angular rule "
+                              "(the paper's quadrature)",
+                        [Run("snm_kf1.33_leb15", 1.33, 1.33, 1 << 20, 16, angular_degree=15, stream=9)])
     raise KeyError(name)
 
 
-WORKLOAD_NAMES = ("cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "c4")
+WORKLOAD_NAMES = ("cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "c4", "paper")
