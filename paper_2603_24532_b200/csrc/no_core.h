@@ -679,4 +679,63 @@ NO_HD void phase3_elem(const double* coef, int row, int col, double& re, double&
   im = gi - hi;
 }
 
+// ------------------------------------------------------------------------------------------
+// Phase 3, lane-mapped (what the kernel runs for the full matrix): lane = 2 sc + h, sc = 8 s1o + 4 s2o +
+// 2 s1i + s2i a fixed spin element; the six charge-conserving isospin blocks nb = 2 it + h are visited
+// in three steps, the ten structurally zero blocks in five.  For a fixed spin element only four
+// (mu, nu) terms of G and four of G~ contribute, each with a constant unit i^k: offsets and units are
+// computed once per lane, a block costs 8 loads and 16 multiply-adds.  Same sum as phase3_elem.
+// ------------------------------------------------------------------------------------------
+struct P3Lane {
+  int spin_off;             // element offset of the spin part: 16 (8 s1o + 4 s2o) + 8 s1i + 4 s2i
+  int cof[2][4];            // coefficient offsets (16 g + 4 mu + nu) 6 of the four terms of G (0) and G~ (1)
+  double pr[2][4], pi[2][4];   // their units i^k as (re, im)
+};
+
+NO_HD void phase3_terms(int g, int ao, int bo, int ai, int bi, int* cof, double* pr, double* pi) {
+  const int da = ao ^ ai, db = bo ^ bi;
+  const int mu[2] = {da, 3 - da}, nu[2] = {db, 3 - db};
+  const int ka[2] = {0, da ? (ao ? 1 : 3) : (ao ? 2 : 0)};
+  const int kb[2] = {0, db ? (bo ? 1 : 3) : (bo ? 2 : 0)};
+  for (int x = 0; x < 2; ++x)
+    for (int y = 0; y < 2; ++y) {
+      const int k = (ka[x] + kb[y] + (((mu[x] == 0) != (nu[y] == 0)) ? 1 : 0)) & 3;
+      cof[2 * x + y] = (16 * g + 4 * mu[x] + nu[y]) * 6;
+      pr[2 * x + y] = k == 0 ? 1.0 : (k == 2 ? -1.0 : 0.0);
+      pi[2 * x + y] = k == 1 ? 1.0 : (k == 3 ? -1.0 : 0.0);
+    }
+}
+
+NO_HD void phase3_lane_setup(int lane, P3Lane& L) {
+  const int sc = lane >> 1;
+  const int s1o = (sc >> 3) & 1, s2o = (sc >> 2) & 1, s1i = (sc >> 1) & 1, s2i = sc & 1;
+  L.spin_off = 16 * (8 * s1o + 4 * s2o) + 8 * s1i + 4 * s2i;
+  phase3_terms(0, s1o, s2o, s1i, s2i, L.cof[0], L.pr[0], L.pi[0]);
+  phase3_terms(1, s2o, s1o, s1i, s2i, L.cof[1], L.pr[1], L.pi[1]);      // row of G~ read at (s2, s1, t2, t1)
+}
+
+// charge-conserving block nb = 0..5: (to, ti) = (0,0) (1,1) (2,2) (3,3) (1,2) (2,1); returns the element offset
+NO_HD int phase3_block(const double* coef, const P3Lane& L, int nb, double& re, double& im) {
+  const int to = nb < 4 ? nb : nb - 3, ti = nb < 4 ? nb : 6 - nb;
+  const int b0 = nb;                                  // iso_block(to, ti)
+  const int b1 = nb == 0 ? 0 : (nb == 3 ? 3 : 6 - nb);   // iso_block(swap(to), ti): 0 5 4 3 2 1
+  double gr = 0, gi = 0, hr = 0, hi = 0;
+  for (int x = 0; x < 4; ++x) {
+    const double cg = coef[L.cof[0][x] + b0], ch = coef[L.cof[1][x] + b1];
+    gr = fma(cg, L.pr[0][x], gr); gi = fma(cg, L.pi[0][x], gi);
+    hr = fma(ch, L.pr[1][x], hr); hi = fma(ch, L.pi[1][x], hi);
+  }
+  re = gr - hr;
+  im = gi - hi;
+  return L.spin_off + 16 * to + ti;
+}
+
+// structurally zero block nz = 0..9 (charge not conserved): element offset
+NO_HD int phase3_zero_off(const P3Lane& L, int nz) {
+  // (to, ti) in the order (0,1) (0,2) (0,3) (1,0) (1,3) (2,0) (2,3) (3,0) (3,1) (3,2)
+  const int to = nz < 3 ? 0 : (nz < 5 ? 1 : (nz < 7 ? 2 : 3));
+  const int ti = nz < 3 ? nz + 1 : (nz == 3 ? 0 : (nz == 4 ? 3 : (nz == 5 ? 0 : (nz == 6 ? 3 : nz - 7))));
+  return L.spin_off + 16 * to + ti;
+}
+
 }  // namespace no3n

@@ -137,7 +137,7 @@ no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg,
     for (int i = lane; i < P.n_r_pad; i += kLanes) radial_entry(*cc, rad[2 * i], ttab + kRadT * i);
     {
       Pair* z = reinterpret_cast<Pair*>(acc + lane * L::kStride);
-#pragma unroll 1
+#pragma unroll
       for (int k = 0; k < L::kStride / 2; ++k) z[k] = Pair{0.0, 0.0};
     }
     __syncwarp();
@@ -173,10 +173,16 @@ no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg,
 
     // ---- a3: reduce the moments over the 32 lanes (fixed order) ----
     for (int row = lane; row < L::kRows; row += kLanes) {
-      double s = 0.0;
-#pragma unroll 8
-      for (int t = 0; t < kLanes; ++t) s += acc[((lane + t) & 31) * L::kStride + row];
-      mom[row] = s;
+      // four independent chains of eight (fixed order: bit reproducible), then a fixed tree
+      double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+#pragma unroll
+      for (int t = 0; t < 8; ++t) {
+        s0 += acc[((lane + t) & 31) * L::kStride + row];
+        s1 += acc[((lane + t + 8) & 31) * L::kStride + row];
+        s2 += acc[((lane + t + 16) & 31) * L::kStride + row];
+        s3 += acc[((lane + t + 24) & 31) * L::kStride + row];
+      }
+      mom[row] = (s0 + s1) + (s2 + s3);
     }
     __syncwarp();
 
@@ -204,13 +210,17 @@ no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg,
     return;
   }
   double2* o = reinterpret_cast<double2*>(out) + ic * 256;
-#pragma unroll 1
-  for (int it = 0; it < 8; ++it) {
-    const int row = 2 * it + (lane >> 4), col = lane & 15;
+  P3Lane pl;
+  phase3_lane_setup(lane, pl);
+  const int h = lane & 1;
+#pragma unroll
+  for (int it = 0; it < 3; ++it) {
     double re, im;
-    phase3_elem(coef, row, col, re, im);
-    o[row * 16 + col] = make_double2(re, im);
+    const int off = phase3_block(coef, pl, 2 * it + h, re, im);
+    o[off] = make_double2(re, im);
   }
+#pragma unroll
+  for (int it = 0; it < 5; ++it) o[phase3_zero_off(pl, 2 * it + h)] = make_double2(0.0, 0.0);
 }
 
 // ---- Hartree-Fock contraction helpers ----

@@ -7,6 +7,7 @@
 // checked against the oracle on a machine without a GPU.
 #include <cstring>
 #include <cstdint>
+#include <cmath>
 #include <vector>
 
 #include "../paper_2603_24532_b200/csrc/no_host.h"
@@ -68,22 +69,38 @@ static void emu_cfg(const HostPlan& plan, const double* cfg, double* out /*[512]
     }
     for (int lane = 0; lane < kLanes; ++lane)
       for (int row = lane; row < L::kRows; row += kLanes) {
-        double s = 0.0;
-        for (int t = 0; t < kLanes; ++t) s += acc16[((lane + t) & 31) * L::kStride + row];
-        mom[row] = s;
+        double s4[4] = {0.0, 0.0, 0.0, 0.0};
+        for (int t = 0; t < 8; ++t)
+          for (int q = 0; q < 4; ++q) s4[q] += acc16[((lane + t + 8 * q) & 31) * L::kStride + row];
+        mom[row] = (s4[0] + s4[1]) + (s4[2] + s4[3]);
       }
     for (int lane = 0; lane < 6; ++lane) phase1_job<C4>(P, c, mom.data(), lane, rec.data());
     for (int lane = 0; lane < kLanes; ++lane)
       phase2_lane(rec.data(), lane, P.nsp[pass], P.esum[pass], NREG >= 0 ? exp(-c.E0) : 1.0, &coef[lane * 6]);
   }
-  for (int lane = 0; lane < kLanes; ++lane)
-    for (int it = 0; it < 8; ++it) {
-      const int row = 2 * it + (lane >> 4), col = lane & 15;
+  for (int e = 0; e < 512; ++e) out[e] = -777.0;      // every element must be written exactly once below
+  for (int lane = 0; lane < kLanes; ++lane) {
+    P3Lane pl;
+    phase3_lane_setup(lane, pl);
+    const int h = lane & 1;
+    for (int it = 0; it < 3; ++it) {
       double re, im;
-      phase3_elem(coef.data(), row, col, re, im);
-      out[2 * (row * 16 + col)] = re;
-      out[2 * (row * 16 + col) + 1] = im;
+      const int off = phase3_block(coef.data(), pl, 2 * it + h, re, im);
+      // the lane-mapped expansion is the same sum as the per-element definition
+      double re0, im0;
+      phase3_elem(coef.data(), off >> 4, off & 15, re0, im0);
+      if (re != re0 || im != im0 || out[2 * off] != -777.0) { re = im = NAN; }
+      out[2 * off] = re;
+      out[2 * off + 1] = im;
     }
+    for (int it = 0; it < 5; ++it) {
+      const int off = phase3_zero_off(pl, 2 * it + h);
+      double re0, im0;
+      phase3_elem(coef.data(), off >> 4, off & 15, re0, im0);
+      out[2 * off] = (re0 == 0.0 && im0 == 0.0 && out[2 * off] == -777.0) ? 0.0 : NAN;
+      out[2 * off + 1] = out[2 * off];
+    }
+  }
 }
 
 template <bool C4>
