@@ -107,6 +107,18 @@ int no_eval_diag(const no_handle *h, const double *d_cfg, long long n_cfg, doubl
  * double *e_over_v.  Allocates and frees its own device scratch. */
 int no_hf_energy(const no_handle *h, int n_r, int n_cos, int n_phi, double *e_over_v, void *cuda_stream);
 
+/* 3N part of the Hartree-Fock single-particle energy (self-energy) of Eq. (9), isospin
+ * dependent and spin averaged (unpolarised matter):
+ *   Sigma_t1(k1) = sum_j <1j| Vbar_eff^(xi=1/2) |1j>|_3N = (1/4) sum_{t2} sum_{k2 in S(t2)} W2 D[2 t1 + t2],
+ * D = no_eval_diag at (p, p', P) = ((k1-k2)/2, (k1-k2)/2, k1+k2); particle 2 on an n_r x n_cos x n_phi
+ * Gauss-Legendre grid per Fermi sphere of the handle, particle 3 on the handle's own k3 grid.  Summed over
+ * the Fermi sea of particle 1 it gives the energy: E/V = (1/3) sum_{t1} sum_{k1} 2 W1 Sigma_t1(k1).
+ *   h_k1    : HOST, const, [n_k][3] momenta in fm^-1 (any momenta, inside or outside the Fermi sea)
+ *   h_sigma : HOST, [n_k][2] doubles, (proton, neutron), fm^-1 (multiply by hbar c for MeV)
+ * Enqueues on `cuda_stream`, SYNCHRONISES it, allocates and frees its own device scratch. */
+int no_sp_energy(const no_handle *h, const double *h_k1, int n_k, int n_r, int n_cos, int n_phi,
+                 double *h_sigma, void *cuda_stream);
+
 /* Release the handle and everything it owns.  NULL is a no-op. */
 int no_free(no_handle *h);
 

@@ -175,6 +175,26 @@ def hf_energy(n_r12: int, n_cos12: int, n_phi12: int, **params) -> float:
     return e / 6.0
 
 
+def sp_energy(k1, n_r12: int, n_cos12: int, n_phi12: int, **params) -> np.ndarray:
+    """3N Hartree-Fock self-energy of Eq. (9), spin averaged: Sigma[n,2] (proton, neutron), fm^-1:
+    Sigma_t1(k1) = (1/2) sum_{s2 t2} sum_{k2 in S(t2)} W2 (1/2) sum_{s1} M(p=(k1-k2)/2, p'=p, P=k1+k2)[a,a]."""
+    k1 = np.ascontiguousarray(k1, dtype=np.float64).reshape(-1, 3)
+    kf = {0: params.get("kf_p", 0.0), 1: params.get("kf_n", 0.0)}
+    sig = np.zeros((k1.shape[0], 2))
+    for t2 in (0, 1):
+        if kf[t2] <= 0:
+            continue
+        k2, w2 = sphere_nodes(n_r12, n_cos12, n_phi12, kf[t2])
+        cfg = np.empty((len(k1), len(k2), 9))
+        cfg[:, :, 0:3] = (k1[:, None, :] - k2[None, :, :]) / 2
+        cfg[:, :, 3:6] = cfg[:, :, 0:3]
+        cfg[:, :, 6:9] = k1[:, None, :] + k2[None, :, :]
+        D = diag_trace(cfg.reshape(-1, 9), **params).reshape(len(k1), len(k2), 4)
+        for t1 in (0, 1):
+            sig[:, t1] += 0.25 * np.sum(w2[None, :] * D[:, :, 2 * t1 + t2], axis=1)
+    return sig
+
+
 def num_threads() -> int:
     return int(_load().oracle_num_threads())
 

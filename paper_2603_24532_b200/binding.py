@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libno3n.so")
 
 NO_OK, NO_ERR_INVALID, NO_ERR_CUDA, NO_ERR_ALLOC = 0, 1, 2, 3
 
-EXPORTS = ("no_init", "no_init_angular", "no_eval", "no_eval_host", "no_eval_diag", "no_hf_energy", "no_free", "no_strerror", "no_last_cuda_error",
+EXPORTS = ("no_init", "no_init_angular", "no_eval", "no_eval_host", "no_eval_diag", "no_hf_energy", "no_sp_energy", "no_free", "no_strerror", "no_last_cuda_error",
            "no_kernel_info", "no_evals_per_cfg", "no_probe_fp64_peak")
 
 
@@ -54,6 +54,8 @@ def load() -> ctypes.CDLL:
         lib.no_eval_diag.argtypes = [H, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]
         lib.no_hf_energy.argtypes = [H, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double),
                                      ctypes.c_void_p]
+        lib.no_sp_energy.argtypes = [H, ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                     ctypes.c_void_p, ctypes.c_void_p]
         lib.no_free.argtypes = [H]
         lib.no_strerror.argtypes = [ctypes.c_int]
         lib.no_strerror.restype = ctypes.c_char_p
@@ -64,7 +66,7 @@ def load() -> ctypes.CDLL:
         lib.no_evals_per_cfg.restype = ctypes.c_longlong
         lib.no_probe_fp64_peak.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double), ip,
                                            ctypes.c_void_p]
-        for name in ("no_init", "no_init_angular", "no_eval", "no_eval_host", "no_eval_diag", "no_hf_energy", "no_free", "no_kernel_info",
+        for name in ("no_init", "no_init_angular", "no_eval", "no_eval_host", "no_eval_diag", "no_hf_energy", "no_sp_energy", "no_free", "no_kernel_info",
                      "no_probe_fp64_peak"):
             getattr(lib, name).restype = ctypes.c_int
         _lib = lib
@@ -125,6 +127,18 @@ def no_hf_energy(h, n_r: int, n_cos: int, n_phi: int, stream_ptr: Optional[int] 
     if rc != NO_OK:
         raise NoError(rc, "no_hf_energy")
     return float(e.value)
+
+
+def no_sp_energy(h, k1, n_r: int, n_cos: int, n_phi: int, stream_ptr: Optional[int] = None):
+    """no_sp_energy: k1 host array [n,3] -> Sigma[n,2] (proton, neutron) in fm^-1 (synchronises the stream)."""
+    import numpy as np
+    k1 = np.ascontiguousarray(k1, dtype=np.float64).reshape(-1, 3)
+    out = np.zeros((k1.shape[0], 2))
+    rc = load().no_sp_energy(h, ctypes.c_void_p(k1.ctypes.data), k1.shape[0], n_r, n_cos, n_phi,
+                             ctypes.c_void_p(out.ctypes.data), ctypes.c_void_p(stream_ptr or 0))
+    if rc != NO_OK:
+        raise NoError(rc, "no_sp_energy")
+    return out
 
 
 def no_free(h) -> None:

@@ -221,6 +221,66 @@ int no_hf_energy(const no_handle* h, int n_r, int n_cos, int n_phi, double* e_ov
   return NO_OK;
 }
 
+int no_sp_energy(const no_handle* h, const double* h_k1, int n_k, int n_r, int n_cos, int n_phi, double* h_sigma,
+                 void* cuda_stream) {
+  if (!h || n_k < 0) return NO_ERR_INVALID;
+  if (n_k == 0) return NO_OK;
+  if (!h_k1 || !h_sigma) return NO_ERR_INVALID;
+  if (n_r < 1 || n_r > kMaxOrder || n_cos < 1 || n_cos > kMaxOrder || n_phi < 1 || n_phi > kMaxOrder) return NO_ERR_INVALID;
+  DeviceGuard guard(h->device);
+  if (!guard.ok) return cuda_fail(cudaGetLastError(), "cudaSetDevice");
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  const double kf[2] = {h->plan.kf_p, h->plan.kf_n};
+  const long long n2 = (long long)n_r * n_cos * n_phi;
+  const long long rows_chunk = (1LL << 20) / n2 > 0 ? ((1LL << 20) / n2 < n_k ? (1LL << 20) / n2 : n_k) : 1;
+  std::vector<double> k1w(4 * (size_t)n_k), nodes2;
+  for (int i = 0; i < n_k; ++i) {
+    for (int a = 0; a < 3; ++a) k1w[4 * i + a] = h_k1[3 * i + a];
+    k1w[4 * i + 3] = 1.0;                              // particle 1 is not summed: unit weight
+  }
+  double *d_k1 = nullptr, *d_nodes2 = nullptr, *d_cfg = nullptr, *d_w = nullptr, *d_diag = nullptr, *d_sigma = nullptr;
+  int rc = NO_OK;
+  cudaError_t e = cudaSuccess;
+  auto cleanup = [&]() {
+    if (d_k1) cudaFree(d_k1);
+    if (d_nodes2) cudaFree(d_nodes2);
+    if (d_cfg) cudaFree(d_cfg);
+    if (d_w) cudaFree(d_w);
+    if (d_diag) cudaFree(d_diag);
+    if (d_sigma) cudaFree(d_sigma);
+  };
+#define NO_SP_CUDA(call) do { e = (call); if (e != cudaSuccess) { rc = cuda_fail(e, #call); cleanup(); return rc; } } while (0)
+  NO_SP_CUDA(cudaMalloc((void**)&d_k1, sizeof(double) * 4 * (size_t)n_k));
+  NO_SP_CUDA(cudaMalloc((void**)&d_nodes2, sizeof(double) * 4 * (size_t)n2));
+  NO_SP_CUDA(cudaMalloc((void**)&d_cfg, sizeof(double) * 9 * (size_t)(rows_chunk * n2)));
+  NO_SP_CUDA(cudaMalloc((void**)&d_w, sizeof(double) * (size_t)(rows_chunk * n2)));
+  NO_SP_CUDA(cudaMalloc((void**)&d_diag, sizeof(double) * 4 * (size_t)(rows_chunk * n2)));
+  NO_SP_CUDA(cudaMalloc((void**)&d_sigma, sizeof(double) * 2 * (size_t)n_k));
+  NO_SP_CUDA(cudaMemcpyAsync(d_k1, k1w.data(), sizeof(double) * 4 * (size_t)n_k, cudaMemcpyHostToDevice, s));
+  NO_SP_CUDA(cudaMemsetAsync(d_sigma, 0, sizeof(double) * 2 * (size_t)n_k, s));
+  for (int t2 = 0; t2 < 2; ++t2) {
+    if (!(kf[t2] > 0)) continue;
+    sphere_nodes(n_r, n_cos, n_phi, kf[t2], nodes2);
+    NO_SP_CUDA(cudaMemcpyAsync(d_nodes2, nodes2.data(), sizeof(double) * 4 * (size_t)n2, cudaMemcpyHostToDevice, s));
+    for (long long r0 = 0; r0 < n_k; r0 += rows_chunk) {
+      const long long rows = n_k - r0 < rows_chunk ? n_k - r0 : rows_chunk, count = rows * n2;
+      hf_pairs_kernel<<<(unsigned)((count + 255) / 256), 256, 0, s>>>(d_k1, d_nodes2, n2, r0 * n2, count, d_cfg, d_w);
+      NO_SP_CUDA(cudaGetLastError());
+      rc = launch(h, d_cfg, count, d_diag, s, kModeDiag);
+      if (rc != NO_OK) { cleanup(); return rc; }
+      // (1/2) from xi = 1/2 of Eq. (10), (1/2) from averaging the spin of particle 1 out of the traced diagonal
+      sp_reduce_kernel<<<(unsigned)rows, 256, 0, s>>>(d_diag, d_w, n2, t2, 0.25, r0, d_sigma);
+      NO_SP_CUDA(cudaGetLastError());
+    }
+    NO_SP_CUDA(cudaStreamSynchronize(s));             // nodes2 (host) is rebuilt for the next species
+  }
+  NO_SP_CUDA(cudaMemcpyAsync(h_sigma, d_sigma, sizeof(double) * 2 * (size_t)n_k, cudaMemcpyDeviceToHost, s));
+  NO_SP_CUDA(cudaStreamSynchronize(s));
+#undef NO_SP_CUDA
+  cleanup();
+  return NO_OK;
+}
+
 int no_eval_host(no_handle* h, const double* h_cfg, long long n_cfg, double* h_out, void* cuda_stream) {
   if (!h || n_cfg < 0) return NO_ERR_INVALID;
   if (n_cfg == 0) return NO_OK;

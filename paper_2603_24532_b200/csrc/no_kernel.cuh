@@ -243,6 +243,32 @@ __global__ void hf_pairs_kernel(const double* __restrict__ nodes1, const double*
   w[c] = a[3] * b[3];
 }
 
+// sigma[(row0 + i1) 2 + t1] += scale sum_{i2 < n2} w[i1 n2 + i2] diag[i1 n2 + i2][2 t1 + t2], t1 = 0, 1: one CTA per
+// momentum k1 (row i1 of the chunk), fixed summation order
+__global__ void __launch_bounds__(256) sp_reduce_kernel(const double* __restrict__ diag, const double* __restrict__ w,
+                                                        long long n2, int t2, double scale, long long row0,
+                                                        double* __restrict__ sigma) {
+  __shared__ double sh[2][256];
+  const long long base = (long long)blockIdx.x * n2;
+  double s0 = 0.0, s1 = 0.0;
+  for (long long i2 = threadIdx.x; i2 < n2; i2 += 256) {
+    const double wv = w[base + i2];
+    s0 = fma(wv, diag[4 * (base + i2) + t2], s0);
+    s1 = fma(wv, diag[4 * (base + i2) + 2 + t2], s1);
+  }
+  sh[0][threadIdx.x] = s0;
+  sh[1][threadIdx.x] = s1;
+  __syncthreads();
+  for (int half = 128; half > 0; half >>= 1) {
+    if ((int)threadIdx.x < half) {
+      sh[0][threadIdx.x] += sh[0][threadIdx.x + half];
+      sh[1][threadIdx.x] += sh[1][threadIdx.x + half];
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x < 2) sigma[2 * (row0 + blockIdx.x) + threadIdx.x] += scale * sh[threadIdx.x][0];
+}
+
 // acc[0] += sum_c w[c] diag[c][blk], one CTA, fixed summation order (bit reproducible)
 __global__ void __launch_bounds__(1024) hf_reduce_kernel(const double* __restrict__ diag, const double* __restrict__ w,
                                                          long long count, int blk, double* __restrict__ acc) {

@@ -485,3 +485,28 @@ def test_oracle_direction_list_cE_closed_form():
     pref = -(-0.5) * kF ** 3 / (math.pi ** 2 * (92.4 / hbarc) ** 4 * (700.0 / hbarc))
     assert M[1, 1].real == pytest.approx(pref, rel=1e-13) and M[1, 2].real == pytest.approx(-pref, rel=1e-13)
     assert abs(M[0, 0]) < 1e-15
+
+
+# ----------------------------------------------------------------------------------------------
+# Hartree-Fock self-energy of Eq. (9), oracle function sp_energy
+# ----------------------------------------------------------------------------------------------
+def test_sp_energy_sum_rule_gives_the_hf_energy():
+    """E/V = (1/3) sum_{t1} sum_{k1 in S(t1)} 2 W1 Sigma_t1(k1) (three equivalent ways to pick particle 1 out
+    of the 1/6 of Eq. (1)): ties sp_energy to hf_energy, which pin P8 ties to the brute-force 9-D sum."""
+    kw = dict(PHYS, c4=5.4, kf_n=1.2, kf_p=0.9, n_r=2, n_cos=3, n_phi=2)
+    e = 0.0
+    for t1, kf in ((0, kw["kf_p"]), (1, kw["kf_n"])):
+        k1, w1 = O.sphere_nodes(2, 3, 2, kf)
+        e += np.sum(2 * w1 * O.sp_energy(k1, 2, 3, 2, **kw)[:, t1]) / 3
+    assert e == pytest.approx(O.hf3n_bruteforce(**kw), rel=1e-12)
+
+
+def test_sp_energy_cE_closed_form():
+    """unregulated contact term in SNM: from P1, D[t1 t2] = pref (4 - 2 delta_t1t2), so
+    Sigma = (1/4) (kF^3/6 pi^2) 6 pref = pref kF^3/(4 pi^2), independent of k1 and of the isospin."""
+    kF, hbarc = 1.33, 197.3269804
+    kw = dict(kf_n=kF, kf_p=kF, cE=-0.5, gA=1.27, fpi=92.4, mpi=138.04, lambda_chi=700.0, Lambda=-1.0,
+              n_r=2, n_cos=2, n_phi=2)
+    pref = -(-0.5) * kF ** 3 / (math.pi ** 2 * (92.4 / hbarc) ** 4 * (700.0 / hbarc))
+    sig = O.sp_energy(np.array([[0.3, -0.2, 0.5], [2.0, 1.0, -3.0]]), 3, 2, 2, **kw)
+    assert np.allclose(sig, pref * kF ** 3 / (4 * math.pi ** 2), rtol=1e-12, atol=0)

@@ -355,6 +355,34 @@ def test_product_rule_as_list_equals_grid_path_and_bad_rules_are_refused():
         binding.no_init(device=0, angular=np.zeros((5000, 4)), **kw)          # more than 4096 directions
 
 
+def test_sp_energy_matches_oracle_and_sums_to_the_hf_energy():
+    """Eq. (9): isospin-dependent 3N Hartree-Fock self-energy; chunked over k1 rows; sum rule with no_hf_energy."""
+    kw = dict(PHYS, c4=5.4, kf_n=1.3, kf_p=0.9, n_r=4, n_cos=3, n_phi=5)
+    k1 = np.array([[0.0, 0.0, 0.0], [0.3, -0.2, 0.5], [1.0, 0.4, -0.7], [0.0, 0.0, 2.5], [-1.9, 1.2, 0.3]])
+    no = NormalOrdering(device=0, **kw)
+    got = no.sp_energy(k1, 3, 4, 3)
+    assert np.array_equal(got, no.sp_energy(k1, 3, 4, 3))                     # bit reproducible
+    want = O.sp_energy(k1, 3, 4, 3, **kw)
+    assert np.abs(got - want).max() < 1e-11 * np.abs(want).max()
+    assert np.abs(want[:, 0] - want[:, 1]).max() > 1e-3 * np.abs(want).max()   # isospin dependence is there
+    # sum rule on equal grids: E/V = (1/3) sum_t1 sum_k1 2 W1 Sigma_t1(k1)
+    e = 0.0
+    for t1, kf in ((0, kw["kf_p"]), (1, kw["kf_n"])):
+        kk, ww = O.sphere_nodes(3, 4, 3, kf)
+        e += np.sum(2 * ww * no.sp_energy(kk, 3, 4, 3)[:, t1]) / 3
+    assert e == pytest.approx(no.hf_energy(3, 4, 3), rel=1e-11)
+    no.close()
+    # many momenta against a large particle-2 grid: several row chunks (2^20 pairs each)
+    kc = dict(kf_n=1.33, kf_p=1.33, c1=0.0, c3=0.0, c4=0.0, cD=0.0, cE=-0.5, gA=1.27, fpi=92.4, mpi=138.04,
+              lambda_chi=700.0, Lambda=-1.0, n_r=2, n_cos=2, n_phi=2)
+    hbarc = 197.3269804
+    pref = 0.5 * 1.33 ** 3 / (np.pi ** 2 * (92.4 / hbarc) ** 4 * (700.0 / hbarc))
+    no = NormalOrdering(device=0, **kc)
+    sig = no.sp_energy(W.momentum_configurations(4, 0, 100, 2.0, 2.0)[:, :3].copy(), 30, 30, 30)   # 100 x 27000 pairs
+    no.close()
+    assert np.allclose(sig, pref * 1.33 ** 3 / (4 * np.pi ** 2), rtol=1e-11, atol=0)
+
+
 def test_fp64_probe_reports_a_sane_peak():
     r = binding.no_probe_fp64_peak(0, 100)
     assert r["n_sm"] > 0 and 1.0 < r["tflops"] < 100.0
