@@ -95,6 +95,12 @@ no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg,
   double* mom = ttab + kRadT * P.n_r_pad;
   double* acc = mom + rows_pad<C4>();
 
+  // the configuration is requested first: its global-load latency overlaps the table staging
+  const long long ic = (long long)blockIdx.x * WARPS + warp;
+  double q[9];
+#pragma unroll
+  for (int a = 0; a < 9; ++a) q[a] = ic < n_cfg ? __ldg(cfg + ic * 9 + a) : 0.0;
+
   // ---- a0: stage the exp table and the quadrature tables (TMA bulk copy, one per CTA) ----
   if (threadIdx.x == 0) {
     mbar_init(bar, 1);
@@ -104,14 +110,10 @@ no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg,
   }
   __syncthreads();
 
-  const long long ic = (long long)blockIdx.x * WARPS + warp;
   if (ic >= n_cfg) return;
 
   // ---- a1: per-configuration constants, one copy per warp in shared memory ----
   {
-    double q[9];
-#pragma unroll
-    for (int a = 0; a < 9; ++a) q[a] = __ldg(cfg + ic * 9 + a);
     CfgConst c;
     cfg_setup<NREG>(P, q, c);
     if (lane == 0) *cc = c;
