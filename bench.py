@@ -136,6 +136,10 @@ def run_reference(args, workload):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
+    # torchrun exports OMP_NUM_THREADS=1 to every rank; rank 0 alone runs the oracle, so give it the host
+    # cores back (set before libgomp is loaded; the oracle itself is untouched)
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1 and os.environ.get("OMP_NUM_THREADS") == "1":
+        os.environ["OMP_NUM_THREADS"] = str(os.cpu_count() or 1)
     from oracle import oracle as O
     O.build()
     run, cfg, n = oracle_sample(workload, args.cpu_sample)
