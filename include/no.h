@@ -85,8 +85,10 @@ int no_eval(const no_handle *h, const double *d_cfg, long long n_cfg, double *d_
 
 /* Same operation with HOST buffers (pageable or pinned): copies h_cfg to a device scratch owned
  * by the handle, runs the kernels, copies the result back and SYNCHRONISES `cuda_stream` before
- * returning.  Not re-entrant for one handle (the scratch is shared).  Used for the end-to-end
- * measurement. */
+ * returning.  The batch is cut into chunks of a few waves: the device-to-host copy of a finished chunk
+ * runs on an internal stream under the kernel of the next one (pinned h_out is needed for the copies to
+ * be asynchronous; pageable memory is still correct).  Not re-entrant for one handle (the scratch is
+ * shared).  Used for the end-to-end measurement. */
 int no_eval_host(no_handle *h, const double *h_cfg, long long n_cfg, double *h_out, void *cuda_stream);
 
 /* Spin-traced diagonal of the normal-ordered matrix, reduced inside the kernel (the 16x16 matrix is

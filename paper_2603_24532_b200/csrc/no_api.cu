@@ -76,6 +76,9 @@ struct no_handle {
   double* d_cfg;
   double* d_out;
   long long scratch_cfg;
+  cudaStream_t copy_stream;   // device-to-host copies of finished chunks overlap the next chunk's kernel
+  cudaEvent_t ev_chunk[2], ev_copied;
+  bool host_path_ready;
 };
 
 namespace {
@@ -113,7 +116,7 @@ int no_init_angular(no_handle** out, const no_params* p, const double* h_dirs, i
   if (!h_dirs && n_dir != 0) return NO_ERR_INVALID;
   no_handle* h = new (std::nothrow) no_handle();
   if (!h) return NO_ERR_ALLOC;
-  h->d_tab = nullptr; h->d_cfg = nullptr; h->d_out = nullptr; h->scratch_cfg = 0;
+  h->d_tab = nullptr; h->d_cfg = nullptr; h->d_out = nullptr; h->scratch_cfg = 0; h->host_path_ready = false;
   int rc = build_plan(p, h->plan, h_dirs, n_dir);
   if (rc != NO_OK) { delete h; return rc; }
   int n_dev = 0;
@@ -299,10 +302,28 @@ int no_eval_host(no_handle* h, const double* h_cfg, long long n_cfg, double* h_o
     if (e != cudaSuccess) { cudaFree(h->d_cfg); h->d_cfg = nullptr; cuda_fail(e, "cudaMalloc(out scratch)"); return NO_ERR_ALLOC; }
     h->scratch_cfg = n_cfg;
   }
+  if (!h->host_path_ready) {
+    NO_CUDA(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
+    NO_CUDA(cudaEventCreateWithFlags(&h->ev_chunk[0], cudaEventDisableTiming));
+    NO_CUDA(cudaEventCreateWithFlags(&h->ev_chunk[1], cudaEventDisableTiming));
+    NO_CUDA(cudaEventCreateWithFlags(&h->ev_copied, cudaEventDisableTiming));
+    h->host_path_ready = true;
+  }
   NO_CUDA(cudaMemcpyAsync(h->d_cfg, h_cfg, sizeof(double) * 9 * (size_t)n_cfg, cudaMemcpyHostToDevice, s));
-  const int rc = launch(h, h->d_cfg, n_cfg, h->d_out, s);
-  if (rc != NO_OK) return rc;
-  NO_CUDA(cudaMemcpyAsync(h_out, h->d_out, sizeof(double) * 512 * (size_t)n_cfg, cudaMemcpyDeviceToHost, s));
+  // chunks of a few waves: the copy of chunk k (copy stream) runs under the kernel of chunk k + 1 (caller's stream)
+  const long long chunk = n_cfg <= 2048 ? n_cfg : (n_cfg / 8 < 2048 ? 2048 : (n_cfg / 8 > 65536 ? 65536 : n_cfg / 8));
+  int k = 0;
+  for (long long c0 = 0; c0 < n_cfg; c0 += chunk, ++k) {
+    const long long cnt = n_cfg - c0 < chunk ? n_cfg - c0 : chunk;
+    const int rc = launch(h, h->d_cfg + 9 * c0, cnt, h->d_out + 512 * c0, s);
+    if (rc != NO_OK) return rc;
+    NO_CUDA(cudaEventRecord(h->ev_chunk[k & 1], s));
+    NO_CUDA(cudaStreamWaitEvent(h->copy_stream, h->ev_chunk[k & 1], 0));
+    NO_CUDA(cudaMemcpyAsync(h_out + 512 * c0, h->d_out + 512 * c0, sizeof(double) * 512 * (size_t)cnt,
+                            cudaMemcpyDeviceToHost, h->copy_stream));
+  }
+  NO_CUDA(cudaEventRecord(h->ev_copied, h->copy_stream));
+  NO_CUDA(cudaStreamWaitEvent(s, h->ev_copied, 0));
   NO_CUDA(cudaStreamSynchronize(s));
   return NO_OK;
 }
@@ -313,6 +334,12 @@ int no_free(no_handle* h) {
   if (h->d_tab) cudaFree(h->d_tab);
   if (h->d_cfg) cudaFree(h->d_cfg);
   if (h->d_out) cudaFree(h->d_out);
+  if (h->host_path_ready) {
+    cudaStreamDestroy(h->copy_stream);
+    cudaEventDestroy(h->ev_chunk[0]);
+    cudaEventDestroy(h->ev_chunk[1]);
+    cudaEventDestroy(h->ev_copied);
+  }
   delete h;
   return NO_OK;
 }
