@@ -51,7 +51,8 @@ def check_parity(got, want, label=""):
 def sample_indices(n, k):
     """first k/2 and k/2 evenly strided configurations."""
     head = list(range(min(k // 2, n)))
-    stride = [int(i) for i in np.linspace(0, n - 1, k - len(head))] if n > len(head) else []
+    m = k - len(head)
+    stride = [int(i) for i in np.linspace(0, n - 1, m + 1)[1:]] if n > len(head) and m > 0 else []   # ends at n - 1
     return sorted(set(head + stride))
 
 
