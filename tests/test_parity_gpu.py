@@ -70,7 +70,7 @@ def test_cfg1_all_configurations():
     print(f"cfg1: 256 configurations, max rel err {worst:.2e}")
 
 
-FULL_SIZE = [("cfg2", 4), ("cfg3", 8), ("cfg4", 4), ("cfg5", 2)]
+FULL_SIZE = [("cfg2", 4), ("cfg3", 8), ("cfg4", 4), ("cfg5", 2), ("paper", 16)]
 
 
 @pytest.mark.parametrize("name,n_sample", FULL_SIZE)
@@ -79,7 +79,7 @@ def test_full_size_launch_sampled_outputs(name, n_sample):
     the sampled matrices one by one."""
     for run in W.workload(name).runs:
         cfg = run.configurations()
-        no = NormalOrdering(device=0, **run.params())
+        no = NormalOrdering(device=0, angular=run.angular(), **run.params())
         d_cfg = torch.from_numpy(cfg).cuda()
         out = torch.empty((run.n_cfg, 16, 16, 2), dtype=torch.float64, device="cuda")
         no.eval_into(d_cfg, out)
@@ -87,7 +87,7 @@ def test_full_size_launch_sampled_outputs(name, n_sample):
         assert no.evals_per_cfg == run.nodes_per_cfg
         idx = sample_indices(run.n_cfg, n_sample)
         got = torch.view_as_complex(out[idx]).cpu().numpy()
-        want = O.normal_order(cfg[idx], **run.params())
+        want = O.normal_order(cfg[idx], dirs=run.angular(), **run.params())
         worst = check_parity(got, want, run.name)
         # properties that hold at any size, on a 1% subsample of the whole launch (P4, P5, P6)
         sub = np.arange(0, run.n_cfg, 100)
@@ -120,6 +120,39 @@ def _p12():
                 for t2 in range(2):
                     P[8 * s2 + 4 * s1 + 2 * t2 + t1, 8 * s1 + 4 * s2 + 2 * t1 + t2] = 1.0
     return P
+
+
+def test_random_parameter_sweep():
+    """24 seeded random parameter sets (matter composition, LECs incl. c4, cutoff, regulator exponent, ragged
+    quadrature orders, product grid or Lebedev-type rule), a few configurations each, every element compared."""
+    from paper_2603_24532_b200 import angular_rules as A
+    rng = np.random.default_rng(20260324)
+    worst = 0.0
+    for case in range(24):
+        kf = rng.uniform(0.6, 2.1, 2)
+        comp = case % 4
+        kf_n, kf_p = (kf[0], 0.0) if comp == 0 else ((0.0, kf[1]) if comp == 1 else ((kf[0], kf[0]) if comp == 2 else kf))
+        kw = dict(kf_n=float(kf_n), kf_p=float(kf_p), c1=rng.uniform(-1.5, 0.5), c3=rng.uniform(-5, -1),
+                  c4=0.0 if case % 3 else rng.uniform(2, 6), cD=rng.uniform(-2, 2), cE=rng.uniform(-1, 1),
+                  gA=rng.uniform(1.2, 1.3), fpi=rng.uniform(88, 95), mpi=rng.uniform(134, 140),
+                  lambda_chi=rng.uniform(600, 1000), Lambda=-1.0 if case % 7 == 6 else rng.uniform(380, 700),
+                  n_reg=int(rng.integers(1, 7)), n_r=int(rng.integers(1, 13)))
+        kw = {k: (float(v) if isinstance(v, np.floating) else v) for k, v in kw.items()}
+        cfg = W.momentum_configurations(100 + case, 0, 3, float(rng.uniform(0.5, 3.0)), 2.0 * max(kf_n, kf_p))
+        if case % 5 == 4:
+            dirs = A.octahedral_rule([5, 9, 11, 15][case % 4])
+            no = NormalOrdering(device=0, angular=dirs, **kw)
+            want = O.normal_order(cfg, dirs=dirs, n_cos=1, n_phi=1, **kw)
+        else:
+            grid = dict(n_cos=int(rng.integers(1, 12)), n_phi=int(rng.integers(1, 12)))
+            no = NormalOrdering(device=0, **kw, **grid)
+            want = O.normal_order(cfg, **kw, **grid)
+        got = no(torch.from_numpy(cfg).cuda()).cpu().numpy()
+        no.close()
+        if np.abs(want).max() < 1e-280:
+            continue                                             # regulator underflow: nothing to compare (R18)
+        worst = max(worst, check_parity(got, want, f"random case {case}: {kw}"))
+    print(f"random sweep: worst rel err {worst:.2e}")
 
 
 def test_c4_topology_extra_case():
