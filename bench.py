@@ -31,7 +31,7 @@ UNIT = "evals/s"
 
 # FP64 flops the shipped kernel executes per k3-point evaluation (static count of the hot loop's SASS,
 # 2 per DFMA, 1 per DADD/DMUL; DESIGN.md section 7 shows the count and the ncu cross-check).
-FLOPS_PER_EVAL = {False: 78.0, True: 78.0}          # keyed by "c4 != 0" (the hot loop is the same)
+FLOPS_PER_EVAL = {False: 76.0, True: 76.0}          # keyed by "c4 != 0" (the hot loop is the same)
 # nominal FP64 vector peak: 148 SMs x 64 DFMA lanes x 2 flops x 1.965 GHz
 FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the cfg2 kernel, from the ncu --set full capture

@@ -25,8 +25,8 @@
 // k3-independent part of the exponent, dE a degree-n polynomial in d^2 = |k3 - P/2|^2 without a
 // constant term: identical to Eq. (13) applied to the in- and outgoing triples (R5), but the
 // node-dependent rounding error scales with dE (O(1) where the integrand is large) instead of
-// with the full exponent.  exp(-dE) is a branch-free 2^(s/64), s = -64 log2(e) dE: 64-entry table
-// of 2^(j/64), degree-5 polynomial on the remainder, exponent added as an integer.
+// with the full exponent.  exp(-dE) is a branch-free 2^(s/N), s = -N log2(e) dE, N = kExpTab = 256:
+// table of 2^(j/N), degree-4 polynomial on the remainder, exponent added as an integer.
 #pragma once
 
 #include <math.h>
@@ -44,7 +44,11 @@ namespace no3n {
 constexpr int kLanes = 32;
 constexpr int kMaxRegPoly = 12;   // largest regulator exponent of the generic path
 constexpr int kMaxNr = 128;      // largest radial order (n_r_pad <= kMaxNr)
-constexpr int kExpTab = 64;       // entries of the 2^(j/64) table at the start of the device tables
+#ifndef NO_EXPTAB
+#define NO_EXPTAB 256
+#endif
+constexpr int kExpTab = NO_EXPTAB;   // entries of the 2^(j/kExpTab) table at the start of the device tables (64 or 256)
+static_assert(kExpTab == 64 || kExpTab == 256, "exp table size");
 #ifndef NO_NPT
 #define NO_NPT 4
 #endif
@@ -75,7 +79,7 @@ struct DevParams {
                               // read in the hot loop through the constant bank (uniform operands)
 };
 
-// table layout: tab[0..64) = 2^(j/64); then for each pass: radial nodes as [n_r_pad][2] =
+// table layout: tab[0..kExpTab) = 2^(j/kExpTab); then for each pass: radial nodes as [n_r_pad][2] =
 // (r, w_r r^2/(2 pi)^3), then cos(theta)[n_cos], sin(theta)[n_cos], w_cos[n_cos], cos(phi)[n_phi],
 // sin(phi)[n_phi], w_phi[n_phi] (padded to a multiple of 4 doubles: every radial block 32-byte aligned)
 // (list mode: the six angular arrays are replaced by dirs[n_list][4] = (ux, uy, uz, w))
@@ -158,7 +162,7 @@ NO_HD void cfg_setup(const DevParams& P, const double* cfg, CfgConst& c) {
       px1[j] = px1[j - 1] * X1;
       ps3[j] = ps3[j - 1] * s3;
     }
-    const double scale = -92.33248261689366;   // -64 log2(e)
+    const double scale = -1.4426950408889634 * kExpTab;   // -kExpTab log2(e)
     double binom = 1.0;                       // C(n, k), exact in double
     for (int k = 1; k <= n; ++k) {
       binom = binom * (double)(n - k + 1) / (double)k;
@@ -174,7 +178,7 @@ NO_HD void cfg_setup(const DevParams& P, const double* cfg, CfgConst& c) {
 }
 
 // the hot loop may skip the underflow guard of exp2_table when s >= kFlushBelow at every node
-constexpr double kFlushBelow = -65000.0;
+constexpr double kFlushBelow = -1015.625 * kExpTab;   // -65000 for 64 entries: exp(-dE) < 1e-305
 NO_HD bool needs_flush(const CfgConst& c) { return !(c.smin > kFlushBelow); }
 
 // ---- bit access to doubles ----
@@ -202,7 +206,7 @@ NO_HD double hilo(int hi, int lo) {
 
 // exp(-dE(d2)) = 2^(s/64), s = d2 * h(d2) <= 0, h = rs0 + d2 (rs1 + ...).  Branch free:
 //   tm = s + 1.5 2^52 holds round(s) in its low mantissa bits, f = s - round(s) in [-1/2, 1/2],
-//   2^(s/64) = 2^(ky >> 6) * tab[ky & 63] * exp(f ln2/64)  (degree-5 Taylor, |error| < 4e-17).
+//   2^(s/N) = 2^floor(ky/N) * tab[ky mod N] * exp(f ln2/N)  (Taylor polynomial, |error| < 4e-17).
 // Below s = -65000 (exp(-dE) < 1e-305) the result is replaced by a subnormal (< 3e-308), i.e. zero
 // (FLUSH); configurations whose bound smin shows that no node gets there run without that guard.
 // The stages are separate functions so that the W nodes of one trip can be interleaved.
@@ -233,25 +237,30 @@ NO_HD int mulhi32(int a, int b) {
 template <bool FLUSH>
 NO_HD double exp2_table(double tm, double kf, const double* e2tab) {
   const int ky = lo32(tm);
-  const int n = mulhi32(ky, 1 << 26);                     // floor(ky / 64)
-  const double T = e2tab[ky - 64 * n];                    // ky mod 64 in [0, 64)
+  const int n = mulhi32(ky, (int)(4294967296LL / kExpTab));   // floor(ky / kExpTab)
+  const double T = e2tab[ky - kExpTab * n];               // ky mod kExpTab in [0, kExpTab)
   int hiT = hi32(T) + n * 1048576;                        // exponent field += n
-  if (FLUSH) hiT = (uint32_t)hi32(kf) > 0xC0EFBD00u ? 0 : hiT;   // kf < -65000 (or not finite): flush
+  if (FLUSH) hiT = !(kf >= kFlushBelow) ? 0 : hiT;        // kf below the bound (or not finite): flush
   return hilo(hiT, lo32(T));
 }
 
-// exp(f ln2/64), |f| <= 1/2
+// exp(f ln2/kExpTab), |f| <= 1/2: Taylor polynomial, degree 5 for 64 entries (|error| < 4e-17), degree 4
+// for 256 entries (|x| <= 1.36e-3, x^5/120 < 4e-17); coefficients (ln2/kExpTab)^m / m!
 NO_HD double exp2_poly(double f) {
-  const double c1 = 0.010830424696249145;                 // (ln2/64)^m / m!
-  const double c2 = 5.86490495505617e-05;
-  const double c3 = 2.1173137155464776e-07;
-  const double c4 = 5.732851688640402e-10;
-  const double c5 = 1.2417843701716925e-12;
-  double p = fma(f, c5, c4);
-  p = fma(f, p, c3);
-  p = fma(f, p, c2);
-  p = fma(f, p, c1);
-  return fma(f, p, 1.0);
+  if (kExpTab == 64) {
+    const double c1 = 0.010830424696249145, c2 = 5.864904955056169e-05, c3 = 2.1173137155464774e-07, c4 = 5.732851688640402e-10, c5 = 1.2417843701716923e-12;
+    double p = fma(f, c5, c4);
+    p = fma(f, p, c3);
+    p = fma(f, p, c2);
+    p = fma(f, p, c1);
+    return fma(f, p, 1.0);
+  } else {
+    const double c1 = 0.0027076061740622863, c2 = 3.665565596910106e-06, c3 = 3.308302680541371e-09, c4 = 2.239395190875157e-12;
+    double p = fma(f, c4, c3);
+    p = fma(f, p, c2);
+    p = fma(f, p, c1);
+    return fma(f, p, 1.0);
+  }
 }
 
 // hardware seed of 1/x (relative error <= 2^-20, measured), x normal and positive

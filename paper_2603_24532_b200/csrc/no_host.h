@@ -165,7 +165,7 @@ inline int build_plan(const no_params* p, HostPlan& plan, const double* dirs = n
   total = (total + 1) & ~1;               // 16-byte granularity of the bulk copy
   d.tab_doubles = total;
   plan.tab.assign(total, 0.0);
-  for (int j = 0; j < kExpTab; ++j) plan.tab[j] = (double)exp2l((long double)j / kExpTab);   // 2^(j/64)
+  for (int j = 0; j < kExpTab; ++j) plan.tab[j] = (double)exp2l((long double)j / kExpTab);   // 2^(j/kExpTab)
   const double pi = 3.14159265358979323846;
   const double norm = 1.0 / (8.0 * pi * pi * pi);
   std::vector<double> xr, wr, xc, wc, xp, wp;

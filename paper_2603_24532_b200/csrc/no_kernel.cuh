@@ -6,7 +6,7 @@
 // weights are read from the kernel-parameter block, i.e. as uniform-register operands), folds them into
 // lane-private shared-memory accumulators (no3n::second_level), then the warp reduces the 57
 // (81 with c4) moments, turns them into Pauli-operator coefficients and writes the 16x16 complex
-// matrix.  A CTA holds WARPS warps; the 2^(j/64) table and the quadrature tables of every Fermi
+// matrix.  A CTA holds WARPS warps; the 2^(j/256) table and the quadrature tables of every Fermi
 // sphere are staged once per CTA into shared memory with one TMA bulk copy (cp.async.bulk +
 // mbarrier); r^2 + gam_l of the configuration is tabulated per warp.
 #pragma once
@@ -50,11 +50,14 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t phase) {
 }
 
 // shared memory per CTA, in doubles:
-//   tables | mbarrier (2) | per warp: CfgConst (40) | radial table [n_r_pad][6] | mom[rows_pad] | acc[rows][32]
+//   tables | mbarrier (2) | per warp: CfgConst (40) | radial table [n_r_pad][6] aliased with mom[rows_pad] | acc[32][stride]
+// (the reduced moments are written after the last read of the radial table of a pass, and the table is rebuilt
+//  at the start of the next pass: the two share one region, sized for the larger)
 template <bool C4> __host__ __device__ constexpr int rows_pad() { return (Layout<C4>::kRows + 3) & ~3; }
 
 template <bool C4> __host__ __device__ inline int warp_doubles(int n_r_pad) {
-  return kCfgDoubles + kRadT * n_r_pad + rows_pad<C4>() + Layout<C4>::kStride * kLanes;
+  const int shared_region = kRadT * n_r_pad > rows_pad<C4>() ? kRadT * n_r_pad : rows_pad<C4>();
+  return kCfgDoubles + shared_region + Layout<C4>::kStride * kLanes;
 }
 
 template <bool C4>
@@ -92,8 +95,8 @@ no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg,
   double* wbase = smem + P.tab_doubles + 2 + warp * warp_doubles<C4>(P.n_r_pad);
   CfgConst* cc = reinterpret_cast<CfgConst*>(wbase);
   double* ttab = wbase + kCfgDoubles;
-  double* mom = ttab + kRadT * P.n_r_pad;
-  double* acc = mom + rows_pad<C4>();
+  double* mom = ttab;                                 // alias, see the layout comment
+  double* acc = ttab + (kRadT * P.n_r_pad > rows_pad<C4>() ? kRadT * P.n_r_pad : rows_pad<C4>());
 
   // the configuration is requested first: its global-load latency overlaps the table staging
   const long long ic = (long long)blockIdx.x * WARPS + warp;

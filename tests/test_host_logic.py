@@ -46,10 +46,10 @@ def test_plan_passes_variants_and_tables():
     assert (p["n_pass"], p["nreg_variant"], p["has_c4"], p["evals_per_cfg"]) == (2, 4, 0, 2 * 60)
     n_pad = 4                                           # n_r = 3 padded to a multiple of 4 with zero-weight nodes
     per = (2 * n_pad + 3 * 4 + 3 * 5 + 3) // 4 * 4      # each pass padded to 32 bytes
-    assert p["tab_doubles"] == 64 + 2 * per
+    assert p["tab_doubles"] == 256 + 2 * per
     t = p["tab"]
-    assert t[0] == 1.0 and np.abs(t[:64] - 2.0 ** (np.arange(64) / 64.0)).max() < 2.3e-16   # 2^(j/64)
-    t = t[64:]
+    assert t[0] == 1.0 and np.abs(t[:256] - 2.0 ** (np.arange(256) / 256.0)).max() < 2.3e-16   # 2^(j/256)
+    t = t[256:]
     r, wr = O.gauss_legendre(3, 0.0, 0.9)               # pass 0 = protons
     assert np.allclose(t[0:6:2], r, rtol=0, atol=3e-16)
     assert np.allclose(t[1:6:2], wr * r * r / (2 * math.pi) ** 3, rtol=1e-14)
