@@ -35,8 +35,8 @@ FLOPS_PER_EVAL = {False: 76.0, True: 76.0}          # keyed by "c4 != 0" (the ho
 # nominal FP64 vector peak: 148 SMs x 64 DFMA lanes x 2 flops x 1.965 GHz
 FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the cfg2 kernel, from the ncu --set full capture
-# summarised in profiles/r01d.md (the output is still in L2 when the capture ends; the kernel is ALU bound)
-NCU_DRAM_BYTES_PER_LAUNCH = {"cfg2": 641024}
+# summarised in profiles/r01e.md (the output is still in L2 when the capture ends; the kernel is ALU bound)
+NCU_DRAM_BYTES_PER_LAUNCH = {"cfg2": 639232}
 
 
 def parse_args():
@@ -261,7 +261,7 @@ def run_b200(args, workload):
     probe = binding.no_probe_fp64_peak(local, 200, stream.cuda_stream)
     roofline = {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
                 "frac": achieved / FP64_PEAK_NOMINAL_TFLOPS, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(workload.name),
-                "traffic_source": "profiles/r01d.md (ncu --set full, per launch)" if workload.name in NCU_DRAM_BYTES_PER_LAUNCH else None,
+                "traffic_source": "profiles/r01e.md (ncu --set full, per launch)" if workload.name in NCU_DRAM_BYTES_PER_LAUNCH else None,
                 "peak_source": "nominal 148 SM x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md section 7); "
                                "MEASURED_PEAKS.json has no FP64 entry",
                 "peak_measured_dfma_probe": probe["tflops"],

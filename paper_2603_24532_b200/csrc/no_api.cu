@@ -76,6 +76,7 @@ struct no_handle {
   double* d_cfg;
   double* d_out;
   long long scratch_cfg;
+  long long wave_cfg;         // configurations of one full wave of resident CTAs (chunk granularity of the host path)
   cudaStream_t copy_stream;   // device-to-host copies of finished chunks overlap the next chunk's kernel
   cudaEvent_t ev_chunk[2], ev_copied;
   bool host_path_ready;
@@ -136,6 +137,13 @@ int no_init_angular(no_handle** out, const no_params* p, const double* h_dirs, i
   if (h->var.smem > (size_t)smem_optin) { delete h; return NO_ERR_INVALID; }
   e = cudaFuncSetAttribute((const void*)h->var.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
   if (e != cudaSuccess) { delete h; return cuda_fail(e, "cudaFuncSetAttribute(smem)"); }
+  {
+    int occ = 0, sms = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void*)h->var.fn, kWarps * 32, h->var.smem);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device);
+    if (e != cudaSuccess || occ < 1 || sms < 1) { delete h; return cuda_fail(e, "occupancy query"); }
+    h->wave_cfg = (long long)occ * sms * kWarps;
+  }
   const size_t bytes = sizeof(double) * (size_t)(h->plan.dp.tab_doubles > 0 ? h->plan.dp.tab_doubles : 2);
   e = cudaMalloc((void**)&h->d_tab, bytes);
   if (e != cudaSuccess) { delete h; cuda_fail(e, "cudaMalloc(tables)"); return NO_ERR_ALLOC; }
@@ -310,8 +318,12 @@ int no_eval_host(no_handle* h, const double* h_cfg, long long n_cfg, double* h_o
     h->host_path_ready = true;
   }
   NO_CUDA(cudaMemcpyAsync(h->d_cfg, h_cfg, sizeof(double) * 9 * (size_t)n_cfg, cudaMemcpyHostToDevice, s));
-  // chunks of a few waves: the copy of chunk k (copy stream) runs under the kernel of chunk k + 1 (caller's stream)
-  const long long chunk = n_cfg <= 2048 ? n_cfg : (n_cfg / 8 < 2048 ? 2048 : (n_cfg / 8 > 65536 ? 65536 : n_cfg / 8));
+  // chunks of whole waves of resident CTAs (about n/8, at most ~64 Ki configurations): the copy of chunk k
+  // (copy stream) runs under the kernel of chunk k + 1 (caller's stream)
+  long long waves = n_cfg / 8 / h->wave_cfg;
+  if (waves < 1) waves = 1;
+  if (waves * h->wave_cfg > 65536) waves = 65536 / h->wave_cfg > 0 ? 65536 / h->wave_cfg : 1;
+  const long long chunk = waves * h->wave_cfg;
   int k = 0;
   for (long long c0 = 0; c0 < n_cfg; c0 += chunk, ++k) {
     const long long cnt = n_cfg - c0 < chunk ? n_cfg - c0 : chunk;
