@@ -417,6 +417,30 @@ def test_sp_energy_matches_oracle_and_sums_to_the_hf_energy():
     assert np.allclose(sig, pref * 1.33 ** 3 / (4 * np.pi ** 2), rtol=1e-11, atol=0)
 
 
+def test_no_eval_is_cuda_graph_capturable():
+    """no_eval only enqueues (no synchronisation, no allocation): a batch of launches can be captured once in a
+    CUDA graph and replayed (launch-bound inner loops of small batches)."""
+    run = W.workload("cfg1").runs[0].shrunk(64, 8)
+    h = binding.no_init(device=0, **run.params())
+    cfg = torch.from_numpy(run.configurations()).cuda()
+    ref = torch.empty((64, 16, 16, 2), dtype=torch.float64, device="cuda")
+    binding.no_eval(h, cfg.data_ptr(), 64, ref.data_ptr(), torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    outs = [torch.zeros_like(ref) for _ in range(4)]
+    g, s = torch.cuda.CUDAGraph(), torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        with torch.cuda.graph(g, stream=s):
+            for o in outs:
+                binding.no_eval(h, cfg.data_ptr(), 64, o.data_ptr(), torch.cuda.current_stream().cuda_stream)
+    for o in outs:
+        o.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert all(torch.equal(ref, o) for o in outs)
+    del g
+    binding.no_free(h)
+
+
 def test_fp64_probe_reports_a_sane_peak():
     r = binding.no_probe_fp64_peak(0, 100)
     assert r["n_sm"] > 0 and 1.0 < r["tflops"] < 100.0
