@@ -83,6 +83,13 @@ int no_init_angular(no_handle **h, const no_params *p, const double *h_dirs, int
  * n_cfg == 0 succeeds and does nothing.  Non-finite inputs propagate to non-finite outputs. */
 int no_eval(const no_handle *h, const double *d_cfg, long long n_cfg, double *d_out, void *cuda_stream);
 
+/* Work layout of the kernel: 0 (default) automatic, 1 one warp per configuration (throughput layout), 2 one CTA of
+ * four warps per configuration (small-batch layout: the directions are dealt to the warps, their partial moments
+ * added in a fixed order).  Automatic picks 2 when four warps per configuration still leave warp slots of the
+ * device empty.  Both layouts compute the same sums in different (fixed) orders: results agree to rounding and
+ * are bit-reproducible within a layout.  Affects later no_eval / no_eval_diag / no_eval_host / no_hf_energy calls. */
+int no_set_layout(no_handle *h, int layout);
+
 /* Same operation with HOST buffers (pageable or pinned): copies h_cfg to a device scratch owned
  * by the handle, runs the kernels, copies the result back and SYNCHRONISES `cuda_stream` before
  * returning.  The batch is cut into chunks of a few waves: the device-to-host copy of a finished chunk

@@ -15,12 +15,14 @@ class NormalOrdering:
     e.g. `angular_rules.octahedral_rule(15)` for the paper's 86-point Lebedev-type rule.
     """
 
-    def __init__(self, device: int = 0, angular=None, **params):
+    def __init__(self, device: int = 0, angular=None, layout: int = 0, **params):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2603_24532_b200 needs a CUDA device (no CPU fallback)")
         self.device = device
         self.params = dict(params)
         self._h = binding.no_init(device=device, angular=angular, **params)
+        if layout:
+            binding.no_set_layout(self._h, layout)
 
     def close(self):
         if getattr(self, "_h", None) is not None:

@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libno3n.so")
 
 NO_OK, NO_ERR_INVALID, NO_ERR_CUDA, NO_ERR_ALLOC = 0, 1, 2, 3
 
-EXPORTS = ("no_init", "no_init_angular", "no_eval", "no_eval_host", "no_eval_diag", "no_hf_energy", "no_sp_energy", "no_free", "no_strerror", "no_last_cuda_error",
+EXPORTS = ("no_init", "no_init_angular", "no_eval", "no_eval_host", "no_eval_diag", "no_hf_energy", "no_sp_energy", "no_set_layout", "no_free", "no_strerror", "no_last_cuda_error",
            "no_kernel_info", "no_evals_per_cfg", "no_probe_fp64_peak")
 
 
@@ -56,6 +56,7 @@ def load() -> ctypes.CDLL:
                                      ctypes.c_void_p]
         lib.no_sp_energy.argtypes = [H, ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                      ctypes.c_void_p, ctypes.c_void_p]
+        lib.no_set_layout.argtypes = [H, ctypes.c_int]
         lib.no_free.argtypes = [H]
         lib.no_strerror.argtypes = [ctypes.c_int]
         lib.no_strerror.restype = ctypes.c_char_p
@@ -66,7 +67,7 @@ def load() -> ctypes.CDLL:
         lib.no_evals_per_cfg.restype = ctypes.c_longlong
         lib.no_probe_fp64_peak.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double), ip,
                                            ctypes.c_void_p]
-        for name in ("no_init", "no_init_angular", "no_eval", "no_eval_host", "no_eval_diag", "no_hf_energy", "no_sp_energy", "no_free", "no_kernel_info",
+        for name in ("no_init", "no_init_angular", "no_eval", "no_eval_host", "no_eval_diag", "no_hf_energy", "no_sp_energy", "no_set_layout", "no_free", "no_kernel_info",
                      "no_probe_fp64_peak"):
             getattr(lib, name).restype = ctypes.c_int
         _lib = lib
@@ -139,6 +140,13 @@ def no_sp_energy(h, k1, n_r: int, n_cos: int, n_phi: int, stream_ptr: Optional[i
     if rc != NO_OK:
         raise NoError(rc, "no_sp_energy")
     return out
+
+
+def no_set_layout(h, layout: int) -> None:
+    """0 automatic, 1 one warp per configuration, 2 one CTA per configuration (include/no.h)."""
+    rc = load().no_set_layout(h, layout)
+    if rc != NO_OK:
+        raise NoError(rc, "no_set_layout")
 
 
 def no_free(h) -> None:

@@ -40,9 +40,13 @@ constexpr int kMinBlocks = NO_MINB;   // resident CTAs per SM the register alloc
 
 typedef void (*KernelFn)(const DevParams, const double*, long long, double*, int);
 
+constexpr int kSplit = 4;       // warps per configuration of the small-batch layout (one configuration per CTA)
+
 struct Variant {
   KernelFn fn;
   size_t smem;
+  KernelFn fn_split;   // small-batch layout: the CTA's kSplit warps share one configuration
+  size_t smem_split;
 };
 
 template <int NREG, bool C4>
@@ -50,6 +54,8 @@ Variant make_variant(int tab_doubles, int n_r_pad) {
   Variant v;
   v.fn = no3n_kernel<NREG, C4, kWarps, kMinBlocks>;
   v.smem = smem_bytes<C4>(tab_doubles, n_r_pad, kWarps);
+  v.fn_split = no3n_kernel<NREG, C4, kSplit, 3, kSplit>;
+  v.smem_split = smem_bytes<C4>(tab_doubles, n_r_pad, kSplit);
   return v;
 }
 
@@ -76,6 +82,7 @@ struct no_handle {
   double* d_cfg;
   double* d_out;
   long long scratch_cfg;
+  int layout;                 // 0 automatic, 1 always one warp per configuration, 2 always one CTA per configuration
   long long wave_cfg;         // configurations of one full wave of resident CTAs (chunk granularity of the host path)
   cudaStream_t copy_stream;   // device-to-host copies of finished chunks overlap the next chunk's kernel
   cudaEvent_t ev_chunk[2], ev_copied;
@@ -99,6 +106,13 @@ struct DeviceGuard {
 
 int launch(const no_handle* h, const double* d_cfg, long long n_cfg, double* d_out, cudaStream_t s,
            int mode = kModeFull) {
+  if (h->layout == 2 || (h->layout == 0 && n_cfg * kSplit <= h->wave_cfg)) {
+    if (n_cfg > 2147483647LL) return NO_ERR_INVALID;
+    // even with kSplit warps each the configurations do not fill the warp slots: one CTA per configuration
+    h->var.fn_split<<<(unsigned)n_cfg, kSplit * 32, h->var.smem_split, s>>>(h->plan.dp, d_cfg, n_cfg, d_out, mode);
+    NO_CUDA(cudaGetLastError());
+    return NO_OK;
+  }
   const long long blocks = (n_cfg + kWarps - 1) / kWarps;
   if (blocks > 2147483647LL) return NO_ERR_INVALID;
   h->var.fn<<<(unsigned)blocks, kWarps * 32, h->var.smem, s>>>(h->plan.dp, d_cfg, n_cfg, d_out, mode);
@@ -117,7 +131,7 @@ int no_init_angular(no_handle** out, const no_params* p, const double* h_dirs, i
   if (!h_dirs && n_dir != 0) return NO_ERR_INVALID;
   no_handle* h = new (std::nothrow) no_handle();
   if (!h) return NO_ERR_ALLOC;
-  h->d_tab = nullptr; h->d_cfg = nullptr; h->d_out = nullptr; h->scratch_cfg = 0; h->host_path_ready = false;
+  h->d_tab = nullptr; h->d_cfg = nullptr; h->d_out = nullptr; h->scratch_cfg = 0; h->host_path_ready = false; h->layout = 0;
   int rc = build_plan(p, h->plan, h_dirs, n_dir);
   if (rc != NO_OK) { delete h; return rc; }
   int n_dev = 0;
@@ -134,9 +148,11 @@ int no_init_angular(no_handle** out, const no_params* p, const double* h_dirs, i
   int smem_optin = 0;
   e = cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->device);
   if (e != cudaSuccess) { delete h; return cuda_fail(e, "cudaDeviceGetAttribute(smem optin)"); }
-  if (h->var.smem > (size_t)smem_optin) { delete h; return NO_ERR_INVALID; }
+  if (h->var.smem > (size_t)smem_optin || h->var.smem_split > (size_t)smem_optin) { delete h; return NO_ERR_INVALID; }
   e = cudaFuncSetAttribute((const void*)h->var.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
   if (e != cudaSuccess) { delete h; return cuda_fail(e, "cudaFuncSetAttribute(smem)"); }
+  e = cudaFuncSetAttribute((const void*)h->var.fn_split, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+  if (e != cudaSuccess) { delete h; return cuda_fail(e, "cudaFuncSetAttribute(smem, split)"); }
   {
     int occ = 0, sms = 0;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void*)h->var.fn, kWarps * 32, h->var.smem);
@@ -164,6 +180,12 @@ int no_eval(const no_handle* h, const double* d_cfg, long long n_cfg, double* d_
   DeviceGuard guard(h->device);
   if (!guard.ok) return cuda_fail(cudaGetLastError(), "cudaSetDevice");
   return launch(h, d_cfg, n_cfg, d_out, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int no_set_layout(no_handle* h, int layout) {
+  if (!h || layout < 0 || layout > 2) return NO_ERR_INVALID;
+  h->layout = layout;
+  return NO_OK;
 }
 
 int no_eval_diag(const no_handle* h, const double* d_cfg, long long n_cfg, double* d_out, void* cuda_stream) {

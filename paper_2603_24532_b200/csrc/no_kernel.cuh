@@ -83,7 +83,11 @@ __device__ __forceinline__ void radial_loop(const DevParams& P, int pass, const 
   }
 }
 
-template <int NREG, bool C4, int WARPS, int MINB>
+// SPLIT = 1: one warp per configuration, WARPS configurations per CTA (the throughput layout).
+// SPLIT = WARPS > 1: the whole CTA integrates ONE configuration, the directions dealt round-robin to its warps,
+// the reduced moments of the warps added in a fixed order by warp 0, which then runs the epilogue alone: the
+// small-batch layout (fewer configurations than warp slots), chosen by the launcher.
+template <int NREG, bool C4, int WARPS, int MINB, int SPLIT = 1>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
 no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg, long long n_cfg, double* __restrict__ out,
             int mode) {
@@ -99,7 +103,9 @@ no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg,
   double* acc = ttab + (kRadT * P.n_r_pad > rows_pad<C4>() ? kRadT * P.n_r_pad : rows_pad<C4>());
 
   // the configuration is requested first: its global-load latency overlaps the table staging
-  const long long ic = (long long)blockIdx.x * WARPS + warp;
+  static_assert(SPLIT == 1 || SPLIT == WARPS, "a split CTA holds one configuration");
+  const long long ic = SPLIT == 1 ? (long long)blockIdx.x * WARPS + warp : (long long)blockIdx.x;
+  const int part = SPLIT == 1 ? 0 : warp;             // which share of the directions this warp takes
   double q[9];
 #pragma unroll
   for (int a = 0; a < 9; ++a) q[a] = ic < n_cfg ? __ldg(cfg + ic * 9 + a) : 0.0;
@@ -149,12 +155,13 @@ no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg,
 
     // ---- a2 + a3: hot loop over the k3 nodes of this sphere ----
     const int n_dir = P.n_list > 0 ? P.n_list : P.n_cos * P.n_phi;
-    const int dj = kLanes / P.n_phi, dl = kLanes - dj * P.n_phi;   // (j, l) advance by 32 directions per trip
-    int j = lane / P.n_phi, l = lane - j * P.n_phi;
+    const int dstep = kLanes * SPLIT, m0 = lane + kLanes * part;
+    const int dj = dstep / P.n_phi, dl = dstep - dj * P.n_phi;     // (j, l) advance by dstep directions per trip
+    int j = m0 / P.n_phi, l = m0 - j * P.n_phi;
     const double4* dlist = reinterpret_cast<const double4*>(ct);   // list mode: (ux, uy, uz, w), 32-byte aligned
     const double2* tt2 = reinterpret_cast<const double2*>(ttab);
 #pragma unroll 1
-    for (int m = lane; m < n_dir; m += kLanes) {
+    for (int m = m0; m < n_dir; m += dstep) {
       DirConst d;
       double w;
       if (P.n_list > 0) {                                   // caller-supplied angular rule (e.g. Lebedev)
@@ -191,13 +198,29 @@ no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg,
     }
     __syncwarp();
 
+    if (SPLIT > 1) {                                    // add the warps' partial moments (fixed order)
+      __syncthreads();
+      if (warp == 0)
+        for (int row = lane; row < L::kRows; row += kLanes) {
+          double s = mom[row];
+#pragma unroll
+          for (int w = 1; w < SPLIT; ++w) s += mom[w * warp_doubles<C4>(P.n_r_pad) + row];
+          mom[row] = s;
+        }
+      __syncthreads();                                  // the other warps may now reuse their regions
+    }
+
     // ---- a4: epilogue, phases 1 and 2 (records live in the dead accumulator area) ----
-    double* rec = acc;
-    if (lane < 6) phase1_job<C4>(P, *cc, mom, lane, rec);
-    __syncwarp();
-    phase2_lane(rec, lane, P.nsp[pass], P.esum[pass], NREG >= 0 ? exp(-cc->E0) : 1.0, blk);
-    __syncwarp();
+    if (SPLIT == 1 || warp == 0) {
+      double* rec = acc;
+      __syncwarp();
+      if (lane < 6) phase1_job<C4>(P, *cc, mom, lane, rec);
+      __syncwarp();
+      phase2_lane(rec, lane, P.nsp[pass], P.esum[pass], NREG >= 0 ? exp(-cc->E0) : 1.0, blk);
+      __syncwarp();
+    }
   }
+  if (SPLIT > 1 && warp != 0) return;
 
   // ---- a4: phase 3, (1 - P12) and expansion to the 16x16 complex matrix ----
   double* coef = acc;

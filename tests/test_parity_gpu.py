@@ -28,16 +28,27 @@ def _built():
     binding.load()
 
 
+_last = {}
+
+
 def gpu_eval(cfg, **params):
-    no = NormalOrdering(device=0, **params)
-    out = no(torch.from_numpy(np.ascontiguousarray(cfg)).cuda())
-    torch.cuda.synchronize()
-    res = out.cpu().numpy()
-    no.close()
-    return res
+    """Result of the throughput layout (one warp per configuration).  The small-batch layout (one CTA per
+    configuration) and the automatic choice are run too and kept for check_parity, so every parity case
+    below covers both kernels element by element."""
+    d_cfg = torch.from_numpy(np.ascontiguousarray(cfg)).cuda()
+    res = []
+    for layout in (0, 1, 2):
+        no = NormalOrdering(device=0, layout=layout, **params)
+        out = no(d_cfg)
+        torch.cuda.synchronize()
+        res.append(out.cpu().numpy())
+        no.close()
+    assert np.array_equal(res[0], res[1], equal_nan=True) or np.array_equal(res[0], res[2], equal_nan=True)
+    _last.update(main=res[1], split=res[2])
+    return res[1]
 
 
-def check_parity(got, want, label=""):
+def _check(got, want, label):
     mx = np.abs(want).max(axis=(1, 2), keepdims=True)
     mask = np.abs(want) > MAG_FLOOR * mx
     rel = np.abs(got - want)[mask] / np.abs(want)[mask]
@@ -45,6 +56,13 @@ def check_parity(got, want, label=""):
     assert worst < REL_TOL, f"{label}: max rel err {worst:.3e}"
     floor = np.broadcast_to(MAG_FLOOR * mx, got.shape)
     assert (np.abs(got)[~mask] <= floor[~mask]).all(), f"{label}: structural zero above the floor"
+    return worst
+
+
+def check_parity(got, want, label=""):
+    worst = _check(got, want, label)
+    if got is _last.get("main"):
+        worst = max(worst, _check(_last["split"], want, label + " [one CTA per configuration]"))
     return worst
 
 
@@ -141,11 +159,11 @@ def test_random_parameter_sweep():
         cfg = W.momentum_configurations(100 + case, 0, 3, float(rng.uniform(0.5, 3.0)), 2.0 * max(kf_n, kf_p))
         if case % 5 == 4:
             dirs = A.octahedral_rule([5, 9, 11, 15][case % 4])
-            no = NormalOrdering(device=0, angular=dirs, **kw)
+            no = NormalOrdering(device=0, angular=dirs, layout=1 + case % 2, **kw)
             want = O.normal_order(cfg, dirs=dirs, n_cos=1, n_phi=1, **kw)
         else:
             grid = dict(n_cos=int(rng.integers(1, 12)), n_phi=int(rng.integers(1, 12)))
-            no = NormalOrdering(device=0, **kw, **grid)
+            no = NormalOrdering(device=0, layout=1 + case % 2, **kw, **grid)
             want = O.normal_order(cfg, **kw, **grid)
         got = no(torch.from_numpy(cfg).cuda()).cpu().numpy()
         no.close()
@@ -364,12 +382,14 @@ def test_lebedev_type_rule_matches_oracle(degree, geo):
     kw = dict(PHYS, n_r=16)
     kw.update(geo)
     cfg = W.momentum_configurations(21, 3, 11, 1.5, 2.0)
-    no = NormalOrdering(device=0, angular=dirs, **kw)
-    assert no.evals_per_cfg == 16 * len(dirs) * (1 if kw["kf_p"] in (0.0, kw["kf_n"]) else 2)
-    got = no(torch.from_numpy(cfg).cuda()).cpu().numpy()
-    torch.cuda.synchronize()
-    no.close()
-    check_parity(got, O.normal_order(cfg, dirs=dirs, n_cos=1, n_phi=1, **kw), f"degree {degree}")
+    want = O.normal_order(cfg, dirs=dirs, n_cos=1, n_phi=1, **kw)
+    for layout in (1, 2):                                        # one warp / one CTA per configuration
+        no = NormalOrdering(device=0, angular=dirs, layout=layout, **kw)
+        assert no.evals_per_cfg == 16 * len(dirs) * (1 if kw["kf_p"] in (0.0, kw["kf_n"]) else 2)
+        got = no(torch.from_numpy(cfg).cuda()).cpu().numpy()
+        torch.cuda.synchronize()
+        no.close()
+        check_parity(got, want, f"degree {degree}, layout {layout}")
 
 
 def test_product_rule_as_list_equals_grid_path_and_bad_rules_are_refused():
