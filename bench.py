@@ -44,7 +44,7 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "c4", "paper"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "c4", "paper", "hf"])
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg")
@@ -294,8 +294,126 @@ def run_b200(args, workload):
     print(json.dumps(line), flush=True)
 
 
+# --------------------------------------------------------------------------------------------
+# the Hartree-Fock contraction (no_hf_energy) as a workload of its own
+# --------------------------------------------------------------------------------------------
+HF_PARAMS = dict(kf_n=1.33, kf_p=1.33, c1=-0.81, c3=-3.2, c4=0.0, cD=1.0, cE=-0.5, gA=1.27, fpi=92.4, mpi=138.04,
+                 lambda_chi=700.0, Lambda=500.0, n_reg=4, n_r=16, n_cos=16, n_phi=16)
+HF_PAIR_GRID = (12, 12, 12)          # particles 1 and 2: 1728 nodes per Fermi sphere, 4 species pairs in SNM
+
+
+def run_hf(args):
+    """One step = one no_hf_energy call: 4 x 1728^2 pair configurations generated on the device, each reduced
+    to its spin-traced diagonal over a 16^3 k3 grid inside the kernel, fixed-order reduction to E/V."""
+    import torch
+
+    from paper_2603_24532_b200 import binding, build, replicas
+
+    if args.impl == "reference":
+        if int(os.environ.get("RANK", "0")) != 0:
+            return
+        from oracle import oracle as O
+        O.build()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            e = O.hf_energy(2, 2, 2, **HF_PARAMS)
+        dt = (time.perf_counter() - t0) / args.steps
+        evals = 4 * 64 * 4096
+        sample = "pair grid 2x2x2 per sphere (256 pair configurations x 16^3 k3 nodes per step), level-1 long double"
+        print(json.dumps({"impl": "reference", "metric": METRIC, "value": evals / dt, "unit": UNIT, "n_gpus": args.gpus,
+                          "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+                          "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                          "config": {"workload": "hf", "sample": sample, "e_over_v_fm4": e},
+                          "cpu_baseline": {"value": evals / dt, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
+                                           "sample": sample},
+                          "e2e": {"value": evals / dt, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                          "gpu_launches": 0}), flush=True)
+        return
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        torch.distributed.init_process_group("nccl", device_id=torch.device("cuda", local))
+    build.build()
+    binding.load()
+    dev = torch.device("cuda", local)
+    stream = torch.cuda.current_stream(dev)
+    h = binding.no_init(device=local, **HF_PARAMS)
+    n1 = HF_PAIR_GRID[0] * HF_PAIR_GRID[1] * HF_PAIR_GRID[2]
+    n_pairs = 4 * n1 * n1
+    evals_step = n_pairs * binding.no_evals_per_cfg(h)
+    chunks = 4 * ((n1 * n1 + (1 << 20) - 1) >> 20)
+    flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)
+    for _ in range(max(args.warmup, 3)):
+        e_v = binding.no_hf_energy(h, *HF_PAIR_GRID, stream.cuda_stream)
+    replicas.barrier()
+    torch.cuda.synchronize(dev)
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.25)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    wall = []
+    for a, b in ev:
+        flush.zero_()
+        torch.cuda.synchronize(dev)
+        t0 = time.perf_counter()
+        a.record(stream)
+        e_v = binding.no_hf_energy(h, *HF_PAIR_GRID, stream.cuda_stream)      # synchronises the stream itself
+        b.record(stream)
+        torch.cuda.synchronize(dev)
+        wall.append(time.perf_counter() - t0)
+    replicas.barrier()
+    clocks = sampler.stop()
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    t_dev = replicas.max_over_ranks(sum(step_ms) * 1e-3, dev)
+    t_wall = replicas.max_over_ranks(sum(wall), dev)
+    value = replicas.whole_job_rate(evals_step, args.steps, t_dev)
+    flops = FLOPS_PER_EVAL[False]
+    achieved = flops * evals_step * args.steps / (sum(step_ms) * 1e-3) / 1e12
+    probe = binding.no_probe_fp64_peak(local, 200, stream.cuda_stream)
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        from oracle import oracle as O
+        t0 = time.perf_counter()
+        O.hf_energy(2, 2, 2, **HF_PARAMS)
+        dt = time.perf_counter() - t0
+        cpu = {"value": 4 * 64 * 4096 / dt, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
+               "sample": f"pair grid 2x2x2 per sphere (256 pair configurations x 16^3 k3 nodes, {dt:.1f} s), level-1 long double"}
+    binding.no_free(h)
+    if world > 1:
+        torch.distributed.destroy_process_group()
+    if rank != 0:
+        return
+    print(json.dumps({
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": t_dev / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "hf", "description": "3N Hartree-Fock energy of SNM kF=1.33 by repeated normal ordering "
+                   "(no_hf_energy): 12^3 nodes per sphere for particles 1, 2 (4 x 1728^2 pair configurations, generated "
+                   "on the device), 16^3 k3 grid", "n_cfg": n_pairs, "evals_per_step": evals_step,
+                   "cfg_per_s": world * n_pairs * args.steps / t_dev, "e_over_v_fm4": e_v,
+                   "l2": "256 MiB buffer rewritten between timed steps (L2 flush); the kernel is ALU bound",
+                   "parallelism": "replicas only: every rank integrates the whole workload"},
+        "clocks": clocks,
+        "e2e": {"value": world * evals_step * args.steps / t_wall, "unit": UNIT,
+                "h2d_bytes_per_step": 4 * n1 * 32, "d2h_bytes_per_step": 4 * 8, "ms_per_step": t_wall / args.steps * 1e3,
+                "note": "the call itself is the public API: node lists up, one scalar down, wall clock around it"},
+        "gpu_launches": 3 * chunks * args.steps,
+        "roofline": {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
+                     "frac": achieved / FP64_PEAK_NOMINAL_TFLOPS, "traffic": None,
+                     "peak_measured_dfma_probe": probe["tflops"], "flops_per_eval": flops,
+                     "kernel": "no3n::no3n_kernel (diagonal mode) + hf_pairs_kernel + hf_reduce_kernel"},
+        "cpu_baseline": cpu}), flush=True)
+
+
 def main():
     args = parse_args()
+    if args.workload == "hf":
+        run_hf(args)
+        return
     from paper_2603_24532_b200 import workloads
     wl = workloads.workload(args.workload)
     if args.impl == "reference":

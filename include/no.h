@@ -113,8 +113,8 @@ int no_eval_diag(const no_handle *h, const double *d_cfg, long long n_cfg, doubl
  * handle's own k3 grid; configuration (p, p', P) = ((k1-k2)/2, (k1-k2)/2, k1+k2).  On the same grids this
  * equals the brute-force 9-dimensional sum exactly (pin P8).  Generates the pair configurations on the
  * device in chunks, enqueues on `cuda_stream`, SYNCHRONISES it, and writes the result to the HOST
- * double *e_over_v.  Allocates and frees its own device scratch. */
-int no_hf_energy(const no_handle *h, int n_r, int n_cos, int n_phi, double *e_over_v, void *cuda_stream);
+ * double *e_over_v.  Uses a grow-only device scratch owned by the handle (not re-entrant for one handle). */
+int no_hf_energy(no_handle *h, int n_r, int n_cos, int n_phi, double *e_over_v, void *cuda_stream);
 
 /* 3N part of the Hartree-Fock single-particle energy (self-energy) of Eq. (9), isospin
  * dependent and spin averaged (unpolarised matter):
@@ -124,8 +124,8 @@ int no_hf_energy(const no_handle *h, int n_r, int n_cos, int n_phi, double *e_ov
  * the Fermi sea of particle 1 it gives the energy: E/V = (1/3) sum_{t1} sum_{k1} 2 W1 Sigma_t1(k1).
  *   h_k1    : HOST, const, [n_k][3] momenta in fm^-1 (any momenta, inside or outside the Fermi sea)
  *   h_sigma : HOST, [n_k][2] doubles, (proton, neutron), fm^-1 (multiply by hbar c for MeV)
- * Enqueues on `cuda_stream`, SYNCHRONISES it, allocates and frees its own device scratch. */
-int no_sp_energy(const no_handle *h, const double *h_k1, int n_k, int n_r, int n_cos, int n_phi,
+ * Enqueues on `cuda_stream`, SYNCHRONISES it; same handle-owned scratch as no_hf_energy (not re-entrant). */
+int no_sp_energy(no_handle *h, const double *h_k1, int n_k, int n_r, int n_cos, int n_phi,
                  double *h_sigma, void *cuda_stream);
 
 /* Release the handle and everything it owns.  NULL is a no-op. */

@@ -82,6 +82,8 @@ struct no_handle {
   double* d_cfg;
   double* d_out;
   long long scratch_cfg;
+  double* hf_arena;           // grow-only device scratch of no_hf_energy / no_sp_energy
+  long long hf_arena_doubles;
   int layout;                 // 0 automatic, 1 always one warp per configuration, 2 always one CTA per configuration
   long long wave_cfg;         // configurations of one full wave of resident CTAs (chunk granularity of the host path)
   cudaStream_t copy_stream;   // device-to-host copies of finished chunks overlap the next chunk's kernel
@@ -120,6 +122,21 @@ int launch(const no_handle* h, const double* d_cfg, long long n_cfg, double* d_o
   return NO_OK;
 }
 
+// grow-only scratch of the Hartree-Fock entry points (allocation inside a timed call costs far more than the
+// kernels when another process queries the driver, e.g. nvidia-smi)
+int hf_scratch(no_handle* h, long long doubles, double** out) {
+  if (doubles > h->hf_arena_doubles) {
+    if (h->hf_arena) cudaFree(h->hf_arena);
+    h->hf_arena = nullptr;
+    h->hf_arena_doubles = 0;
+    const cudaError_t e = cudaMalloc((void**)&h->hf_arena, sizeof(double) * (size_t)doubles);
+    if (e != cudaSuccess) { cuda_fail(e, "cudaMalloc(HF scratch)"); return NO_ERR_ALLOC; }
+    h->hf_arena_doubles = doubles;
+  }
+  *out = h->hf_arena;
+  return NO_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -131,7 +148,7 @@ int no_init_angular(no_handle** out, const no_params* p, const double* h_dirs, i
   if (!h_dirs && n_dir != 0) return NO_ERR_INVALID;
   no_handle* h = new (std::nothrow) no_handle();
   if (!h) return NO_ERR_ALLOC;
-  h->d_tab = nullptr; h->d_cfg = nullptr; h->d_out = nullptr; h->scratch_cfg = 0; h->host_path_ready = false; h->layout = 0;
+  h->d_tab = nullptr; h->d_cfg = nullptr; h->d_out = nullptr; h->scratch_cfg = 0; h->host_path_ready = false; h->layout = 0; h->hf_arena = nullptr; h->hf_arena_doubles = 0;
   int rc = build_plan(p, h->plan, h_dirs, n_dir);
   if (rc != NO_OK) { delete h; return rc; }
   int n_dev = 0;
@@ -198,7 +215,7 @@ int no_eval_diag(const no_handle* h, const double* d_cfg, long long n_cfg, doubl
   return launch(h, d_cfg, n_cfg, d_out, static_cast<cudaStream_t>(cuda_stream), kModeDiag);
 }
 
-int no_hf_energy(const no_handle* h, int n_r, int n_cos, int n_phi, double* e_over_v, void* cuda_stream) {
+int no_hf_energy(no_handle* h, int n_r, int n_cos, int n_phi, double* e_over_v, void* cuda_stream) {
   if (!h || !e_over_v) return NO_ERR_INVALID;
   if (n_r < 1 || n_r > kMaxOrder || n_cos < 1 || n_cos > kMaxOrder || n_phi < 1 || n_phi > kMaxOrder) return NO_ERR_INVALID;
   DeviceGuard guard(h->device);
@@ -214,23 +231,18 @@ int no_hf_energy(const no_handle* h, int n_r, int n_cos, int n_phi, double* e_ov
   double *d_nodes[2] = {nullptr, nullptr}, *d_cfg = nullptr, *d_w = nullptr, *d_diag = nullptr, *d_acc = nullptr;
   int rc = NO_OK;
   cudaError_t e = cudaSuccess;
-  auto cleanup = [&]() {
-    for (int t = 0; t < 2; ++t) if (d_nodes[t]) cudaFree(d_nodes[t]);
-    if (d_cfg) cudaFree(d_cfg);
-    if (d_w) cudaFree(d_w);
-    if (d_diag) cudaFree(d_diag);
-    if (d_acc) cudaFree(d_acc);
-  };
+  {
+    double* base = nullptr;
+    rc = hf_scratch(h, 8 * n1 + 14 * chunk + 2, &base);
+    if (rc != NO_OK) return rc;
+    d_nodes[0] = base; d_nodes[1] = base + 4 * n1; d_cfg = base + 8 * n1; d_w = d_cfg + 9 * chunk;
+    d_diag = d_w + chunk; d_acc = d_diag + 4 * chunk;
+  }
+  auto cleanup = [&]() {};
 #define NO_HF_CUDA(call) do { e = (call); if (e != cudaSuccess) { rc = cuda_fail(e, #call); cleanup(); return rc; } } while (0)
   for (int t = 0; t < 2; ++t)
-    if (kf[t] > 0) {
-      NO_HF_CUDA(cudaMalloc((void**)&d_nodes[t], sizeof(double) * 4 * (size_t)n1));
+    if (kf[t] > 0)
       NO_HF_CUDA(cudaMemcpyAsync(d_nodes[t], nodes[t].data(), sizeof(double) * 4 * (size_t)n1, cudaMemcpyHostToDevice, s));
-    }
-  NO_HF_CUDA(cudaMalloc((void**)&d_cfg, sizeof(double) * 9 * (size_t)chunk));
-  NO_HF_CUDA(cudaMalloc((void**)&d_w, sizeof(double) * (size_t)chunk));
-  NO_HF_CUDA(cudaMalloc((void**)&d_diag, sizeof(double) * 4 * (size_t)chunk));
-  NO_HF_CUDA(cudaMalloc((void**)&d_acc, sizeof(double)));
   NO_HF_CUDA(cudaMemsetAsync(d_acc, 0, sizeof(double), s));
   for (int t1 = 0; t1 < 2; ++t1)
     for (int t2 = 0; t2 < 2; ++t2) {
@@ -254,7 +266,7 @@ int no_hf_energy(const no_handle* h, int n_r, int n_cos, int n_phi, double* e_ov
   return NO_OK;
 }
 
-int no_sp_energy(const no_handle* h, const double* h_k1, int n_k, int n_r, int n_cos, int n_phi, double* h_sigma,
+int no_sp_energy(no_handle* h, const double* h_k1, int n_k, int n_r, int n_cos, int n_phi, double* h_sigma,
                  void* cuda_stream) {
   if (!h || n_k < 0) return NO_ERR_INVALID;
   if (n_k == 0) return NO_OK;
@@ -274,21 +286,16 @@ int no_sp_energy(const no_handle* h, const double* h_k1, int n_k, int n_r, int n
   double *d_k1 = nullptr, *d_nodes2 = nullptr, *d_cfg = nullptr, *d_w = nullptr, *d_diag = nullptr, *d_sigma = nullptr;
   int rc = NO_OK;
   cudaError_t e = cudaSuccess;
-  auto cleanup = [&]() {
-    if (d_k1) cudaFree(d_k1);
-    if (d_nodes2) cudaFree(d_nodes2);
-    if (d_cfg) cudaFree(d_cfg);
-    if (d_w) cudaFree(d_w);
-    if (d_diag) cudaFree(d_diag);
-    if (d_sigma) cudaFree(d_sigma);
-  };
+  {
+    double* base = nullptr;
+    const long long pairs = rows_chunk * n2;
+    rc = hf_scratch(h, 4LL * n_k + 4 * n2 + 14 * pairs + 2LL * n_k, &base);
+    if (rc != NO_OK) return rc;
+    d_k1 = base; d_nodes2 = d_k1 + 4LL * n_k; d_cfg = d_nodes2 + 4 * n2; d_w = d_cfg + 9 * pairs;
+    d_diag = d_w + pairs; d_sigma = d_diag + 4 * pairs;
+  }
+  auto cleanup = [&]() {};
 #define NO_SP_CUDA(call) do { e = (call); if (e != cudaSuccess) { rc = cuda_fail(e, #call); cleanup(); return rc; } } while (0)
-  NO_SP_CUDA(cudaMalloc((void**)&d_k1, sizeof(double) * 4 * (size_t)n_k));
-  NO_SP_CUDA(cudaMalloc((void**)&d_nodes2, sizeof(double) * 4 * (size_t)n2));
-  NO_SP_CUDA(cudaMalloc((void**)&d_cfg, sizeof(double) * 9 * (size_t)(rows_chunk * n2)));
-  NO_SP_CUDA(cudaMalloc((void**)&d_w, sizeof(double) * (size_t)(rows_chunk * n2)));
-  NO_SP_CUDA(cudaMalloc((void**)&d_diag, sizeof(double) * 4 * (size_t)(rows_chunk * n2)));
-  NO_SP_CUDA(cudaMalloc((void**)&d_sigma, sizeof(double) * 2 * (size_t)n_k));
   NO_SP_CUDA(cudaMemcpyAsync(d_k1, k1w.data(), sizeof(double) * 4 * (size_t)n_k, cudaMemcpyHostToDevice, s));
   NO_SP_CUDA(cudaMemsetAsync(d_sigma, 0, sizeof(double) * 2 * (size_t)n_k, s));
   for (int t2 = 0; t2 < 2; ++t2) {
@@ -368,6 +375,7 @@ int no_free(no_handle* h) {
   if (h->d_tab) cudaFree(h->d_tab);
   if (h->d_cfg) cudaFree(h->d_cfg);
   if (h->d_out) cudaFree(h->d_out);
+  if (h->hf_arena) cudaFree(h->hf_arena);
   if (h->host_path_ready) {
     cudaStreamDestroy(h->copy_stream);
     cudaEventDestroy(h->ev_chunk[0]);
