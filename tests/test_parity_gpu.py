@@ -88,7 +88,7 @@ def test_cfg1_all_configurations():
     print(f"cfg1: 256 configurations, max rel err {worst:.2e}")
 
 
-FULL_SIZE = [("cfg2", 4), ("cfg3", 8), ("cfg4", 4), ("cfg5", 2), ("paper", 16)]
+FULL_SIZE = [("cfg2", 16), ("cfg3", 32), ("cfg4", 8), ("cfg5", 2), ("paper", 64)]
 
 
 @pytest.mark.parametrize("name,n_sample", FULL_SIZE)
