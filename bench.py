@@ -371,7 +371,7 @@ def run_hf(args):
     t_dev = replicas.max_over_ranks(sum(step_ms) * 1e-3, dev)
     t_wall = replicas.max_over_ranks(sum(wall), dev)
     value = replicas.whole_job_rate(evals_step, args.steps, t_dev)
-    flops = FLOPS_PER_EVAL[False]
+    flops = 59.0      # forward fast path (p' = p): 20 DFMA + 12 DMUL + 7 DADD per node
     achieved = flops * evals_step * args.steps / (sum(step_ms) * 1e-3) / 1e12
     probe = binding.no_probe_fp64_peak(local, 200, stream.cuda_stream)
     cpu = None
@@ -405,7 +405,7 @@ def run_hf(args):
         "roofline": {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
                      "frac": achieved / FP64_PEAK_NOMINAL_TFLOPS, "traffic": None,
                      "peak_measured_dfma_probe": probe["tflops"], "flops_per_eval": flops,
-                     "kernel": "no3n::no3n_kernel (diagonal mode) + hf_pairs_kernel + hf_reduce_kernel"},
+                     "kernel": "no3n::no3n_kernel (forward fast path, diagonal mode) + hf_pairs_kernel + hf_reduce_kernel"},
         "cpu_baseline": cpu}), flush=True)
 
 

@@ -47,6 +47,7 @@ struct Variant {
   size_t smem;
   KernelFn fn_split;   // small-batch layout: the CTA's kSplit warps share one configuration
   size_t smem_split;
+  KernelFn fn_fwd;     // throughput layout for launches whose configurations all have p' = p (Hartree-Fock)
 };
 
 template <int NREG, bool C4>
@@ -55,6 +56,7 @@ Variant make_variant(int tab_doubles, int n_r_pad) {
   v.fn = no3n_kernel<NREG, C4, kWarps, kMinBlocks>;
   v.smem = smem_bytes<C4>(tab_doubles, n_r_pad, kWarps);
   v.fn_split = no3n_kernel<NREG, C4, kSplit, 3, kSplit>;
+  v.fn_fwd = no3n_kernel<NREG, C4, kWarps, kMinBlocks, 1, true>;
   v.smem_split = smem_bytes<C4>(tab_doubles, n_r_pad, kSplit);
   return v;
 }
@@ -107,7 +109,14 @@ struct DeviceGuard {
 };
 
 int launch(const no_handle* h, const double* d_cfg, long long n_cfg, double* d_out, cudaStream_t s,
-           int mode = kModeFull) {
+           int mode = kModeFull, bool forward = false) {
+  if (forward && h->layout != 2) {
+    const long long fb = (n_cfg + kWarps - 1) / kWarps;
+    if (fb > 2147483647LL) return NO_ERR_INVALID;
+    h->var.fn_fwd<<<(unsigned)fb, kWarps * 32, h->var.smem, s>>>(h->plan.dp, d_cfg, n_cfg, d_out, mode);
+    NO_CUDA(cudaGetLastError());
+    return NO_OK;
+  }
   if (h->layout == 2 || (h->layout == 0 && n_cfg * kSplit <= h->wave_cfg)) {
     if (n_cfg > 2147483647LL) return NO_ERR_INVALID;
     // even with kSplit warps each the configurations do not fill the warp slots: one CTA per configuration
@@ -168,6 +177,8 @@ int no_init_angular(no_handle** out, const no_params* p, const double* h_dirs, i
   if (h->var.smem > (size_t)smem_optin || h->var.smem_split > (size_t)smem_optin) { delete h; return NO_ERR_INVALID; }
   e = cudaFuncSetAttribute((const void*)h->var.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
   if (e != cudaSuccess) { delete h; return cuda_fail(e, "cudaFuncSetAttribute(smem)"); }
+  e = cudaFuncSetAttribute((const void*)h->var.fn_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
+  if (e != cudaSuccess) { delete h; return cuda_fail(e, "cudaFuncSetAttribute(smem, forward)"); }
   e = cudaFuncSetAttribute((const void*)h->var.fn_split, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
   if (e != cudaSuccess) { delete h; return cuda_fail(e, "cudaFuncSetAttribute(smem, split)"); }
   {
@@ -251,7 +262,7 @@ int no_hf_energy(no_handle* h, int n_r, int n_cos, int n_phi, double* e_over_v, 
         const long long count = n1 * n1 - c0 < chunk ? n1 * n1 - c0 : chunk;
         hf_pairs_kernel<<<(unsigned)((count + 255) / 256), 256, 0, s>>>(d_nodes[t1], d_nodes[t2], n1, c0, count, d_cfg, d_w);
         NO_HF_CUDA(cudaGetLastError());
-        rc = launch(h, d_cfg, count, d_diag, s, kModeDiag);
+        rc = launch(h, d_cfg, count, d_diag, s, kModeDiag, true);   // p' = p by construction
         if (rc != NO_OK) { cleanup(); return rc; }
         hf_reduce_kernel<<<1, 1024, 0, s>>>(d_diag, d_w, count, 2 * t1 + t2, d_acc);
         NO_HF_CUDA(cudaGetLastError());
@@ -306,7 +317,7 @@ int no_sp_energy(no_handle* h, const double* h_k1, int n_k, int n_r, int n_cos, 
       const long long rows = n_k - r0 < rows_chunk ? n_k - r0 : rows_chunk, count = rows * n2;
       hf_pairs_kernel<<<(unsigned)((count + 255) / 256), 256, 0, s>>>(d_k1, d_nodes2, n2, r0 * n2, count, d_cfg, d_w);
       NO_SP_CUDA(cudaGetLastError());
-      rc = launch(h, d_cfg, count, d_diag, s, kModeDiag);
+      rc = launch(h, d_cfg, count, d_diag, s, kModeDiag, true);   // p' = p by construction
       if (rc != NO_OK) { cleanup(); return rc; }
       // (1/2) from xi = 1/2 of Eq. (10), (1/2) from averaging the spin of particle 1 out of the traced diagonal
       sp_reduce_kernel<<<(unsigned)rows, 256, 0, s>>>(d_diag, d_w, n2, t2, 0.25, r0, d_sigma);

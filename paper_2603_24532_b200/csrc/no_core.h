@@ -319,7 +319,11 @@ NO_HD void radial_entry(const CfgConst& c, double r, double* T) {
 // instead of 2 (profiles/r01b.md), so the body is arranged to need at most two: the weight wF is
 // folded into the shared reciprocal, y = wF/(D0 D1 D2 D3), the pair and leg terms are products of y
 // with the D's, the k = 0 sums are plain additions and the k = 1 sums are FMAs with the uniform r.
-template <int NREG, int W, bool FLUSH>
+//
+// FWD: forward configurations p' = p (the Hartree-Fock contractions): k1' = k1 and k2' = k2, so legs 2, 3 coincide
+// with legs 0, 1 and pair 3 with pair 2.  The duplicates are not computed: D2 = D0, D3 = D1 (the common
+// subexpressions collapse), S[2], S[3], G[3] are not accumulated (first_fwd_fill copies them per direction).
+template <int NREG, int W, bool FLUSH, bool FWD = false>
 NO_HD void nodes(const double* rs, int n_reg, const double* e2tab, const DirConst& d, const double* r,
                  const double* wr, const double (*T)[5], First& f) {
   double F[W], D0[W], D1[W], D2[W], D3[W], q02[W], q13[W], q03[W], q12[W], den[W], x[W];
@@ -327,8 +331,8 @@ NO_HD void nodes(const double* rs, int n_reg, const double* e2tab, const DirCons
   for (int k = 0; k < W; ++k) {
     D0[k] = fma(d.bet[0], r[k], T[k][1]);
     D1[k] = fma(d.bet[1], r[k], T[k][2]);
-    D2[k] = fma(d.bet[2], r[k], T[k][3]);
-    D3[k] = fma(d.bet[3], r[k], T[k][4]);
+    D2[k] = FWD ? D0[k] : fma(d.bet[2], r[k], T[k][3]);
+    D3[k] = FWD ? D1[k] : fma(d.bet[3], r[k], T[k][4]);
   }
 #pragma unroll
   for (int k = 0; k < W; ++k) { q02[k] = D0[k] * D2[k]; q13[k] = D1[k] * D3[k]; }
@@ -337,7 +341,7 @@ NO_HD void nodes(const double* rs, int n_reg, const double* e2tab, const DirCons
 #pragma unroll
   for (int k = 0; k < W; ++k) x[k] = rcp_seed(den[k]);
 #pragma unroll
-  for (int k = 0; k < W; ++k) { q03[k] = D0[k] * D3[k]; q12[k] = D1[k] * D2[k]; }
+  for (int k = 0; k < W; ++k) { q03[k] = D0[k] * D3[k]; q12[k] = FWD ? q03[k] : D1[k] * D2[k]; }
   if (NREG >= 0) {
     double d2[W], h[W], tm[W], kf[W], fr[W], Ts[W];
 #pragma unroll
@@ -378,34 +382,32 @@ NO_HD void nodes(const double* rs, int n_reg, const double* e2tab, const DirCons
     g0[k] = y[k] * q13[k];   // wF/(D0 D2): pair 0 = legs (0, 2)
     g1[k] = y[k] * q02[k];   // wF/(D1 D3): pair 1 = legs (1, 3)
     g2[k] = y[k] * q12[k];   // wF/(D0 D3): pair 2 = legs (0, 3)
-    g3[k] = y[k] * q03[k];   // wF/(D1 D2): pair 3 = legs (1, 2)
+    g3[k] = FWD ? g2[k] : y[k] * q03[k];   // wF/(D1 D2): pair 3 = legs (1, 2)
   }
 #pragma unroll
   for (int k = 0; k < W; ++k) {
     i0[k] = g0[k] * D2[k];   // wF/D0
-    i2[k] = g0[k] * D0[k];   // wF/D2
+    i2[k] = FWD ? i0[k] : g0[k] * D0[k];   // wF/D2
     i1[k] = g1[k] * D3[k];   // wF/D1
-    i3[k] = g1[k] * D1[k];   // wF/D3
+    i3[k] = FWD ? i1[k] : g1[k] * D1[k];   // wF/D3
   }
 #pragma unroll
   for (int k = 0; k < W; ++k) {
     f.R0 += wf[k];
     f.S[0][0] += i0[k];
     f.S[1][0] += i1[k];
-    f.S[2][0] += i2[k];
-    f.S[3][0] += i3[k];
+    if (!FWD) { f.S[2][0] += i2[k]; f.S[3][0] += i3[k]; }
     f.G[0][0] += g0[k];
     f.G[1][0] += g1[k];
     f.G[2][0] += g2[k];
-    f.G[3][0] += g3[k];
+    if (!FWD) f.G[3][0] += g3[k];
     f.S[0][1] = fma(i0[k], r[k], f.S[0][1]);
     f.S[1][1] = fma(i1[k], r[k], f.S[1][1]);
-    f.S[2][1] = fma(i2[k], r[k], f.S[2][1]);
-    f.S[3][1] = fma(i3[k], r[k], f.S[3][1]);
+    if (!FWD) { f.S[2][1] = fma(i2[k], r[k], f.S[2][1]); f.S[3][1] = fma(i3[k], r[k], f.S[3][1]); }
     f.G[0][1] = fma(g0[k], r[k], f.G[0][1]);
     f.G[1][1] = fma(g1[k], r[k], f.G[1][1]);
     f.G[2][1] = fma(g2[k], r[k], f.G[2][1]);
-    f.G[3][1] = fma(g3[k], r[k], f.G[3][1]);
+    if (!FWD) f.G[3][1] = fma(g3[k], r[k], f.G[3][1]);
   }
 }
 
@@ -430,34 +432,37 @@ NO_HD void rmw_rank012(double* a, const double* wt, double s0, double s1, double
   for (int k = 0; k < 5; ++k) p[k] = v[k];
 }
 
-template <bool C4>
+// FWD: the rows of legs 2, 3 and of pair 3 are left untouched (the kernel copies them from legs 0, 1 and pair 2
+// after the lane reduction)
+template <bool C4, bool FWD = false>
 NO_HD void second_level(const First& f, const DirConst& d, const double* gam, double w, double* acc /* this lane's rows */) {
   const double ux = d.u[0], uy = d.u[1], uz = d.u[2];
   double wt[10];      // w * (1, ux, uy, uz, ux ux, ux uy, ux uz, uy uy, uy uz, uz uz)
   wt[0] = w; wt[1] = w * ux; wt[2] = w * uy; wt[3] = w * uz;
   wt[4] = wt[1] * ux; wt[5] = wt[1] * uy; wt[6] = wt[1] * uz; wt[7] = wt[2] * uy; wt[8] = wt[2] * uz; wt[9] = wt[3] * uz;
   NO_FENCE();
-  for (int l = 0; l < 4; ++l) {
+  for (int l = 0; l < (FWD ? 2 : 4); ++l) {
     const double S2 = fma(-gam[l], f.S[l][0], fma(-d.bet[l], f.S[l][1], f.R0));   // sum wF r^2 / D_l
     rmw_rank012(acc + Layout<C4>::kRowLeg + 10 * l, wt, f.S[l][0], f.S[l][1], S2);
   }
   if (C4) {
-    for (int t = 0; t < 4; ++t) {
-      const int x = NO_PAIR_X(t), y = NO_PAIR_Y(t);
+    for (int t = 0; t < (FWD ? 3 : 4); ++t) {
+      const int x = NO_PAIR_X(t), y = FWD ? (NO_PAIR_Y(t) - 2) : NO_PAIR_Y(t);          // FWD: leg y coincides with y - 2
       const double G2 = fma(-gam[x], f.G[t][0], fma(-d.bet[x], f.G[t][1], f.S[y][0]));   // sum wF r^2/(D_x D_y)
       rmw_rank012(acc + Layout<C4>::kRowPair + 10 * t, wt, f.G[t][0], f.G[t][1], G2);     // Gm0, Gm1, Gm2
     }
   } else {
     Pair* p = reinterpret_cast<Pair*>(acc + Layout<C4>::kRowPair);   // Gm0, Gm1[3] of the four pairs
+    constexpr int np = FWD ? 3 : 4;
     Pair v[8];
-    for (int k = 0; k < 8; ++k) v[k] = p[k];
-    for (int t = 0; t < 4; ++t) {
+    for (int k = 0; k < 2 * np; ++k) v[k] = p[k];
+    for (int t = 0; t < np; ++t) {
       v[2 * t].x = fma(wt[0], f.G[t][0], v[2 * t].x);
       v[2 * t].y = fma(wt[1], f.G[t][1], v[2 * t].y);
       v[2 * t + 1].x = fma(wt[2], f.G[t][1], v[2 * t + 1].x);
       v[2 * t + 1].y = fma(wt[3], f.G[t][1], v[2 * t + 1].y);
     }
-    for (int k = 0; k < 8; ++k) p[k] = v[k];
+    for (int k = 0; k < 2 * np; ++k) p[k] = v[k];
   }
   acc[Layout<C4>::kRowR0] = fma(w, f.R0, acc[Layout<C4>::kRowR0]);
   NO_FENCE();

@@ -66,7 +66,7 @@ inline size_t smem_bytes(int tab_doubles, int n_r_pad, int warps) {
 }
 
 // radial loop of one direction: kNodesPerTrip independent nodes per trip
-template <int NREG, bool FLUSH>
+template <int NREG, bool FLUSH, bool FWD>
 __device__ __forceinline__ void radial_loop(const DevParams& P, int pass, const double* rsp, const double* e2tab,
                                             const DirConst& d, const double2* tt2, const double* ttab, First& f) {
 #pragma unroll 1
@@ -79,7 +79,7 @@ __device__ __forceinline__ void radial_loop(const DevParams& P, int pass, const 
       r[k] = P.radk[pass][i + k][0]; wr[k] = P.radk[pass][i + k][1];
       T[k][0] = t0.x; T[k][1] = t0.y; T[k][2] = t1.x; T[k][3] = t1.y; T[k][4] = t2;
     }
-    nodes<NREG, kNodesPerTrip, FLUSH>(rsp, P.n_reg, e2tab, d, r, wr, T, f);
+    nodes<NREG, kNodesPerTrip, FLUSH, FWD>(rsp, P.n_reg, e2tab, d, r, wr, T, f);
   }
 }
 
@@ -87,7 +87,9 @@ __device__ __forceinline__ void radial_loop(const DevParams& P, int pass, const 
 // SPLIT = WARPS > 1: the whole CTA integrates ONE configuration, the directions dealt round-robin to its warps,
 // the reduced moments of the warps added in a fixed order by warp 0, which then runs the epilogue alone: the
 // small-batch layout (fewer configurations than warp slots), chosen by the launcher.
-template <int NREG, bool C4, int WARPS, int MINB, int SPLIT = 1>
+// FWD: every configuration of the launch has p' = p exactly (set by the Hartree-Fock entry points, which build
+// the configurations themselves): duplicate legs and pairs are skipped, see no3n::nodes.
+template <int NREG, bool C4, int WARPS, int MINB, int SPLIT = 1, bool FWD = false>
 __global__ void __launch_bounds__(WARPS * 32, MINB)
 no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg, long long n_cfg, double* __restrict__ out,
             int mode) {
@@ -175,9 +177,9 @@ no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg,
       }
       First f;
       first_zero(f);
-      if (flush) radial_loop<NREG, true>(P, pass, rsp, e2tab, d, tt2, ttab, f);
-      else radial_loop<NREG, false>(P, pass, rsp, e2tab, d, tt2, ttab, f);
-      second_level<C4>(f, d, cc->gam, w, acc + lane * L::kStride);
+      if (flush) radial_loop<NREG, true, FWD>(P, pass, rsp, e2tab, d, tt2, ttab, f);
+      else radial_loop<NREG, false, FWD>(P, pass, rsp, e2tab, d, tt2, ttab, f);
+      second_level<C4, FWD>(f, d, cc->gam, w, acc + lane * L::kStride);
       j += dj; l += dl;
       if (l >= P.n_phi) { l -= P.n_phi; ++j; }
     }
@@ -198,6 +200,12 @@ no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg,
     }
     __syncwarp();
 
+    if (FWD) {                                          // legs 2, 3 = legs 0, 1; pair 3 = pair 2
+      __syncwarp();
+      if (lane < 20) mom[L::kRowLeg + 20 + lane] = mom[L::kRowLeg + lane];
+      if (lane < L::kPairRows) mom[L::kRowPair + 3 * L::kPairRows + lane] = mom[L::kRowPair + 2 * L::kPairRows + lane];
+      __syncwarp();
+    }
     if (SPLIT > 1) {                                    // add the warps' partial moments (fixed order)
       __syncthreads();
       if (warp == 0)
