@@ -29,14 +29,30 @@ if ROOT not in sys.path:
 METRIC = "3N-NO k3-point matrix-element evals/s (FP64) on 1 B200; % FP64 peak"
 UNIT = "evals/s"
 
-# FP64 flops the shipped kernel executes per k3-point evaluation (static count of the hot loop's SASS,
-# 2 per DFMA, 1 per DADD/DMUL; DESIGN.md section 7 shows the count and the ncu cross-check).
-FLOPS_PER_EVAL = {False: 76.0, True: 76.0}          # keyed by "c4 != 0" (the hot loop is the same)
 # nominal FP64 vector peak: 148 SMs x 64 DFMA lanes x 2 flops x 1.965 GHz
 FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the cfg2 kernel, from the ncu --set full capture
-# summarised in profiles/r01e.md (the output is still in L2 when the capture ends; the kernel is ALU bound)
-NCU_DRAM_BYTES_PER_LAUNCH = {"cfg2": 639232}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch (mean over the launches of one step) of the workload's
+# kernel, from the ncu capture named beside it (profiles/); None = no capture of that workload exists
+NCU_DRAM_BYTES_PER_LAUNCH = {}
+NCU_DRAM_SOURCE = {}
+
+
+def flops_per_eval(n_reg: int, regulated: bool, forward: bool = False) -> float:
+    """FP64 flops the shipped kernel executes per k3-point evaluation, by kernel variant: static count of the
+    hot loop body (no3n::nodes; 2 per DFMA, 1 per DADD/DMUL; DESIGN.md section 7 shows the count and the ncu
+    cross-check).  Regulated, exponent n: 22 + (n - 1) DFMA, 16 DMUL, 10 DADD (n = 4: 25/16/10 = 76 flops);
+    unregulated: 15/14/9; the forward variant (p' = p) drops 5 DFMA, 4 DMUL, 3 DADD."""
+    if regulated:
+        fma, mul, add = 22 + (n_reg - 1), 16, 10
+    else:
+        fma, mul, add = 15, 14, 9
+    if forward:
+        fma, mul, add = fma - 5, mul - 4, add - 3
+    return float(2 * fma + mul + add)
+
+
+def run_flops(run) -> float:
+    return flops_per_eval(run.n_reg, run.Lambda > 0)
 
 
 def parse_args():
@@ -44,10 +60,11 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "c4", "paper", "hf"])
+    ap.add_argument("--workload", default="cfg5", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "c4", "paper", "hf"])
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the short runs of the other BASELINE configs")
     ap.add_argument("--cpu-sample", type=int, default=0, help="configurations in the oracle sample (0 = auto)")
     return ap.parse_args()
 
@@ -110,25 +127,32 @@ class ClockSampler:
 # --------------------------------------------------------------------------------------------
 # CPU oracle legs
 # --------------------------------------------------------------------------------------------
-def oracle_sample(workload, n_sample: int):
+def oracle_sample(workload, n_sample: int, target_evals: float):
     """Bounded sample of the workload for the oracle: the first n_sample configurations of run 0 at the
-    full k3 grid (auto: about 5e5 evaluations, ~10-30 s on 8 cores)."""
+    full k3 grid (auto: about target_evals evaluations, at least one configuration per host core so that the
+    OpenMP loop over configurations uses every core)."""
+    from oracle import oracle as O
     run = workload.runs[0]
     if n_sample <= 0:
-        n_sample = max(1, min(run.n_cfg, int(round(5.0e5 / run.nodes_per_cfg))))
+        n_sample = max(O.num_threads(), int(round(target_evals / run.nodes_per_cfg)))
+    n_sample = max(1, min(run.n_cfg, n_sample))
     return run, run.configurations(n_sample), n_sample
 
 
+ORACLE_KIND = "oracle (level 1, f64 instantiation; the parity reference is the long-double one)"
+
+
 def time_oracle(workload, n_sample: int):
+    """cpu_baseline: the oracle as it stands (level 1, double), about 10-20 s on the box's host cores."""
     from oracle import oracle as O
-    run, cfg, n = oracle_sample(workload, n_sample)
+    run, cfg, n = oracle_sample(workload, n_sample, 8.0e6)
     t0 = time.perf_counter()
-    O.normal_order(cfg, level=1, precision="ld", dirs=run.angular(), **run.params())
+    O.normal_order(cfg, level=1, precision="f64", dirs=run.angular(), **run.params())
     dt = time.perf_counter() - t0
     evals = n * run.nodes_per_cfg
-    return {"value": evals / dt, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
+    return {"value": evals / dt, "unit": UNIT, "cores": O.num_threads(), "kind": ORACLE_KIND,
             "sample": f"first {n} configurations of run '{run.name}' of {workload.name} at the full "
-                      f"{run.nodes_per_cfg}-node grid ({evals} evaluations, {dt:.1f} s, level-1 long double)"}, dt
+                      f"{run.nodes_per_cfg}-node grid ({evals} evaluations, {dt:.1f} s)"}, dt
 
 
 def run_reference(args, workload):
@@ -142,13 +166,13 @@ def run_reference(args, workload):
         os.environ["OMP_NUM_THREADS"] = str(os.cpu_count() or 1)
     from oracle import oracle as O
     O.build()
-    run, cfg, n = oracle_sample(workload, args.cpu_sample)
+    run, cfg, n = oracle_sample(workload, args.cpu_sample, 2.5e6)
     evals = n * run.nodes_per_cfg
     for _ in range(args.warmup):
-        O.normal_order(cfg[:max(1, n // 8)], dirs=run.angular(), **run.params())
+        O.normal_order(cfg[:max(1, n // 8)], level=1, precision="f64", dirs=run.angular(), **run.params())
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        O.normal_order(cfg, level=1, precision="ld", dirs=run.angular(), **run.params())
+        O.normal_order(cfg, level=1, precision="f64", dirs=run.angular(), **run.params())
     dt = (time.perf_counter() - t0) / args.steps
     value = evals / dt
     sample = (f"first {n} configurations of run '{run.name}' of {workload.name} at the full "
@@ -157,7 +181,7 @@ def run_reference(args, workload):
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload.name, "description": workload.description, "sample": sample},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": O.num_threads(), "kind": ORACLE_KIND,
                              "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -167,12 +191,60 @@ def run_reference(args, workload):
 # --------------------------------------------------------------------------------------------
 # the CUDA arm
 # --------------------------------------------------------------------------------------------
+class DeviceWorkload:
+    """A workload resident on the device: one handle, one configuration array and one output array per run."""
+
+    def __init__(self, workload, local, dev, pinned_inputs=False):
+        import torch
+
+        from paper_2603_24532_b200 import binding, replicas
+        self.binding = binding
+        self.workload = workload
+        # replicas only (DESIGN.md section 9): every rank integrates the whole workload on its own GPU
+        self.runs = replicas.replica_runs(workload)
+        self.handles = [binding.no_init(device=local, angular=r.angular(), **r.params()) for r in self.runs]
+        self.h_cfg = [torch.from_numpy(r.configurations()) for r in self.runs]
+        if pinned_inputs:
+            self.h_cfg = [c.pin_memory() for c in self.h_cfg]
+        self.d_cfg = [c.to(dev, non_blocking=True) for c in self.h_cfg]
+        self.d_out = [torch.empty((r.n_cfg, 16, 16, 2), dtype=torch.float64, device=dev) for r in self.runs]
+        self.evals_step = sum(binding.no_evals_per_cfg(h) * r.n_cfg for h, r in zip(self.handles, self.runs))
+        assert self.evals_step == workload.evals
+        self.flops_step = sum(run_flops(r) * r.evals for r in self.runs)
+
+    def step(self, stream):
+        for h, c, o, r in zip(self.handles, self.d_cfg, self.d_out, self.runs):
+            self.binding.no_eval(h, c.data_ptr(), r.n_cfg, o.data_ptr(), stream.cuda_stream)
+
+    def close(self):
+        for h in self.handles:
+            self.binding.no_free(h)
+        self.handles = []
+        self.d_cfg = self.d_out = self.h_cfg = None
+
+
+def timed_steps(dw, stream, dev, flush, steps, warmup, barrier):
+    """`warmup` untimed steps, then `steps` timed ones: CUDA events on the launching stream around each step,
+    the L2 flushed (256 MiB rewritten) before each, outside the event bracket.  Returns the per-step ms."""
+    import torch
+    for _ in range(warmup):
+        dw.step(stream)
+    barrier()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for a, b in ev:
+        flush.zero_()
+        a.record(stream)
+        dw.step(stream)
+        b.record(stream)
+    barrier()
+    return [a.elapsed_time(b) for a, b in ev]
+
+
 def run_b200(args, workload):
-    import numpy as np
     import torch
     import torch.distributed as dist
 
-    from paper_2603_24532_b200 import binding, build, replicas
+    from paper_2603_24532_b200 import binding, build, replicas, workloads
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -187,44 +259,26 @@ def run_b200(args, workload):
     dev = torch.device("cuda", local)
     stream = torch.cuda.current_stream(dev)
 
-    # replicas only: every rank integrates the whole workload on its own GPU
-    runs = replicas.replica_runs(workload)
-    handles = [binding.no_init(device=local, angular=r.angular(), **r.params()) for r in runs]
-    h_cfg = [torch.from_numpy(r.configurations()).pin_memory() for r in runs]
-    d_cfg = [c.to(dev, non_blocking=True) for c in h_cfg]
-    d_out = [torch.empty((r.n_cfg, 16, 16, 2), dtype=torch.float64, device=dev) for r in runs]
-    evals_step = sum(binding.no_evals_per_cfg(h) * r.n_cfg for h, r in zip(handles, runs))
-    assert evals_step == workload.evals
+    dw = DeviceWorkload(workload, local, dev, pinned_inputs=not args.no_e2e)
+    runs, handles, evals_step = dw.runs, dw.handles, dw.evals_step
     flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)   # 256 MiB > 126 MB L2
     info = binding.no_kernel_info(handles[0])
-
-    def step_device():
-        for h, c, o, r in zip(handles, d_cfg, d_out, runs):
-            binding.no_eval(h, c.data_ptr(), r.n_cfg, o.data_ptr(), stream.cuda_stream)
 
     def barrier():
         replicas.barrier()
         torch.cuda.synchronize(dev)
 
-    for _ in range(max(args.warmup, 3)):
-        step_device()
+    warmup = max(args.warmup, 3)
+    for _ in range(warmup):
+        dw.step(stream)
     barrier()
-
     sampler = ClockSampler(local)
     sampler.start()
     time.sleep(0.25)
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    barrier()
     t_wall0 = time.perf_counter()
-    for a, b in ev:
-        flush.zero_()                      # L2 flush between timed iterations, outside the event bracket
-        a.record(stream)
-        step_device()
-        b.record(stream)
-    barrier()
+    step_ms = timed_steps(dw, stream, dev, flush, args.steps, 0, barrier)
     t_wall = time.perf_counter() - t_wall0
     clocks = sampler.stop()
-    step_ms = [a.elapsed_time(b) for a, b in ev]
     t_dev = replicas.max_over_ranks(sum(step_ms) * 1e-3, dev)
     value = replicas.whole_job_rate(evals_step, args.steps, t_dev)
     n_launch = len(runs) * args.steps
@@ -232,15 +286,15 @@ def run_b200(args, workload):
     # ---- end to end through the C ABI with HOST buffers (H2D + D2H inside the timed region) ----
     e2e = None
     if not args.no_e2e:
-        h_out = [torch.empty((r.n_cfg, 16, 16, 2), dtype=torch.float64).pin_memory() for r in runs]
+        h_out = [torch.empty((r.n_cfg, 16, 16, 2), dtype=torch.float64, pin_memory=True) for r in runs]
 
         def step_host():
-            for h, c, o, r in zip(handles, h_cfg, h_out, runs):
+            for h, c, o, r in zip(handles, dw.h_cfg, h_out, runs):
                 binding.no_eval_host(h, c.data_ptr(), r.n_cfg, o.data_ptr(), stream.cuda_stream)
 
         step_host()
         barrier()
-        k = max(1, min(args.steps, 3))
+        k = max(1, min(args.steps, 5))
         t0 = time.perf_counter()
         for _ in range(k):
             step_host()
@@ -248,47 +302,68 @@ def run_b200(args, workload):
         t_e2e = replicas.max_over_ranks((time.perf_counter() - t0) / k, dev)
         chk = float(h_out[0][0].abs().sum())          # the step's result is read on the host
         e2e = {"value": world * evals_step / t_e2e, "unit": UNIT,
-               "h2d_bytes_per_step": int(sum(c.numel() * 8 for c in h_cfg)),
+               "h2d_bytes_per_step": int(sum(c.numel() * 8 for c in dw.h_cfg)),
                "d2h_bytes_per_step": int(sum(o.numel() * 8 for o in h_out)),
-               "ms_per_step": t_e2e * 1e3, "steps": k, "checksum": chk}
+               "ms_per_step": t_e2e * 1e3, "steps": k, "checksum": chk,
+               "api": "no_eval_host (pinned host buffers; full 16x16 matrices)"}
         del h_out
 
     # ---- roofline of the (single) kernel: FP64 ALU bound ----
-    has_c4 = any(r.c4 != 0.0 for r in runs)
-    flops_step = FLOPS_PER_EVAL[has_c4] * evals_step
     launch_ms = sum(step_ms) / n_launch
-    achieved = flops_step * args.steps / (sum(step_ms) * 1e-3) / 1e12
+    achieved = dw.flops_step * args.steps / (sum(step_ms) * 1e-3) / 1e12
     probe = binding.no_probe_fp64_peak(local, 200, stream.cuda_stream)
+    per_run_flops = sorted({run_flops(r) for r in runs})
     roofline = {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
                 "frac": achieved / FP64_PEAK_NOMINAL_TFLOPS, "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(workload.name),
-                "traffic_source": "profiles/r01e.md (ncu --set full, per launch)" if workload.name in NCU_DRAM_BYTES_PER_LAUNCH else None,
+                "traffic_source": NCU_DRAM_SOURCE.get(workload.name),
                 "peak_source": "nominal 148 SM x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md section 7); "
-                               "MEASURED_PEAKS.json has no FP64 entry",
+                               "MEASURED_PEAKS.json has no FP64 entry, the in-run DFMA probe is the measured figure",
                 "peak_measured_dfma_probe": probe["tflops"],
                 "frac_of_measured_dfma": achieved / probe["tflops"] if probe["tflops"] > 0 else None,
-                "flops_per_eval": FLOPS_PER_EVAL[has_c4], "kernel": "no3n::no3n_kernel",
-                "avg_launch_ms": launch_ms, "launches_per_step": len(runs),
+                "flops_per_eval": dw.flops_step / evals_step, "flops_per_eval_by_variant": per_run_flops,
+                "kernel": "no3n::no3n_kernel", "avg_launch_ms": launch_ms, "launches_per_step": len(runs),
                 "algorithmic_bytes_per_launch": int(sum(r.n_cfg * (72 + 4096) for r in runs) / len(runs)),
                 "kernel_info": info}
+    dw.close()
+
+    # ---- the other BASELINE configs, a few steps each in the same run (not the headline) ----
+    per_config = None
+    if world == 1 and not args.no_per_config:
+        per_config = {}
+        for name in ("cfg1", "cfg2", "cfg3", "cfg4", "cfg5"):
+            if name == workload.name:
+                continue
+            if name == "cfg5" and args.workload != "cfg5":
+                continue                                           # 2.8 s per step: only as the headline
+            wl = workloads.workload(name)
+            d2 = DeviceWorkload(wl, local, dev)
+            ms = timed_steps(d2, stream, dev, flush, 3, 3, barrier)
+            rate = wl.evals * len(ms) / (sum(ms) * 1e-3)
+            fl = d2.flops_step / wl.evals
+            per_config[name] = {"evals_per_s": rate, "cfg_per_s": wl.n_cfg * len(ms) / (sum(ms) * 1e-3),
+                                "ms_per_step": sum(ms) / len(ms), "steps": len(ms), "flops_per_eval": fl,
+                                "frac": rate * fl / 1e12 / FP64_PEAK_NOMINAL_TFLOPS}
+            d2.close()
+            del d2
+            torch.cuda.empty_cache()
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu, _ = time_oracle(workload, args.cpu_sample)
 
-    for h in handles:
-        binding.no_free(h)
     if world > 1:
         dist.destroy_process_group()
     if rank != 0:
         return
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": max(args.warmup, 3), "ms_per_step": t_dev / args.steps * 1e3, "higher_is_better": True,
+            "warmup": warmup, "ms_per_step": t_dev / args.steps * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload.name, "description": workload.description,
                        "n_cfg": workload.n_cfg, "evals_per_step": evals_step, "launches_per_step": len(runs),
                        "cfg_per_s": world * workload.n_cfg * args.steps / t_dev,
                        "l2": "256 MiB buffer rewritten between timed steps (L2 flush); the kernel is ALU bound",
-                       "parallelism": "replicas only: every rank integrates the whole workload"},
+                       "parallelism": "replicas only: every rank integrates the whole workload",
+                       "per_config": per_config},
             "clocks": clocks, "e2e": e2e, "gpu_launches": n_launch, "roofline": roofline, "cpu_baseline": cpu,
             "wall_s_timed_region": t_wall}
     print(json.dumps(line), flush=True)
@@ -303,7 +378,7 @@ HF_PAIR_GRID = (12, 12, 12)          # particles 1 and 2: 1728 nodes per Fermi s
 
 
 def run_hf(args):
-    """One step = one no_hf_energy call: 4 x 1728^2 pair configurations generated on the device, each reduced
+    """One step = one no_hf_energy call: 1728^2 pair configurations generated on the device, each reduced
     to its spin-traced diagonal over a 16^3 k3 grid inside the kernel, fixed-order reduction to E/V."""
     import torch
 
@@ -343,9 +418,10 @@ def run_hf(args):
     stream = torch.cuda.current_stream(dev)
     h = binding.no_init(device=local, **HF_PARAMS)
     n1 = HF_PAIR_GRID[0] * HF_PAIR_GRID[1] * HF_PAIR_GRID[2]
-    n_pairs = 4 * n1 * n1
+    # kF_n = kF_p: the four (t1, t2) pair grids coincide and the library integrates the pair grid once
+    n_pairs = n1 * n1
     evals_step = n_pairs * binding.no_evals_per_cfg(h)
-    chunks = 4 * ((n1 * n1 + (1 << 20) - 1) >> 20)
+    chunks = (n1 * n1 + (1 << 20) - 1) >> 20
     flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)
     for _ in range(max(args.warmup, 3)):
         e_v = binding.no_hf_energy(h, *HF_PAIR_GRID, stream.cuda_stream)
@@ -392,14 +468,14 @@ def run_hf(args):
         "ms_per_step": t_dev / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": "hf", "description": "3N Hartree-Fock energy of SNM kF=1.33 by repeated normal ordering "
-                   "(no_hf_energy): 12^3 nodes per sphere for particles 1, 2 (4 x 1728^2 pair configurations, generated "
-                   "on the device), 16^3 k3 grid", "n_cfg": n_pairs, "evals_per_step": evals_step,
+                   "(no_hf_energy): 12^3 nodes per sphere for particles 1, 2 (1728^2 pair configurations, generated "
+                   "on the device; since kF_n = kF_p the four isospin pair grids coincide and 1728^2 are integrated), 16^3 k3 grid", "n_cfg": n_pairs, "evals_per_step": evals_step,
                    "cfg_per_s": world * n_pairs * args.steps / t_dev, "e_over_v_fm4": e_v,
                    "l2": "256 MiB buffer rewritten between timed steps (L2 flush); the kernel is ALU bound",
                    "parallelism": "replicas only: every rank integrates the whole workload"},
         "clocks": clocks,
         "e2e": {"value": world * evals_step * args.steps / t_wall, "unit": UNIT,
-                "h2d_bytes_per_step": 4 * n1 * 32, "d2h_bytes_per_step": 4 * 8, "ms_per_step": t_wall / args.steps * 1e3,
+                "h2d_bytes_per_step": n1 * 32, "d2h_bytes_per_step": 8, "ms_per_step": t_wall / args.steps * 1e3,
                 "note": "the call itself is the public API: node lists up, one scalar down, wall clock around it"},
         "gpu_launches": 3 * chunks * args.steps,
         "roofline": {"bound": "alu", "achieved": achieved, "peak": FP64_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",

@@ -34,7 +34,8 @@ extern "C" {
 #endif
 
 #define NO_OK          0
-#define NO_ERR_INVALID 1   /* bad parameter, null pointer, n_cfg < 0, misaligned pointer   */
+#define NO_ERR_INVALID 1   /* bad parameter, null pointer, n_cfg < 0, misaligned pointer, or a second
+                              concurrent call of a non-re-entrant entry point on one handle  */
 #define NO_ERR_CUDA    2   /* CUDA runtime or launch failure; text via no_last_cuda_error() */
 #define NO_ERR_ALLOC   3   /* host or device allocation failed                              */
 
@@ -63,8 +64,9 @@ int no_init(no_handle **h, const no_params *p);
 /* no_init with a caller-supplied ANGULAR rule instead of the cos(theta) x phi Gauss-Legendre grid:
  * the paper's own quadrature is "Gauss-Legendre radial x Lebedev angular" (16 radial points, order-15
  * Lebedev).  The k3 nodes of a sphere are r_i u_m, weights r_i^2 w_i w_m / (2 pi)^3.
- *   h_dirs : HOST, const, [n_dir][4] doubles = (ux, uy, uz, w): unit vectors in the fixed lab frame and
- *            weights with sum w = 4 pi (neither is checked; both are used as given), all finite
+ *   h_dirs : HOST, const, [n_dir][4] doubles = (ux, uy, uz, w): unit vectors in the fixed lab frame
+ *            (| |u|^2 - 1 | <= 1e-12, NO_ERR_INVALID otherwise: the kernel relies on |u| = 1) and weights
+ *            with sum w = 4 pi (not checked, used as given), all finite
  *   n_dir  : 1..4096 (NO_ERR_INVALID otherwise, or if the tables do not fit in shared memory)
  * p->n_cos and p->n_phi must still be valid orders but are otherwise unused; no_evals_per_cfg is
  * n_r * n_dir * (number of spheres).  h_dirs == NULL (with n_dir == 0) is no_init.  The array is
@@ -74,7 +76,8 @@ int no_init_angular(no_handle **h, const no_params *p, const double *h_dirs, int
 /* Enqueue the normal ordering of n_cfg configurations on `cuda_stream` (a cudaStream_t; NULL is
  * the default stream).  No synchronisation inside: the call returns as soon as the work is
  * enqueued ("asynchronous GPU transaction"); one handle may be used from several
- * streams at once.
+ * streams and host threads at once.  A batch that needs more CTAs than one grid holds is cut into several
+ * launches on the same stream.
  *   d_cfg : DEVICE, const, [n_cfg][9] doubles = p(xyz), p'(xyz), P(xyz) in fm^-1, dense,
  *           8-byte aligned, caller-owned
  *   d_out : DEVICE, [n_cfg][16][16][2] doubles (re, im), row-major rows = outgoing state,
@@ -87,7 +90,11 @@ int no_eval(const no_handle *h, const double *d_cfg, long long n_cfg, double *d_
  * four warps per configuration (small-batch layout: the directions are dealt to the warps, their partial moments
  * added in a fixed order).  Automatic picks 2 when four warps per configuration still leave warp slots of the
  * device empty.  Both layouts compute the same sums in different (fixed) orders: results agree to rounding and
- * are bit-reproducible within a layout.  Affects later no_eval / no_eval_diag / no_eval_host / no_hf_energy calls. */
+ * are bit-reproducible within a layout; with layout 0 the bits of a configuration therefore depend on the size of
+ * the batch it is evaluated in (never on its position in the batch: every entry point decides ONCE per call, from
+ * the whole batch).  The setting is atomic: it may be changed while other threads are inside no_eval (a call
+ * in flight keeps the layout it read at entry).  Affects later no_eval / no_eval_diag / no_eval_host /
+ * no_hf_energy / no_sp_energy calls. */
 int no_set_layout(no_handle *h, int layout);
 
 /* Same operation with HOST buffers (pageable or pinned): copies h_cfg to a device scratch owned
@@ -95,7 +102,9 @@ int no_set_layout(no_handle *h, int layout);
  * returning.  The batch is cut into chunks of a few waves: the device-to-host copy of a finished chunk
  * runs on an internal stream under the kernel of the next one (pinned h_out is needed for the copies to
  * be asynchronous; pageable memory is still correct).  Not re-entrant for one handle (the scratch is
- * shared).  Used for the end-to-end measurement. */
+ * shared): while one of no_eval_host / no_hf_energy / no_sp_energy runs on a handle, a second such call on
+ * the same handle returns NO_ERR_INVALID (no_eval / no_eval_diag stay re-entrant).  On a CUDA failure both
+ * streams are drained before the call returns.  Used for the end-to-end measurement. */
 int no_eval_host(no_handle *h, const double *h_cfg, long long n_cfg, double *h_out, void *cuda_stream);
 
 /* Spin-traced diagonal of the normal-ordered matrix, reduced inside the kernel (the 16x16 matrix is
@@ -113,7 +122,8 @@ int no_eval_diag(const no_handle *h, const double *d_cfg, long long n_cfg, doubl
  * handle's own k3 grid; configuration (p, p', P) = ((k1-k2)/2, (k1-k2)/2, k1+k2).  On the same grids this
  * equals the brute-force 9-dimensional sum exactly (pin P8).  Generates the pair configurations on the
  * device in chunks, enqueues on `cuda_stream`, SYNCHRONISES it, and writes the result to the HOST
- * double *e_over_v.  Uses a grow-only device scratch owned by the handle (not re-entrant for one handle). */
+ * double *e_over_v.  With kF_n = kF_p the four (t1, t2) pair grids coincide and are integrated once.
+ * Uses a grow-only device scratch owned by the handle (not re-entrant for one handle, see no_eval_host). */
 int no_hf_energy(no_handle *h, int n_r, int n_cos, int n_phi, double *e_over_v, void *cuda_stream);
 
 /* 3N part of the Hartree-Fock single-particle energy (self-energy) of Eq. (9), isospin

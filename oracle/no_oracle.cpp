@@ -631,6 +631,11 @@ void oracle_no_level1_dirs_ld(const Params* p, const double* cfg, long long n, c
                               double* out) {
   normal_order_level1<long double>(*p, cfg, n, out, dirs, n_dir);
 }
+// the same template in double (timed as the CPU baseline by bench.py; the parity reference is the _ld one)
+void oracle_no_level1_dirs_f64(const Params* p, const double* cfg, long long n, const double* dirs, int n_dir,
+                               double* out) {
+  normal_order_level1<double>(*p, cfg, n, out, dirs, n_dir);
+}
 double oracle_hf3n_bruteforce(const Params* p) { return hf3n_bruteforce<long double>(*p); }
 
 int oracle_num_threads(void) {

@@ -50,8 +50,9 @@ def _load():
         for name in ("oracle_no_level0_ld", "oracle_no_level1_ld", "oracle_no_level1_f64"):
             getattr(lib, name).argtypes = [pp, dp, ctypes.c_longlong, dp]
             getattr(lib, name).restype = None
-        lib.oracle_no_level1_dirs_ld.argtypes = [pp, dp, ctypes.c_longlong, dp, ctypes.c_int, dp]
-        lib.oracle_no_level1_dirs_ld.restype = None
+        for name in ("oracle_no_level1_dirs_ld", "oracle_no_level1_dirs_f64"):
+            getattr(lib, name).argtypes = [pp, dp, ctypes.c_longlong, dp, ctypes.c_int, dp]
+            getattr(lib, name).restype = None
         lib.oracle_hf3n_bruteforce.argtypes = [pp]
         lib.oracle_hf3n_bruteforce.restype = ctypes.c_double
         lib.oracle_num_threads.restype = ctypes.c_int
@@ -102,17 +103,17 @@ def normal_order(cfg, level: int = 1, precision: str = "ld", dirs=None, **params
     level 0 = definition (64x64 per node); level 1 = spin and isospin traced separately.
     precision "ld" = long double arithmetic (parity reference), "f64" = double (level 1 only).
     dirs: optional caller-supplied angular rule [n_dir,4] = (ux, uy, uz, w), sum w = 4 pi, used instead
-    of the cos(theta) x phi Gauss-Legendre grid (level 1, long double): radial GL x Lebedev.
+    of the cos(theta) x phi Gauss-Legendre grid (level 1): radial GL x Lebedev.
     """
     cfg = np.ascontiguousarray(cfg, dtype=np.float64).reshape(-1, 9)
     n = cfg.shape[0]
     out = np.empty((n, 16, 16, 2))
     if dirs is not None:
-        assert level == 1 and precision == "ld"
+        assert level == 1 and precision in ("ld", "f64")
         dirs = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 4)
         if n:
-            _load().oracle_no_level1_dirs_ld(ctypes.byref(_params(params)), _dptr(cfg), n, _dptr(dirs),
-                                             dirs.shape[0], _dptr(out))
+            getattr(_load(), "oracle_no_level1_dirs_" + precision)(ctypes.byref(_params(params)), _dptr(cfg), n,
+                                                                   _dptr(dirs), dirs.shape[0], _dptr(out))
         return out[..., 0] + 1j * out[..., 1]
     name = {(0, "ld"): "oracle_no_level0_ld", (1, "ld"): "oracle_no_level1_ld",
             (1, "f64"): "oracle_no_level1_f64"}[(level, precision)]

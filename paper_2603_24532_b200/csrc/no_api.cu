@@ -3,7 +3,9 @@
 // no_kernel.cuh.  sm_100a only; there is no CPU path.
 #include <cuda_runtime.h>
 
+#include <atomic>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -40,6 +42,7 @@ constexpr int kMinBlocks = NO_MINB;   // resident CTAs per SM the register alloc
 
 typedef void (*KernelFn)(const DevParams, const double*, long long, double*, int);
 
+constexpr long long kMaxGrid = 2147483647LL;   // gridDim.x limit; larger batches are cut into several launches
 constexpr int kSplit = 4;       // warps per configuration of the small-batch layout (one configuration per CTA)
 
 struct Variant {
@@ -86,7 +89,10 @@ struct no_handle {
   long long scratch_cfg;
   double* hf_arena;           // grow-only device scratch of no_hf_energy / no_sp_energy
   long long hf_arena_doubles;
-  int layout;                 // 0 automatic, 1 always one warp per configuration, 2 always one CTA per configuration
+  std::atomic<int> layout;    // 0 automatic, 1 always one warp per configuration, 2 always one CTA per configuration;
+                              // every entry point reads it ONCE per call (no_set_layout may run concurrently)
+  std::atomic_flag busy;      // set while an entry point that uses the handle-owned scratch is running
+  long long max_grid;         // CTAs per launch (kMaxGrid; the test knob NO3N_MAX_GRID lowers it)
   long long wave_cfg;         // configurations of one full wave of resident CTAs (chunk granularity of the host path)
   cudaStream_t copy_stream;   // device-to-host copies of finished chunks overlap the next chunk's kernel
   cudaEvent_t ev_chunk[2], ev_copied;
@@ -108,28 +114,43 @@ struct DeviceGuard {
   }
 };
 
-int launch(const no_handle* h, const double* d_cfg, long long n_cfg, double* d_out, cudaStream_t s,
+// kernel layout of one call: 1 = one warp per configuration, 2 = one CTA of kSplit warps per configuration.
+// Decided ONCE per entry-point call from the handle's setting and the size of the whole batch, so that every
+// chunk of a call (and hence every configuration of it) runs the same summation order.
+int resolve_layout(const no_handle* h, long long n_cfg) {
+  const int want = h->layout.load(std::memory_order_relaxed);
+  if (want == 1 || want == 2) return want;
+  // automatic: even with kSplit warps each the configurations do not fill the warp slots -> one CTA each
+  return n_cfg * kSplit <= h->wave_cfg ? 2 : 1;
+}
+
+
+int launch(const no_handle* h, const double* d_cfg, long long n_cfg, double* d_out, cudaStream_t s, int layout,
            int mode = kModeFull, bool forward = false) {
-  if (forward && h->layout != 2) {
-    const long long fb = (n_cfg + kWarps - 1) / kWarps;
-    if (fb > 2147483647LL) return NO_ERR_INVALID;
-    h->var.fn_fwd<<<(unsigned)fb, kWarps * 32, h->var.smem, s>>>(h->plan.dp, d_cfg, n_cfg, d_out, mode);
+  const long long out_doubles = mode == kModeDiag ? 4 : 512;
+  const bool split = layout == 2;
+  const long long per_cta = split ? 1 : kWarps;
+  const KernelFn fn = split ? h->var.fn_split : (forward ? h->var.fn_fwd : h->var.fn);
+  const size_t smem = split ? h->var.smem_split : h->var.smem;
+  const int threads = split ? kSplit * 32 : kWarps * 32;
+  const long long max_cfg = h->max_grid * per_cta;
+  for (long long c0 = 0; c0 < n_cfg; c0 += max_cfg) {
+    const long long cnt = n_cfg - c0 < max_cfg ? n_cfg - c0 : max_cfg;
+    const long long blocks = (cnt + per_cta - 1) / per_cta;
+    fn<<<(unsigned)blocks, threads, smem, s>>>(h->plan.dp, d_cfg + 9 * c0, cnt, d_out + out_doubles * c0, mode);
     NO_CUDA(cudaGetLastError());
-    return NO_OK;
   }
-  if (h->layout == 2 || (h->layout == 0 && n_cfg * kSplit <= h->wave_cfg)) {
-    if (n_cfg > 2147483647LL) return NO_ERR_INVALID;
-    // even with kSplit warps each the configurations do not fill the warp slots: one CTA per configuration
-    h->var.fn_split<<<(unsigned)n_cfg, kSplit * 32, h->var.smem_split, s>>>(h->plan.dp, d_cfg, n_cfg, d_out, mode);
-    NO_CUDA(cudaGetLastError());
-    return NO_OK;
-  }
-  const long long blocks = (n_cfg + kWarps - 1) / kWarps;
-  if (blocks > 2147483647LL) return NO_ERR_INVALID;
-  h->var.fn<<<(unsigned)blocks, kWarps * 32, h->var.smem, s>>>(h->plan.dp, d_cfg, n_cfg, d_out, mode);
-  NO_CUDA(cudaGetLastError());
   return NO_OK;
 }
+
+// entry points that use the handle-owned scratch (host path, Hartree-Fock contractions) are not re-entrant for
+// one handle: a second concurrent call is refused instead of racing on the scratch
+struct BusyGuard {
+  no_handle* h;
+  bool ok;
+  explicit BusyGuard(no_handle* h_) : h(h_), ok(!h_->busy.test_and_set(std::memory_order_acquire)) {}
+  ~BusyGuard() { if (ok) h->busy.clear(std::memory_order_release); }
+};
 
 // grow-only scratch of the Hartree-Fock entry points (allocation inside a timed call costs far more than the
 // kernels when another process queries the driver, e.g. nvidia-smi)
@@ -157,7 +178,13 @@ int no_init_angular(no_handle** out, const no_params* p, const double* h_dirs, i
   if (!h_dirs && n_dir != 0) return NO_ERR_INVALID;
   no_handle* h = new (std::nothrow) no_handle();
   if (!h) return NO_ERR_ALLOC;
-  h->d_tab = nullptr; h->d_cfg = nullptr; h->d_out = nullptr; h->scratch_cfg = 0; h->host_path_ready = false; h->layout = 0; h->hf_arena = nullptr; h->hf_arena_doubles = 0;
+  h->d_tab = nullptr; h->d_cfg = nullptr; h->d_out = nullptr; h->scratch_cfg = 0; h->host_path_ready = false;
+  h->layout.store(0); h->busy.clear();
+  h->max_grid = kMaxGrid;
+  if (const char* e = getenv("NO3N_MAX_GRID")) {          // testing knob: exercises the multi-launch path at small sizes
+    const long long v = atoll(e);
+    if (v >= 1 && v < kMaxGrid) h->max_grid = v;
+  } h->hf_arena = nullptr; h->hf_arena_doubles = 0;
   int rc = build_plan(p, h->plan, h_dirs, n_dir);
   if (rc != NO_OK) { delete h; return rc; }
   int n_dev = 0;
@@ -207,12 +234,12 @@ int no_eval(const no_handle* h, const double* d_cfg, long long n_cfg, double* d_
   if ((reinterpret_cast<uintptr_t>(d_cfg) & 7u) || (reinterpret_cast<uintptr_t>(d_out) & 15u)) return NO_ERR_INVALID;
   DeviceGuard guard(h->device);
   if (!guard.ok) return cuda_fail(cudaGetLastError(), "cudaSetDevice");
-  return launch(h, d_cfg, n_cfg, d_out, static_cast<cudaStream_t>(cuda_stream));
+  return launch(h, d_cfg, n_cfg, d_out, static_cast<cudaStream_t>(cuda_stream), resolve_layout(h, n_cfg));
 }
 
 int no_set_layout(no_handle* h, int layout) {
   if (!h || layout < 0 || layout > 2) return NO_ERR_INVALID;
-  h->layout = layout;
+  h->layout.store(layout, std::memory_order_relaxed);
   return NO_OK;
 }
 
@@ -223,56 +250,54 @@ int no_eval_diag(const no_handle* h, const double* d_cfg, long long n_cfg, doubl
   if ((reinterpret_cast<uintptr_t>(d_cfg) & 7u) || (reinterpret_cast<uintptr_t>(d_out) & 7u)) return NO_ERR_INVALID;
   DeviceGuard guard(h->device);
   if (!guard.ok) return cuda_fail(cudaGetLastError(), "cudaSetDevice");
-  return launch(h, d_cfg, n_cfg, d_out, static_cast<cudaStream_t>(cuda_stream), kModeDiag);
+  return launch(h, d_cfg, n_cfg, d_out, static_cast<cudaStream_t>(cuda_stream), resolve_layout(h, n_cfg), kModeDiag);
 }
 
 int no_hf_energy(no_handle* h, int n_r, int n_cos, int n_phi, double* e_over_v, void* cuda_stream) {
   if (!h || !e_over_v) return NO_ERR_INVALID;
   if (n_r < 1 || n_r > kMaxOrder || n_cos < 1 || n_cos > kMaxOrder || n_phi < 1 || n_phi > kMaxOrder) return NO_ERR_INVALID;
+  BusyGuard busy(h);
+  if (!busy.ok) return NO_ERR_INVALID;
   DeviceGuard guard(h->device);
   if (!guard.ok) return cuda_fail(cudaGetLastError(), "cudaSetDevice");
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  const int layout = h->layout.load(std::memory_order_relaxed) == 2 ? 2 : 1;
   // single-particle grids of the two species (t = 0 proton, 1 neutron), [n][4] = (kx, ky, kz, W)
   const double kf[2] = {h->plan.kf_p, h->plan.kf_n};
+  // equal Fermi momenta: the four (t1, t2) pair grids coincide, so the pair grid is integrated ONCE and the
+  // four isospin columns of the traced diagonal are added in the reduction (same sum, a quarter of the work)
+  const bool fused = kf[0] > 0 && kf[0] == kf[1];
   std::vector<double> nodes[2];
   for (int t = 0; t < 2; ++t)
-    if (kf[t] > 0) sphere_nodes(n_r, n_cos, n_phi, kf[t], nodes[t]);
+    if (kf[t] > 0 && !(fused && t == 1)) sphere_nodes(n_r, n_cos, n_phi, kf[t], nodes[t]);
   const long long n1 = (long long)n_r * n_cos * n_phi;
   const long long chunk = n1 * n1 < (1LL << 20) ? n1 * n1 : (1LL << 20);
-  double *d_nodes[2] = {nullptr, nullptr}, *d_cfg = nullptr, *d_w = nullptr, *d_diag = nullptr, *d_acc = nullptr;
-  int rc = NO_OK;
-  cudaError_t e = cudaSuccess;
-  {
-    double* base = nullptr;
-    rc = hf_scratch(h, 8 * n1 + 14 * chunk + 2, &base);
-    if (rc != NO_OK) return rc;
-    d_nodes[0] = base; d_nodes[1] = base + 4 * n1; d_cfg = base + 8 * n1; d_w = d_cfg + 9 * chunk;
-    d_diag = d_w + chunk; d_acc = d_diag + 4 * chunk;
-  }
-  auto cleanup = [&]() {};
-#define NO_HF_CUDA(call) do { e = (call); if (e != cudaSuccess) { rc = cuda_fail(e, #call); cleanup(); return rc; } } while (0)
+  double* base = nullptr;
+  int rc = hf_scratch(h, 8 * n1 + 14 * chunk + 2, &base);
+  if (rc != NO_OK) return rc;
+  double* d_nodes[2] = {base, fused ? base : base + 4 * n1};
+  double *d_cfg = base + 8 * n1, *d_w = d_cfg + 9 * chunk, *d_diag = d_w + chunk, *d_acc = d_diag + 4 * chunk;
   for (int t = 0; t < 2; ++t)
-    if (kf[t] > 0)
-      NO_HF_CUDA(cudaMemcpyAsync(d_nodes[t], nodes[t].data(), sizeof(double) * 4 * (size_t)n1, cudaMemcpyHostToDevice, s));
-  NO_HF_CUDA(cudaMemsetAsync(d_acc, 0, sizeof(double), s));
+    if (!nodes[t].empty())
+      NO_CUDA(cudaMemcpyAsync(d_nodes[t], nodes[t].data(), sizeof(double) * 4 * (size_t)n1, cudaMemcpyHostToDevice, s));
+  NO_CUDA(cudaMemsetAsync(d_acc, 0, sizeof(double), s));
   for (int t1 = 0; t1 < 2; ++t1)
     for (int t2 = 0; t2 < 2; ++t2) {
       if (!(kf[t1] > 0) || !(kf[t2] > 0)) continue;
+      if (fused && (t1 || t2)) continue;
       for (long long c0 = 0; c0 < n1 * n1; c0 += chunk) {
         const long long count = n1 * n1 - c0 < chunk ? n1 * n1 - c0 : chunk;
         hf_pairs_kernel<<<(unsigned)((count + 255) / 256), 256, 0, s>>>(d_nodes[t1], d_nodes[t2], n1, c0, count, d_cfg, d_w);
-        NO_HF_CUDA(cudaGetLastError());
-        rc = launch(h, d_cfg, count, d_diag, s, kModeDiag, true);   // p' = p by construction
-        if (rc != NO_OK) { cleanup(); return rc; }
-        hf_reduce_kernel<<<1, 1024, 0, s>>>(d_diag, d_w, count, 2 * t1 + t2, d_acc);
-        NO_HF_CUDA(cudaGetLastError());
+        NO_CUDA(cudaGetLastError());
+        rc = launch(h, d_cfg, count, d_diag, s, layout, kModeDiag, true);   // p' = p by construction
+        if (rc != NO_OK) return rc;
+        hf_reduce_kernel<<<1, 1024, 0, s>>>(d_diag, d_w, count, fused ? -1 : 2 * t1 + t2, d_acc);
+        NO_CUDA(cudaGetLastError());
       }
     }
   double acc = 0.0;
-  NO_HF_CUDA(cudaMemcpyAsync(&acc, d_acc, sizeof(double), cudaMemcpyDeviceToHost, s));
-  NO_HF_CUDA(cudaStreamSynchronize(s));
-#undef NO_HF_CUDA
-  cleanup();
+  NO_CUDA(cudaMemcpyAsync(&acc, d_acc, sizeof(double), cudaMemcpyDeviceToHost, s));
+  NO_CUDA(cudaStreamSynchronize(s));
   *e_over_v = acc / 6.0;
   return NO_OK;
 }
@@ -283,59 +308,86 @@ int no_sp_energy(no_handle* h, const double* h_k1, int n_k, int n_r, int n_cos, 
   if (n_k == 0) return NO_OK;
   if (!h_k1 || !h_sigma) return NO_ERR_INVALID;
   if (n_r < 1 || n_r > kMaxOrder || n_cos < 1 || n_cos > kMaxOrder || n_phi < 1 || n_phi > kMaxOrder) return NO_ERR_INVALID;
+  BusyGuard busy(h);
+  if (!busy.ok) return NO_ERR_INVALID;
   DeviceGuard guard(h->device);
   if (!guard.ok) return cuda_fail(cudaGetLastError(), "cudaSetDevice");
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  const int layout = h->layout.load(std::memory_order_relaxed) == 2 ? 2 : 1;
   const double kf[2] = {h->plan.kf_p, h->plan.kf_n};
+  const bool fused = kf[0] > 0 && kf[0] == kf[1];   // one particle-2 grid serves both species (see no_hf_energy)
   const long long n2 = (long long)n_r * n_cos * n_phi;
   const long long rows_chunk = (1LL << 20) / n2 > 0 ? ((1LL << 20) / n2 < n_k ? (1LL << 20) / n2 : n_k) : 1;
-  std::vector<double> k1w(4 * (size_t)n_k), nodes2;
+  std::vector<double> k1w(4 * (size_t)n_k), nodes2[2];
   for (int i = 0; i < n_k; ++i) {
     for (int a = 0; a < 3; ++a) k1w[4 * i + a] = h_k1[3 * i + a];
     k1w[4 * i + 3] = 1.0;                              // particle 1 is not summed: unit weight
   }
-  double *d_k1 = nullptr, *d_nodes2 = nullptr, *d_cfg = nullptr, *d_w = nullptr, *d_diag = nullptr, *d_sigma = nullptr;
-  int rc = NO_OK;
-  cudaError_t e = cudaSuccess;
-  {
-    double* base = nullptr;
-    const long long pairs = rows_chunk * n2;
-    rc = hf_scratch(h, 4LL * n_k + 4 * n2 + 14 * pairs + 2LL * n_k, &base);
-    if (rc != NO_OK) return rc;
-    d_k1 = base; d_nodes2 = d_k1 + 4LL * n_k; d_cfg = d_nodes2 + 4 * n2; d_w = d_cfg + 9 * pairs;
-    d_diag = d_w + pairs; d_sigma = d_diag + 4 * pairs;
-  }
-  auto cleanup = [&]() {};
-#define NO_SP_CUDA(call) do { e = (call); if (e != cudaSuccess) { rc = cuda_fail(e, #call); cleanup(); return rc; } } while (0)
-  NO_SP_CUDA(cudaMemcpyAsync(d_k1, k1w.data(), sizeof(double) * 4 * (size_t)n_k, cudaMemcpyHostToDevice, s));
-  NO_SP_CUDA(cudaMemsetAsync(d_sigma, 0, sizeof(double) * 2 * (size_t)n_k, s));
+  const long long pairs = rows_chunk * n2;
+  double* base = nullptr;
+  int rc = hf_scratch(h, 4LL * n_k + 8 * n2 + 14 * pairs + 2LL * n_k, &base);
+  if (rc != NO_OK) return rc;
+  double* d_k1 = base;
+  double* d_nodes2[2] = {d_k1 + 4LL * n_k, d_k1 + 4LL * n_k + 4 * n2};
+  double *d_cfg = d_nodes2[1] + 4 * n2, *d_w = d_cfg + 9 * pairs, *d_diag = d_w + pairs, *d_sigma = d_diag + 4 * pairs;
+  NO_CUDA(cudaMemcpyAsync(d_k1, k1w.data(), sizeof(double) * 4 * (size_t)n_k, cudaMemcpyHostToDevice, s));
+  NO_CUDA(cudaMemsetAsync(d_sigma, 0, sizeof(double) * 2 * (size_t)n_k, s));
   for (int t2 = 0; t2 < 2; ++t2) {
-    if (!(kf[t2] > 0)) continue;
-    sphere_nodes(n_r, n_cos, n_phi, kf[t2], nodes2);
-    NO_SP_CUDA(cudaMemcpyAsync(d_nodes2, nodes2.data(), sizeof(double) * 4 * (size_t)n2, cudaMemcpyHostToDevice, s));
+    if (!(kf[t2] > 0) || (fused && t2 == 1)) continue;
+    sphere_nodes(n_r, n_cos, n_phi, kf[t2], nodes2[t2]);   // each species keeps its own host and device copy
+    NO_CUDA(cudaMemcpyAsync(d_nodes2[t2], nodes2[t2].data(), sizeof(double) * 4 * (size_t)n2, cudaMemcpyHostToDevice, s));
     for (long long r0 = 0; r0 < n_k; r0 += rows_chunk) {
       const long long rows = n_k - r0 < rows_chunk ? n_k - r0 : rows_chunk, count = rows * n2;
-      hf_pairs_kernel<<<(unsigned)((count + 255) / 256), 256, 0, s>>>(d_k1, d_nodes2, n2, r0 * n2, count, d_cfg, d_w);
-      NO_SP_CUDA(cudaGetLastError());
-      rc = launch(h, d_cfg, count, d_diag, s, kModeDiag, true);   // p' = p by construction
-      if (rc != NO_OK) { cleanup(); return rc; }
+      hf_pairs_kernel<<<(unsigned)((count + 255) / 256), 256, 0, s>>>(d_k1, d_nodes2[t2], n2, r0 * n2, count, d_cfg, d_w);
+      NO_CUDA(cudaGetLastError());
+      rc = launch(h, d_cfg, count, d_diag, s, layout, kModeDiag, true);   // p' = p by construction
+      if (rc != NO_OK) return rc;
       // (1/2) from xi = 1/2 of Eq. (10), (1/2) from averaging the spin of particle 1 out of the traced diagonal
-      sp_reduce_kernel<<<(unsigned)rows, 256, 0, s>>>(d_diag, d_w, n2, t2, 0.25, r0, d_sigma);
-      NO_SP_CUDA(cudaGetLastError());
+      sp_reduce_kernel<<<(unsigned)rows, 256, 0, s>>>(d_diag, d_w, n2, fused ? -1 : t2, 0.25, r0, d_sigma);
+      NO_CUDA(cudaGetLastError());
     }
-    NO_SP_CUDA(cudaStreamSynchronize(s));             // nodes2 (host) is rebuilt for the next species
   }
-  NO_SP_CUDA(cudaMemcpyAsync(h_sigma, d_sigma, sizeof(double) * 2 * (size_t)n_k, cudaMemcpyDeviceToHost, s));
-  NO_SP_CUDA(cudaStreamSynchronize(s));
-#undef NO_SP_CUDA
-  cleanup();
+  NO_CUDA(cudaMemcpyAsync(h_sigma, d_sigma, sizeof(double) * 2 * (size_t)n_k, cudaMemcpyDeviceToHost, s));
+  NO_CUDA(cudaStreamSynchronize(s));
   return NO_OK;
 }
+
+namespace {
+
+// body of no_eval_host after the scratch is in place; any failure is reported after the copy stream has drained
+int host_path(no_handle* h, const double* h_cfg, long long n_cfg, double* h_out, cudaStream_t s) {
+  NO_CUDA(cudaMemcpyAsync(h->d_cfg, h_cfg, sizeof(double) * 9 * (size_t)n_cfg, cudaMemcpyHostToDevice, s));
+  // chunks of whole waves of resident CTAs (about n/8, at most ~64 Ki configurations): the copy of chunk k
+  // (copy stream) runs under the kernel of chunk k + 1 (caller's stream).  One layout for the whole call.
+  const int layout = resolve_layout(h, n_cfg);
+  long long waves = n_cfg / 8 / h->wave_cfg;
+  if (waves < 1) waves = 1;
+  if (waves * h->wave_cfg > 65536) waves = 65536 / h->wave_cfg > 0 ? 65536 / h->wave_cfg : 1;
+  const long long chunk = waves * h->wave_cfg;
+  int k = 0;
+  for (long long c0 = 0; c0 < n_cfg; c0 += chunk, ++k) {
+    const long long cnt = n_cfg - c0 < chunk ? n_cfg - c0 : chunk;
+    const int rc = launch(h, h->d_cfg + 9 * c0, cnt, h->d_out + 512 * c0, s, layout);
+    if (rc != NO_OK) return rc;
+    NO_CUDA(cudaEventRecord(h->ev_chunk[k & 1], s));
+    NO_CUDA(cudaStreamWaitEvent(h->copy_stream, h->ev_chunk[k & 1], 0));
+    NO_CUDA(cudaMemcpyAsync(h_out + 512 * c0, h->d_out + 512 * c0, sizeof(double) * 512 * (size_t)cnt,
+                            cudaMemcpyDeviceToHost, h->copy_stream));
+  }
+  NO_CUDA(cudaEventRecord(h->ev_copied, h->copy_stream));
+  NO_CUDA(cudaStreamWaitEvent(s, h->ev_copied, 0));
+  NO_CUDA(cudaStreamSynchronize(s));
+  return NO_OK;
+}
+
+}  // namespace
 
 int no_eval_host(no_handle* h, const double* h_cfg, long long n_cfg, double* h_out, void* cuda_stream) {
   if (!h || n_cfg < 0) return NO_ERR_INVALID;
   if (n_cfg == 0) return NO_OK;
   if (!h_cfg || !h_out) return NO_ERR_INVALID;
+  BusyGuard busy(h);
+  if (!busy.ok) return NO_ERR_INVALID;
   DeviceGuard guard(h->device);
   if (!guard.ok) return cuda_fail(cudaGetLastError(), "cudaSetDevice");
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
@@ -352,32 +404,25 @@ int no_eval_host(no_handle* h, const double* h_cfg, long long n_cfg, double* h_o
   }
   if (!h->host_path_ready) {
     NO_CUDA(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
-    NO_CUDA(cudaEventCreateWithFlags(&h->ev_chunk[0], cudaEventDisableTiming));
-    NO_CUDA(cudaEventCreateWithFlags(&h->ev_chunk[1], cudaEventDisableTiming));
-    NO_CUDA(cudaEventCreateWithFlags(&h->ev_copied, cudaEventDisableTiming));
+    cudaError_t e = cudaEventCreateWithFlags(&h->ev_chunk[0], cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_chunk[1], cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_copied, cudaEventDisableTiming);
+    if (e != cudaSuccess) {
+      // cudaEventDestroy of a never-created (zero) event only returns an error code: nothing leaks
+      cudaEventDestroy(h->ev_chunk[0]); cudaEventDestroy(h->ev_chunk[1]); cudaEventDestroy(h->ev_copied);
+      cudaStreamDestroy(h->copy_stream);
+      h->ev_chunk[0] = h->ev_chunk[1] = h->ev_copied = nullptr;
+      return cuda_fail(e, "cudaEventCreateWithFlags");
+    }
     h->host_path_ready = true;
   }
-  NO_CUDA(cudaMemcpyAsync(h->d_cfg, h_cfg, sizeof(double) * 9 * (size_t)n_cfg, cudaMemcpyHostToDevice, s));
-  // chunks of whole waves of resident CTAs (about n/8, at most ~64 Ki configurations): the copy of chunk k
-  // (copy stream) runs under the kernel of chunk k + 1 (caller's stream)
-  long long waves = n_cfg / 8 / h->wave_cfg;
-  if (waves < 1) waves = 1;
-  if (waves * h->wave_cfg > 65536) waves = 65536 / h->wave_cfg > 0 ? 65536 / h->wave_cfg : 1;
-  const long long chunk = waves * h->wave_cfg;
-  int k = 0;
-  for (long long c0 = 0; c0 < n_cfg; c0 += chunk, ++k) {
-    const long long cnt = n_cfg - c0 < chunk ? n_cfg - c0 : chunk;
-    const int rc = launch(h, h->d_cfg + 9 * c0, cnt, h->d_out + 512 * c0, s);
-    if (rc != NO_OK) return rc;
-    NO_CUDA(cudaEventRecord(h->ev_chunk[k & 1], s));
-    NO_CUDA(cudaStreamWaitEvent(h->copy_stream, h->ev_chunk[k & 1], 0));
-    NO_CUDA(cudaMemcpyAsync(h_out + 512 * c0, h->d_out + 512 * c0, sizeof(double) * 512 * (size_t)cnt,
-                            cudaMemcpyDeviceToHost, h->copy_stream));
+  const int rc = host_path(h, h_cfg, n_cfg, h_out, s);
+  if (rc != NO_OK) {
+    // nothing of this call may still be writing into the caller's buffers or the scratch when it returns
+    cudaStreamSynchronize(h->copy_stream);
+    cudaStreamSynchronize(s);
   }
-  NO_CUDA(cudaEventRecord(h->ev_copied, h->copy_stream));
-  NO_CUDA(cudaStreamWaitEvent(s, h->ev_copied, 0));
-  NO_CUDA(cudaStreamSynchronize(s));
-  return NO_OK;
+  return rc;
 }
 
 int no_free(no_handle* h) {
@@ -442,21 +487,30 @@ int no_probe_fp64_peak(int device, int millis, double* tflops, int* n_sm, void* 
   int sms = 0;
   NO_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device));
   const int threads = 256, blocks = sms * 8;
-  double* sink = nullptr;
-  NO_CUDA(cudaMalloc((void**)&sink, sizeof(double) * threads * blocks));
-  cudaEvent_t e0, e1;
-  NO_CUDA(cudaEventCreate(&e0));
-  NO_CUDA(cudaEventCreate(&e1));
+  // everything the probe allocates is released on every exit
+  struct Res {
+    double* sink = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    ~Res() {
+      if (e0) cudaEventDestroy(e0);
+      if (e1) cudaEventDestroy(e1);
+      if (sink) cudaFree(sink);
+    }
+  } r;
+  NO_CUDA(cudaMalloc((void**)&r.sink, sizeof(double) * threads * blocks));
+  NO_CUDA(cudaEventCreate(&r.e0));
+  NO_CUDA(cudaEventCreate(&r.e1));
   int iters = 1 << 12;
   double best = 0.0;
   float ms = 0.f;
   // grow the launch until it lasts about `millis`, keep the best rate of the long launches
   for (int rep = 0; rep < 24; ++rep) {
-    NO_CUDA(cudaEventRecord(e0, s));
-    dfma_probe_kernel<<<blocks, threads, 0, s>>>(sink, iters, 1.0);
-    NO_CUDA(cudaEventRecord(e1, s));
-    NO_CUDA(cudaEventSynchronize(e1));
-    NO_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+    NO_CUDA(cudaEventRecord(r.e0, s));
+    dfma_probe_kernel<<<blocks, threads, 0, s>>>(r.sink, iters, 1.0);
+    NO_CUDA(cudaGetLastError());
+    NO_CUDA(cudaEventRecord(r.e1, s));
+    NO_CUDA(cudaEventSynchronize(r.e1));
+    NO_CUDA(cudaEventElapsedTime(&ms, r.e0, r.e1));
     const double flops = 2.0 * 16.0 * (double)iters * threads * (double)blocks;
     const double rate = flops / (ms * 1e-3) * 1e-12;
     if (ms >= 0.5f * millis) {
@@ -465,10 +519,6 @@ int no_probe_fp64_peak(int device, int millis, double* tflops, int* n_sm, void* 
     }
     if (ms < (float)millis && iters < (1 << 28)) iters *= 2;
   }
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
-  cudaFree(sink);
-  NO_CUDA(cudaGetLastError());
   *tflops = best;
   if (n_sm) *n_sm = sms;
   return NO_OK;

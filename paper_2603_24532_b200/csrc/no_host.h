@@ -117,6 +117,12 @@ inline int build_plan(const no_params* p, HostPlan& plan, const double* dirs = n
   if (dirs) {
     if (n_dir < 1 || n_dir > kMaxList) return NO_ERR_INVALID;
     for (int i = 0; i < 4 * n_dir; ++i) if (!std::isfinite(dirs[i])) return NO_ERR_INVALID;
+    // the kernel uses |u| = 1 (D_l = r^2 + bet_l r + gam_l, and the bound on |k3 - P/2| that elides the
+    // underflow guard of the regulator): a direction that is not a unit vector is refused, not renormalised
+    for (int i = 0; i < n_dir; ++i) {
+      const double* u = dirs + 4 * i;
+      if (std::fabs(u[0] * u[0] + u[1] * u[1] + u[2] * u[2] - 1.0) > 1e-12) return NO_ERR_INVALID;
+    }
   }
   const bool regulated = p->Lambda > 0;
   if (regulated && (p->n_reg < 1 || p->n_reg > kMaxRegPoly)) return NO_ERR_INVALID;

@@ -280,7 +280,8 @@ __global__ void hf_pairs_kernel(const double* __restrict__ nodes1, const double*
 }
 
 // sigma[(row0 + i1) 2 + t1] += scale sum_{i2 < n2} w[i1 n2 + i2] diag[i1 n2 + i2][2 t1 + t2], t1 = 0, 1: one CTA per
-// momentum k1 (row i1 of the chunk), fixed summation order
+// momentum k1 (row i1 of the chunk), fixed summation order.  t2 < 0: both species of particle 2 share this grid
+// (equal Fermi momenta), their two columns are added
 __global__ void __launch_bounds__(256) sp_reduce_kernel(const double* __restrict__ diag, const double* __restrict__ w,
                                                         long long n2, int t2, double scale, long long row0,
                                                         double* __restrict__ sigma) {
@@ -289,8 +290,9 @@ __global__ void __launch_bounds__(256) sp_reduce_kernel(const double* __restrict
   double s0 = 0.0, s1 = 0.0;
   for (long long i2 = threadIdx.x; i2 < n2; i2 += 256) {
     const double wv = w[base + i2];
-    s0 = fma(wv, diag[4 * (base + i2) + t2], s0);
-    s1 = fma(wv, diag[4 * (base + i2) + 2 + t2], s1);
+    const double* d = diag + 4 * (base + i2);
+    s0 = fma(wv, t2 < 0 ? d[0] + d[1] : d[t2], s0);
+    s1 = fma(wv, t2 < 0 ? d[2] + d[3] : d[2 + t2], s1);
   }
   sh[0][threadIdx.x] = s0;
   sh[1][threadIdx.x] = s1;
@@ -305,12 +307,16 @@ __global__ void __launch_bounds__(256) sp_reduce_kernel(const double* __restrict
   if (threadIdx.x < 2) sigma[2 * (row0 + blockIdx.x) + threadIdx.x] += scale * sh[threadIdx.x][0];
 }
 
-// acc[0] += sum_c w[c] diag[c][blk], one CTA, fixed summation order (bit reproducible)
+// acc[0] += sum_c w[c] diag[c][blk], one CTA, fixed summation order (bit reproducible); blk < 0: the four isospin
+// pairs share this pair grid (equal Fermi momenta) and their columns are added
 __global__ void __launch_bounds__(1024) hf_reduce_kernel(const double* __restrict__ diag, const double* __restrict__ w,
                                                          long long count, int blk, double* __restrict__ acc) {
   __shared__ double sh[1024];
   double s = 0.0;
-  for (long long c = threadIdx.x; c < count; c += 1024) s = fma(w[c], diag[4 * c + blk], s);
+  for (long long c = threadIdx.x; c < count; c += 1024) {
+    const double* d = diag + 4 * c;
+    s = fma(w[c], blk < 0 ? (d[0] + d[1]) + (d[2] + d[3]) : d[blk], s);
+  }
   sh[threadIdx.x] = s;
   __syncthreads();
   for (int half = 512; half > 0; half >>= 1) {

@@ -213,3 +213,21 @@ def test_seeded_configurations_are_reproducible_and_in_range():
     d = W.splitmix64_doubles(0, 0, 0, 5)
     assert np.array_equal(d, W.splitmix64_doubles(0, 0, 0, 8)[:5]) and (0 <= d).all() and (d < 1).all()
     assert np.array_equal(W.splitmix64_doubles(0, 0, 3, 2), W.splitmix64_doubles(0, 0, 0, 8)[3:5])
+
+
+def test_angular_rule_with_non_unit_directions_is_refused():
+    """The kernel relies on |u| = 1 (propagator polynomial in r, bound that elides the underflow guard):
+    build_plan refuses a rule whose directions are not unit vectors instead of silently renormalising."""
+    from paper_2603_24532_b200 import angular_rules as A
+    kw = dict(PHYS, kf_n=1.2, kf_p=0.9, n_r=3)
+    cfg = W.momentum_configurations(1, 0, 2, 1.5, 2.0)
+    dirs = A.octahedral_rule(5)
+    emu.emu_eval_angular(cfg, dirs, **kw)                       # accepted as generated
+    bad = dirs.copy()
+    bad[3, :3] *= 1.0 + 1e-9
+    with pytest.raises(ValueError):
+        emu.emu_eval_angular(cfg, bad, **kw)
+    bad = dirs.copy()
+    bad[0, :3] = 0.0
+    with pytest.raises(ValueError):
+        emu.emu_eval_angular(cfg, bad, **kw)

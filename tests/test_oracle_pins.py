@@ -107,6 +107,43 @@ def test_operator_hand_evaluated_elements():
     assert np.abs(V).max() > 1e-3
 
 
+def test_c4_term_sign_and_size_by_hand():
+    """The c4 part of the two-pion exchange (reading R1),
+        1/2 (gA/2f)^2 c4/f^2 sum_{ijk} (s_i.q_i)(s_j.q_j)/(D_i D_j) (t_i x t_j).t_k s_k.(q_i x q_j),
+    at q1 = (a,0,0), q2 = (0,b,0), q3 = 0: only (i,j,k) = (1,2,3) and (2,1,3) survive and are equal, so
+        V = (gA/2f)^2 c4/f^2 a b/(D1 D2) [s_1x s_2y (a b s_3z)] [(t_1 x t_2).t_3].
+    Every factor is a number between product states:
+        <dn dn s3| s_1x s_2y s_3z |up up s3> = (1)(i)(+1 for s3 = up, -1 for s3 = down),
+        <n p p| (t_1 x t_2).t_3 |p n p> = <n p|t_1x t_2y - t_1y t_2x|p n> <p|t_3z|p> = (1)(-i) - (i)(1) = -2i
+        (and +2i with a spectator neutron, <n|t_3z|n> = -1),
+    so the element is + 2 (gA/2f)^2 (c4/f^2) a^2 b^2 / (D1 D2) for (s3 up, t3 proton): fixes the sign, the
+    factor 1/2 (gA/2f)^2 c4/f^2 and the Levi-Civita isospin factor of the term, none of which P3/P5/P10 see."""
+    a, b = 0.9, -0.6
+    q = np.array([[a, 0, 0], [0, b, 0], [0, 0, 0]])
+    m, f = PHYS["mpi"] / HBARC, PHYS["fpi"] / HBARC
+    c4 = 5.4e-3 * HBARC
+    D1, D2 = a * a + m * m, b * b + m * m
+    want = 2 * (PHYS["gA"] / (2 * f)) ** 2 * c4 / f ** 2 * a * a * b * b / (D1 * D2)
+    V = O.v3n(q, **only(c4=5.4))
+
+    def idx(s, t):                                         # s, t = (b1, b2, b3); 64-dim index = 8 spin + isospin
+        return 8 * (4 * s[0] + 2 * s[1] + s[2]) + 4 * t[0] + 2 * t[1] + t[2]
+
+    assert want > 0.01
+    for s3, t3, sign in ((0, 0, +1), (1, 0, -1), (0, 1, -1), (1, 1, +1)):
+        got = V[idx((1, 1, s3), (1, 0, t3)), idx((0, 0, s3), (0, 1, t3))]
+        assert got.real == pytest.approx(sign * want, rel=1e-14) and abs(got.imag) < 1e-16 * want
+    # the reverse isospin exchange |n p> -> |p n> has the opposite sign ((t_1 x t_2)_z is antisymmetric)
+    got = V[idx((1, 1, 0), (0, 1, 0)), idx((0, 0, 0), (1, 0, 0))]
+    assert got.real == pytest.approx(-want, rel=1e-14)
+    # spectator spin or isospin changed, or the pair's isospin unchanged: no contribution from this topology
+    assert abs(V[idx((1, 1, 1), (1, 0, 0)), idx((0, 0, 0), (0, 1, 0))]) < 1e-16 * want
+    assert abs(V[idx((1, 1, 0), (0, 1, 0)), idx((0, 0, 0), (0, 1, 0))]) < 1e-16 * want
+    # linear in c4, and nothing else of the operator is switched on by it
+    V2 = O.v3n(q, **only(c4=-2.7))
+    assert np.abs(V2 + 0.5 * V).max() < 1e-15 * np.abs(V).max()
+
+
 def _perm_matrix64(pi):
     """<b'|Pi_pi|b> = prod_m delta(b'_{pi(m)}, b_m) on spin (x) isospin of three particles."""
     P8 = np.zeros((8, 8))
@@ -382,7 +419,8 @@ def test_P8_hartree_fock_identity(geo):
 
 
 # ----------------------------------------------------------------------------------------------
-# P12: values of an independent transcription -- a third opinion.
+# P12: values of an independent transcription -- a third opinion; regenerable
+# with tests/golden/make_survey_appendix_a.py.
 # ----------------------------------------------------------------------------------------------
 def test_P12_cross_implementation_values():
     path = os.path.join(os.path.dirname(__file__), "golden", "survey_appendix_a.txt")
@@ -401,6 +439,47 @@ def test_P12_cross_implementation_values():
                 assert np.abs(M).max() == pytest.approx(re, rel=1e-13)
             else:
                 assert abs(M[r, c] - complex(re, im)) < 1e-14
+
+
+def test_P12_golden_file_is_regenerable_by_the_committed_numpy_transcription():
+    """tests/golden/make_survey_appendix_a.py (numpy only; imports neither oracle/ nor the product package)
+    reproduces every stored value: the golden file is the output of a committed, independent script."""
+    import subprocess
+    import sys
+    here = os.path.dirname(__file__)
+    script = os.path.join(here, "golden", "make_survey_appendix_a.py")
+    import ast
+    mods = set()
+    for node in ast.walk(ast.parse(open(script).read())):
+        if isinstance(node, ast.Import):
+            mods.update(a.name.split(".")[0] for a in node.names)
+        elif isinstance(node, ast.ImportFrom):
+            mods.add((node.module or "").split(".")[0])
+    assert mods <= {"itertools", "os", "sys", "numpy"}, mods
+    out = subprocess.run([sys.executable, script], check=True, capture_output=True, text=True).stdout
+
+    def rows(text):
+        return np.array([[float(x) for x in l.split()] for l in text.splitlines() if l.strip() and not l.startswith("#")])
+
+    got, want = rows(out), rows(open(os.path.join(here, "golden", "survey_appendix_a.txt")).read())
+    assert got.shape == want.shape == (22, 5)
+    assert np.array_equal(got[:, :3], want[:, :3])
+    assert np.abs(got[:, 3:] - want[:, 3:]).max() < 1e-13
+
+
+def test_oracle_runs_clean_under_address_and_undefined_behaviour_sanitizers(tmp_path):
+    """the oracle, built with -fsanitize=address,undefined (tests/oracle_sanitize_main.cpp
+    includes oracle/no_oracle.cpp verbatim), runs P11 on a 2^3 grid, the direction-list path, the double
+    instantiation and the brute-force Hartree-Fock sum without a report."""
+    import subprocess
+    here = os.path.dirname(__file__)
+    exe = str(tmp_path / "oracle_sanitized")
+    subprocess.run(["g++", "-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=all",
+                    "-fno-omit-frame-pointer", "-o", exe, os.path.join(here, "oracle_sanitize_main.cpp")], check=True)
+    r = subprocess.run([exe], capture_output=True, text=True, env=dict(os.environ, ASAN_OPTIONS="detect_leaks=1"))
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert "runtime error" not in r.stderr and "AddressSanitizer" not in r.stderr and "LeakSanitizer" not in r.stderr
+    assert "level0-level1" in r.stdout
 
 
 # ----------------------------------------------------------------------------------------------

@@ -88,7 +88,7 @@ def test_cfg1_all_configurations():
     print(f"cfg1: 256 configurations, max rel err {worst:.2e}")
 
 
-FULL_SIZE = [("cfg2", 16), ("cfg3", 32), ("cfg4", 8), ("cfg5", 2), ("paper", 64)]
+FULL_SIZE = [("cfg2", 16), ("cfg3", 32), ("cfg4", 16), ("cfg5", 8), ("paper", 64)]
 
 
 @pytest.mark.parametrize("name,n_sample", FULL_SIZE)
@@ -301,6 +301,62 @@ def test_abi_pointer_checks_streams_and_host_path():
     check_parity(torch.view_as_complex(ref).cpu().numpy(), O.normal_order(cfg, **run.params()), "streams")
     with pytest.raises(binding.NoError):
         binding.no_init(device=99, **run.params())
+
+
+def test_batches_larger_than_one_grid_are_cut_into_several_launches(monkeypatch):
+    """A batch that needs more CTAs than gridDim.x allows is chunked, not refused.  The limit (2^31 - 1 CTAs)
+    cannot be reached in a test, so the testing knob NO3N_MAX_GRID lowers it: same bits as one launch."""
+    run = W.workload("cfg4").runs[0].shrunk(37, 6)
+    cfg = torch.from_numpy(run.configurations()).cuda()
+    ref = {}
+    for layout in (1, 2):
+        no = NormalOrdering(device=0, layout=layout, **run.params())
+        ref[layout] = no(cfg).cpu().numpy()
+        ref[layout, "diag"] = no.diag(cfg).cpu().numpy()
+        no.close()
+    monkeypatch.setenv("NO3N_MAX_GRID", "3")
+    for layout in (1, 2):
+        no = NormalOrdering(device=0, layout=layout, **run.params())          # 37 configurations: 7 or 13 launches
+        assert np.array_equal(no(cfg).cpu().numpy(), ref[layout])
+        assert np.array_equal(no.diag(cfg).cpu().numpy(), ref[layout, "diag"])
+        h_out = np.empty((37, 16, 16, 2))
+        binding.no_eval_host(no._h, run.configurations().ctypes.data, 37, h_out.ctypes.data, None)
+        assert np.array_equal(h_out[..., 0] + 1j * h_out[..., 1], ref[layout])
+        no.close()
+
+
+def test_host_path_uses_one_layout_per_call_and_refuses_concurrent_use():
+    """no_eval_host decides the kernel layout once per call from the whole batch (a small tail chunk does not
+    switch to the small-batch layout), and a second concurrent call on the same handle is refused."""
+    import threading
+    run = W.workload("cfg1").runs[0].shrunk(4000, 6)             # chunked: waves of 1776 configurations + a tail
+    cfg = run.configurations()
+    h = binding.no_init(device=0, **run.params())
+    d_out = torch.empty((4000, 16, 16, 2), dtype=torch.float64, device="cuda")
+    binding.no_set_layout(h, 1)
+    binding.no_eval(h, torch.from_numpy(cfg).cuda().data_ptr(), 4000, d_out.data_ptr(), None)
+    torch.cuda.synchronize()
+    binding.no_set_layout(h, 0)
+    h_out = torch.empty((4000, 16, 16, 2), dtype=torch.float64, pin_memory=True)
+    binding.no_eval_host(h, cfg.ctypes.data, 4000, h_out.data_ptr(), None)
+    assert torch.equal(h_out, d_out.cpu())                       # tail included: bit-identical to the one-warp layout
+    # two threads on one handle: every call either succeeds with the right bits or is refused with NO_ERR_INVALID
+    lib, results = binding.load(), []
+    outs = [torch.empty((4000, 16, 16, 2), dtype=torch.float64, pin_memory=True) for _ in range(2)]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+
+    def work(i):
+        for _ in range(20):
+            rc = lib.no_eval_host(h, ctypes.c_void_p(cfg.ctypes.data), 4000, ctypes.c_void_p(outs[i].data_ptr()),
+                                  ctypes.c_void_p(streams[i].cuda_stream))
+            results.append((rc, rc != 0 or bool(torch.equal(outs[i], h_out))))
+
+    th = [threading.Thread(target=work, args=(i,)) for i in range(2)]
+    [t.start() for t in th]
+    [t.join() for t in th]
+    assert all(rc in (binding.NO_OK, binding.NO_ERR_INVALID) and good for rc, good in results)
+    assert any(rc == binding.NO_OK for rc, _ in results)
+    binding.no_free(h)
 
 
 def test_handles_with_different_shared_memory_sizes_coexist():
