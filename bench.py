@@ -284,13 +284,26 @@ def run_b200(args, workload):
     n_launch = len(runs) * args.steps
 
     # ---- end to end through the C ABI with HOST buffers (H2D + D2H inside the timed region) ----
-    e2e = None
-    if not args.no_e2e:
-        h_out = [torch.empty((r.n_cfg, 16, 16, 2), dtype=torch.float64, pin_memory=True) for r in runs]
+    # e2e: no_eval_host_packed, the symmetry-reduced form the paper describes (isospin form for runs
+    # with kF_n = kF_p, charge-conserving form otherwise; the full matrix follows by an index map, no_unpack);
+    # e2e_full_matrices: no_eval_host, all 256 entries of every matrix over PCIe.
+    def e2e_leg(packed: bool):
+        fmts = []
+        for h in handles:
+            if not packed:
+                fmts.append((0, 512))
+            elif binding.no_packed_doubles(h, binding.NO_PACK_ISOSPIN):
+                fmts.append((binding.NO_PACK_ISOSPIN, binding.no_packed_doubles(h, binding.NO_PACK_ISOSPIN)))
+            else:
+                fmts.append((binding.NO_PACK_CHARGE, binding.no_packed_doubles(h, binding.NO_PACK_CHARGE)))
+        h_out = [torch.empty((r.n_cfg, pd), dtype=torch.float64, pin_memory=True) for r, (_, pd) in zip(runs, fmts)]
 
         def step_host():
-            for h, c, o, r in zip(handles, dw.h_cfg, h_out, runs):
-                binding.no_eval_host(h, c.data_ptr(), r.n_cfg, o.data_ptr(), stream.cuda_stream)
+            for h, c, o, r, (fmt, _) in zip(handles, dw.h_cfg, h_out, runs, fmts):
+                if fmt:
+                    binding.no_eval_host_packed(h, fmt, c.data_ptr(), r.n_cfg, o.data_ptr(), stream.cuda_stream)
+                else:
+                    binding.no_eval_host(h, c.data_ptr(), r.n_cfg, o.data_ptr(), stream.cuda_stream)
 
         step_host()
         barrier()
@@ -301,12 +314,19 @@ def run_b200(args, workload):
         barrier()
         t_e2e = replicas.max_over_ranks((time.perf_counter() - t0) / k, dev)
         chk = float(h_out[0][0].abs().sum())          # the step's result is read on the host
-        e2e = {"value": world * evals_step / t_e2e, "unit": UNIT,
-               "h2d_bytes_per_step": int(sum(c.numel() * 8 for c in dw.h_cfg)),
-               "d2h_bytes_per_step": int(sum(o.numel() * 8 for o in h_out)),
-               "ms_per_step": t_e2e * 1e3, "steps": k, "checksum": chk,
-               "api": "no_eval_host (pinned host buffers; full 16x16 matrices)"}
-        del h_out
+        names = {0: "full 16x16", binding.NO_PACK_CHARGE: "NO_PACK_CHARGE (96 entries)",
+                 binding.NO_PACK_ISOSPIN: "NO_PACK_ISOSPIN (32 entries)"}
+        return {"value": world * evals_step / t_e2e, "unit": UNIT,
+                "h2d_bytes_per_step": int(sum(c.numel() * 8 for c in dw.h_cfg)),
+                "d2h_bytes_per_step": int(sum(o.numel() * 8 for o in h_out)),
+                "ms_per_step": t_e2e * 1e3, "steps": k, "checksum": chk,
+                "api": ("no_eval_host_packed" if packed else "no_eval_host") + " (pinned host buffers); result form per run: "
+                       + ", ".join(sorted({names[f] for f, _ in fmts}))}
+
+    e2e = e2e_full = None
+    if not args.no_e2e:
+        e2e = e2e_leg(True)
+        e2e_full = e2e_leg(False)
 
     # ---- roofline of the (single) kernel: FP64 ALU bound ----
     launch_ms = sum(step_ms) / n_launch
@@ -364,7 +384,7 @@ def run_b200(args, workload):
                        "l2": "256 MiB buffer rewritten between timed steps (L2 flush); the kernel is ALU bound",
                        "parallelism": "replicas only: every rank integrates the whole workload",
                        "per_config": per_config},
-            "clocks": clocks, "e2e": e2e, "gpu_launches": n_launch, "roofline": roofline, "cpu_baseline": cpu,
+            "clocks": clocks, "e2e": e2e, "e2e_full_matrices": e2e_full, "gpu_launches": n_launch, "roofline": roofline, "cpu_baseline": cpu,
             "wall_s_timed_region": t_wall}
     print(json.dumps(line), flush=True)
 

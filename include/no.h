@@ -107,6 +107,49 @@ int no_set_layout(no_handle *h, int layout);
  * streams are drained before the call returns.  Used for the end-to-end measurement. */
 int no_eval_host(no_handle *h, const double *h_cfg, long long n_cfg, double *h_out, void *cuda_stream);
 
+/* ---- Packed, symmetry-reduced output -------------------------------------------
+ * "only up to 4^A C(2A,A) matrix elements can be non-zero ... only a subset of the remaining matrix
+ * elements needs to be computed from which the entire matrix can be efficiently reconstructed."  For A = 2 that is
+ * 96 of the 256 entries (charge conservation, t1' + t2' = t1 + t2); in isospin-symmetric matter the isospin
+ * invariance of the effective interaction (it has the form A + B tau_1.tau_2) leaves 32.
+ * A packed matrix is indexed [spin element sp][entry][2] (re, im), sp = 4 (2 s1' + s2') + (2 s1 + s2), i.e. the
+ * full-matrix element is row = 8 s1' + 4 s2' + (row isospin pair), col = 8 s1 + 4 s2 + (column isospin pair),
+ * isospin pair = 2 t1 + t2 (pp = 0, pn = 1, np = 2, nn = 3):
+ *   NO_PACK_CHARGE  : 6 entries per spin element, (row pair, column pair) =
+ *                     (pp,pp) (pn,pn) (np,np) (nn,nn) (pn,np) (np,pn): 96 complex = 192 doubles = 1536 bytes;
+ *                     valid for every handle.
+ *   NO_PACK_ISOSPIN : 2 entries per spin element, (pn,pn) and (pn,np): 32 complex = 64 doubles = 512 bytes;
+ *                     only for handles with kF_n == kF_p > 0 (NO_ERR_INVALID otherwise).  Reconstruction:
+ *                     (np,np) = (pn,pn), (np,pn) = (pn,np), (pp,pp) = (nn,nn) = (pn,pn) + (pn,np).
+ * The packed kernels compute and store only the subset (the 160 structural zeros are neither computed nor written;
+ * in isospin-symmetric matter 64 more entries are skipped). */
+#define NO_PACK_CHARGE  1
+#define NO_PACK_ISOSPIN 2
+
+/* Doubles per configuration of a packed format for this handle: 192 or 64; 0 if the format does not apply
+ * to the handle (NO_PACK_ISOSPIN without kF_n == kF_p) or is unknown. */
+int no_packed_doubles(const no_handle *h, int format);
+
+/* no_eval writing the packed form.  Same arguments, ownership, alignment and asynchrony as no_eval, except
+ *   d_packed : DEVICE, [n_cfg][no_packed_doubles(h, format)] doubles, 16-byte aligned, dense, caller-owned.
+ * NO_ERR_INVALID if the format does not apply to the handle. */
+int no_eval_packed(const no_handle *h, int format, const double *d_cfg, long long n_cfg, double *d_packed,
+                   void *cuda_stream);
+
+/* Rebuild the full matrices from a packed form on the device (one kernel, enqueued on `cuda_stream`, no
+ * synchronisation; runs on the caller's current device, which must own both pointers):
+ *   d_packed : DEVICE, const, [n_cfg][192 or 64] doubles as written by no_eval_packed, 16-byte aligned
+ *   d_out    : DEVICE, [n_cfg][16][16][2] doubles as no_eval writes them, 16-byte aligned; every element is written.
+ * With NO_PACK_CHARGE the result equals no_eval's bit for bit; with NO_PACK_ISOSPIN the pp and nn blocks are the
+ * sum of the two stored entries (equal to no_eval's to rounding). */
+int no_unpack(int format, const double *d_packed, long long n_cfg, double *d_out, void *cuda_stream);
+
+/* no_eval_host shipping the packed form over PCIe: HOST buffers, h_packed [n_cfg][192 or 64] doubles; otherwise
+ * as no_eval_host (chunked, copies overlapped, synchronises, not re-entrant for one handle).  The device-to-host
+ * traffic per configuration drops from 4096 to 1536 or 512 bytes. */
+int no_eval_host_packed(no_handle *h, int format, const double *h_cfg, long long n_cfg, double *h_packed,
+                        void *cuda_stream);
+
 /* Spin-traced diagonal of the normal-ordered matrix, reduced inside the kernel (the 16x16 matrix is
  * never written): the integrand of the Hartree-Fock contractions Eq. (1) and Eq. (9),
  * obtained "by repeatedly normal ordering".  Same arguments as no_eval except

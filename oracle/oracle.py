@@ -196,6 +196,62 @@ def sp_energy(k1, n_r12: int, n_cos12: int, n_phi12: int, **params) -> np.ndarra
     return sig
 
 
+# ---- packed, symmetry-reduced form of the 16x16 matrix ----
+# "only up to 4^A C(2A,A) matrix elements can be non-zero ... only a subset of the remaining matrix elements
+# needs to be computed from which the entire matrix can be efficiently reconstructed."  The plain definitions
+# of the two subsets the library writes, element by element.
+#   format 1 ("charge"): the 96 = 4^2 C(4,2) entries with t1' + t2' = t1 + t2, as [16 spin elements][6 isospin blocks],
+#       spin element sp = 4 (2 s1' + s2') + (2 s1 + s2), isospin block nb -> (row pair, column pair), pair = 2 t1 + t2:
+#       (pp,pp) (pn,pn) (np,np) (nn,nn) (pn,np) (np,pn)
+#   format 2 ("isospin"): isospin-symmetric matter only (kF_n = kF_p, pin P9): per spin element the two entries
+#       (pn,pn) and (pn,np); the others follow from isospin invariance of the effective interaction,
+#       (pp,pp) = (nn,nn) = (pn,pn) + (pn,np)   [T = 1],   (np,np) = (pn,pn),   (np,pn) = (pn,np).
+PACK_CHARGE, PACK_ISOSPIN = 1, 2
+PACK_BLOCKS = ((0, 0), (1, 1), (2, 2), (3, 3), (1, 2), (2, 1))     # (row isospin pair, column isospin pair)
+PACKED_COMPLEX = {PACK_CHARGE: 96, PACK_ISOSPIN: 32}
+
+
+def _spin_rc(sp: int):
+    """row and column offsets 8 s1 + 4 s2 of spin element sp = 4 (2 s1' + s2') + (2 s1 + s2)."""
+    return 4 * (sp >> 2), 4 * (sp & 3)
+
+
+def pack(M, fmt: int) -> np.ndarray:
+    """M[n,16,16] complex -> packed[n, 96 or 32] complex: copies the entries of the subset, nothing else."""
+    M = np.asarray(M)
+    out = np.zeros((M.shape[0], PACKED_COMPLEX[fmt]), dtype=complex)
+    for sp in range(16):
+        r0, c0 = _spin_rc(sp)
+        if fmt == PACK_CHARGE:
+            for nb, (to, ti) in enumerate(PACK_BLOCKS):
+                out[:, 6 * sp + nb] = M[:, r0 + to, c0 + ti]
+        else:
+            out[:, 2 * sp + 0] = M[:, r0 + 1, c0 + 1]
+            out[:, 2 * sp + 1] = M[:, r0 + 1, c0 + 2]
+    return out
+
+
+def unpack(P, fmt: int) -> np.ndarray:
+    """packed[n, 96 or 32] complex -> M[n,16,16]: the 160 charge-violating entries are 0 (P6); format 2 fills the
+    other four blocks from isospin symmetry (P9)."""
+    P = np.asarray(P)
+    M = np.zeros((P.shape[0], 16, 16), dtype=complex)
+    for sp in range(16):
+        r0, c0 = _spin_rc(sp)
+        if fmt == PACK_CHARGE:
+            for nb, (to, ti) in enumerate(PACK_BLOCKS):
+                M[:, r0 + to, c0 + ti] = P[:, 6 * sp + nb]
+        else:
+            d, x = P[:, 2 * sp + 0], P[:, 2 * sp + 1]
+            M[:, r0 + 1, c0 + 1] = d
+            M[:, r0 + 2, c0 + 2] = d
+            M[:, r0 + 1, c0 + 2] = x
+            M[:, r0 + 2, c0 + 1] = x
+            M[:, r0 + 0, c0 + 0] = d + x
+            M[:, r0 + 3, c0 + 3] = d + x
+    return M
+
+
 def num_threads() -> int:
     return int(_load().oracle_num_threads())
 

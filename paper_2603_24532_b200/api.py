@@ -60,6 +60,32 @@ class NormalOrdering:
         binding.no_eval_diag(self._h, cfg.data_ptr(), n, out.data_ptr(), torch.cuda.current_stream(cfg.device).cuda_stream)
         return out
 
+    def packed(self, cfg: torch.Tensor, fmt: int = binding.NO_PACK_CHARGE) -> torch.Tensor:
+        """no_eval_packed (CUDA cfg) or no_eval_host_packed (CPU cfg): complex128 [n, 96] (fmt 1: the charge-conserving
+        entries) or [n, 32] (fmt 2: isospin-symmetric matter only), on the device of cfg."""
+        cfg = cfg.to(torch.float64).contiguous().reshape(-1, 9)
+        n = cfg.shape[0]
+        pd = binding.no_packed_doubles(self._h, fmt)
+        if pd == 0:
+            raise ValueError("packed format does not apply to this handle (NO_PACK_ISOSPIN needs kF_n == kF_p)")
+        out = torch.empty((n, pd // 2, 2), dtype=torch.float64, device=cfg.device)
+        s = torch.cuda.current_stream(self.device).cuda_stream
+        if cfg.is_cuda:
+            binding.no_eval_packed(self._h, fmt, cfg.data_ptr(), n, out.data_ptr(), s)
+        elif n:
+            binding.no_eval_host_packed(self._h, fmt, cfg.data_ptr(), n, out.data_ptr(), s)
+        return torch.view_as_complex(out)
+
+    @staticmethod
+    def unpack(packed: torch.Tensor, fmt: int = binding.NO_PACK_CHARGE) -> torch.Tensor:
+        """no_unpack: packed complex128 CUDA tensor [n, 96 or 32] -> complex128 [n, 16, 16] on the same device."""
+        assert packed.is_cuda and packed.dtype == torch.complex128 and packed.is_contiguous()
+        n = packed.shape[0]
+        out = torch.empty((n, 16, 16, 2), dtype=torch.float64, device=packed.device)
+        with torch.cuda.device(packed.device):
+            binding.no_unpack(fmt, packed.data_ptr(), n, out.data_ptr(), torch.cuda.current_stream(packed.device).cuda_stream)
+        return torch.view_as_complex(out)
+
     def hf_energy(self, n_r: int, n_cos: int, n_phi: int) -> float:
         """no_hf_energy: 3N Hartree-Fock energy per volume (fm^-4) on the given grids for particles 1 and 2."""
         return binding.no_hf_energy(self._h, n_r, n_cos, n_phi, torch.cuda.current_stream(self.device).cuda_stream)

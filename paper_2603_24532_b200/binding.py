@@ -16,7 +16,10 @@ LIB_PATH = os.path.join(_HERE, "libno3n.so")
 NO_OK, NO_ERR_INVALID, NO_ERR_CUDA, NO_ERR_ALLOC = 0, 1, 2, 3
 
 EXPORTS = ("no_init", "no_init_angular", "no_eval", "no_eval_host", "no_eval_diag", "no_hf_energy", "no_sp_energy", "no_set_layout", "no_free", "no_strerror", "no_last_cuda_error",
-           "no_kernel_info", "no_evals_per_cfg", "no_probe_fp64_peak")
+           "no_kernel_info", "no_evals_per_cfg", "no_probe_fp64_peak",
+           "no_packed_doubles", "no_eval_packed", "no_unpack", "no_eval_host_packed")
+
+NO_PACK_CHARGE, NO_PACK_ISOSPIN = 1, 2
 
 
 class no_params(ctypes.Structure):
@@ -57,6 +60,11 @@ def load() -> ctypes.CDLL:
         lib.no_sp_energy.argtypes = [H, ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                      ctypes.c_void_p, ctypes.c_void_p]
         lib.no_set_layout.argtypes = [H, ctypes.c_int]
+        lib.no_packed_doubles.argtypes = [H, ctypes.c_int]
+        lib.no_eval_packed.argtypes = [H, ctypes.c_int, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]
+        lib.no_unpack.argtypes = [ctypes.c_int, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]
+        lib.no_eval_host_packed.argtypes = [H, ctypes.c_int, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p,
+                                            ctypes.c_void_p]
         lib.no_free.argtypes = [H]
         lib.no_strerror.argtypes = [ctypes.c_int]
         lib.no_strerror.restype = ctypes.c_char_p
@@ -68,7 +76,7 @@ def load() -> ctypes.CDLL:
         lib.no_probe_fp64_peak.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double), ip,
                                            ctypes.c_void_p]
         for name in ("no_init", "no_init_angular", "no_eval", "no_eval_host", "no_eval_diag", "no_hf_energy", "no_sp_energy", "no_set_layout", "no_free", "no_kernel_info",
-                     "no_probe_fp64_peak"):
+                     "no_probe_fp64_peak", "no_packed_doubles", "no_eval_packed", "no_unpack", "no_eval_host_packed"):
             getattr(lib, name).restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -119,6 +127,36 @@ def no_eval_diag(h, d_cfg_ptr: int, n_cfg: int, d_out_ptr: int, stream_ptr: Opti
                              ctypes.c_void_p(stream_ptr or 0))
     if rc != NO_OK:
         raise NoError(rc, "no_eval_diag")
+
+
+def no_packed_doubles(h, fmt: int) -> int:
+    """doubles per configuration of packed format fmt for this handle (0: the format does not apply)."""
+    return int(load().no_packed_doubles(h, fmt))
+
+
+def no_eval_packed(h, fmt: int, d_cfg_ptr: int, n_cfg: int, d_packed_ptr: int, stream_ptr: Optional[int] = None) -> None:
+    """no_eval_packed with raw DEVICE pointers: d_packed is [n_cfg][no_packed_doubles(h, fmt)] doubles."""
+    rc = load().no_eval_packed(h, fmt, ctypes.c_void_p(d_cfg_ptr), n_cfg, ctypes.c_void_p(d_packed_ptr),
+                               ctypes.c_void_p(stream_ptr or 0))
+    if rc != NO_OK:
+        raise NoError(rc, "no_eval_packed")
+
+
+def no_unpack(fmt: int, d_packed_ptr: int, n_cfg: int, d_out_ptr: int, stream_ptr: Optional[int] = None) -> None:
+    """no_unpack with raw DEVICE pointers: packed -> [n_cfg][16][16][2]."""
+    rc = load().no_unpack(fmt, ctypes.c_void_p(d_packed_ptr), n_cfg, ctypes.c_void_p(d_out_ptr),
+                          ctypes.c_void_p(stream_ptr or 0))
+    if rc != NO_OK:
+        raise NoError(rc, "no_unpack")
+
+
+def no_eval_host_packed(h, fmt: int, h_cfg_ptr: int, n_cfg: int, h_packed_ptr: int,
+                        stream_ptr: Optional[int] = None) -> None:
+    """no_eval_host_packed with raw HOST pointers; synchronises the stream before returning."""
+    rc = load().no_eval_host_packed(h, fmt, ctypes.c_void_p(h_cfg_ptr), n_cfg, ctypes.c_void_p(h_packed_ptr),
+                                    ctypes.c_void_p(stream_ptr or 0))
+    if rc != NO_OK:
+        raise NoError(rc, "no_eval_host_packed")
 
 
 def no_hf_energy(h, n_r: int, n_cos: int, n_phi: int, stream_ptr: Optional[int] = None) -> float:

@@ -86,7 +86,8 @@ struct no_handle {
   // scratch of the host-buffer path
   double* d_cfg;
   double* d_out;
-  long long scratch_cfg;
+  long long scratch_cfg;      // configurations d_cfg holds
+  long long scratch_out;      // doubles d_out holds
   double* hf_arena;           // grow-only device scratch of no_hf_energy / no_sp_energy
   long long hf_arena_doubles;
   std::atomic<int> layout;    // 0 automatic, 1 always one warp per configuration, 2 always one CTA per configuration;
@@ -127,7 +128,7 @@ int resolve_layout(const no_handle* h, long long n_cfg) {
 
 int launch(const no_handle* h, const double* d_cfg, long long n_cfg, double* d_out, cudaStream_t s, int layout,
            int mode = kModeFull, bool forward = false) {
-  const long long out_doubles = mode == kModeDiag ? 4 : 512;
+  const long long out_doubles = no3n::out_doubles(mode);
   const bool split = layout == 2;
   const long long per_cta = split ? 1 : kWarps;
   const KernelFn fn = split ? h->var.fn_split : (forward ? h->var.fn_fwd : h->var.fn);
@@ -178,7 +179,7 @@ int no_init_angular(no_handle** out, const no_params* p, const double* h_dirs, i
   if (!h_dirs && n_dir != 0) return NO_ERR_INVALID;
   no_handle* h = new (std::nothrow) no_handle();
   if (!h) return NO_ERR_ALLOC;
-  h->d_tab = nullptr; h->d_cfg = nullptr; h->d_out = nullptr; h->scratch_cfg = 0; h->host_path_ready = false;
+  h->d_tab = nullptr; h->d_cfg = nullptr; h->d_out = nullptr; h->scratch_cfg = 0; h->scratch_out = 0; h->host_path_ready = false;
   h->layout.store(0); h->busy.clear();
   h->max_grid = kMaxGrid;
   if (const char* e = getenv("NO3N_MAX_GRID")) {          // testing knob: exercises the multi-launch path at small sizes
@@ -355,7 +356,8 @@ int no_sp_energy(no_handle* h, const double* h_k1, int n_k, int n_r, int n_cos, 
 namespace {
 
 // body of no_eval_host after the scratch is in place; any failure is reported after the copy stream has drained
-int host_path(no_handle* h, const double* h_cfg, long long n_cfg, double* h_out, cudaStream_t s) {
+int host_path(no_handle* h, const double* h_cfg, long long n_cfg, double* h_out, cudaStream_t s, int mode) {
+  const long long od = no3n::out_doubles(mode);
   NO_CUDA(cudaMemcpyAsync(h->d_cfg, h_cfg, sizeof(double) * 9 * (size_t)n_cfg, cudaMemcpyHostToDevice, s));
   // chunks of whole waves of resident CTAs (about n/8, at most ~64 Ki configurations): the copy of chunk k
   // (copy stream) runs under the kernel of chunk k + 1 (caller's stream).  One layout for the whole call.
@@ -367,11 +369,11 @@ int host_path(no_handle* h, const double* h_cfg, long long n_cfg, double* h_out,
   int k = 0;
   for (long long c0 = 0; c0 < n_cfg; c0 += chunk, ++k) {
     const long long cnt = n_cfg - c0 < chunk ? n_cfg - c0 : chunk;
-    const int rc = launch(h, h->d_cfg + 9 * c0, cnt, h->d_out + 512 * c0, s, layout);
+    const int rc = launch(h, h->d_cfg + 9 * c0, cnt, h->d_out + od * c0, s, layout, mode);
     if (rc != NO_OK) return rc;
     NO_CUDA(cudaEventRecord(h->ev_chunk[k & 1], s));
     NO_CUDA(cudaStreamWaitEvent(h->copy_stream, h->ev_chunk[k & 1], 0));
-    NO_CUDA(cudaMemcpyAsync(h_out + 512 * c0, h->d_out + 512 * c0, sizeof(double) * 512 * (size_t)cnt,
+    NO_CUDA(cudaMemcpyAsync(h_out + od * c0, h->d_out + od * c0, sizeof(double) * (size_t)(od * cnt),
                             cudaMemcpyDeviceToHost, h->copy_stream));
   }
   NO_CUDA(cudaEventRecord(h->ev_copied, h->copy_stream));
@@ -382,8 +384,19 @@ int host_path(no_handle* h, const double* h_cfg, long long n_cfg, double* h_out,
 
 }  // namespace
 
-int no_eval_host(no_handle* h, const double* h_cfg, long long n_cfg, double* h_out, void* cuda_stream) {
-  if (!h || n_cfg < 0) return NO_ERR_INVALID;
+namespace {
+
+// kernel output mode of a packed format for this handle; -1 if the format does not apply
+int packed_mode(const no_handle* h, int format) {
+  if (format == NO_PACK_CHARGE) return kModePacked;
+  // the isospin-reduced form exists only where the effective interaction is isospin invariant: one Fermi sphere
+  // shared by both species (kF_n = kF_p), traced over the full isospin of the third nucleon
+  if (format == NO_PACK_ISOSPIN && h->plan.dp.n_pass == 1 && h->plan.dp.esum[0] == 0.0 && h->plan.dp.nsp[0] == 2.0)
+    return kModeIso;
+  return -1;
+}
+
+int eval_host_mode(no_handle* h, const double* h_cfg, long long n_cfg, double* h_out, void* cuda_stream, int mode) {
   if (n_cfg == 0) return NO_OK;
   if (!h_cfg || !h_out) return NO_ERR_INVALID;
   BusyGuard busy(h);
@@ -391,16 +404,22 @@ int no_eval_host(no_handle* h, const double* h_cfg, long long n_cfg, double* h_o
   DeviceGuard guard(h->device);
   if (!guard.ok) return cuda_fail(cudaGetLastError(), "cudaSetDevice");
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  const long long need_out = no3n::out_doubles(mode) * n_cfg;
   if (n_cfg > h->scratch_cfg) {
     if (h->d_cfg) cudaFree(h->d_cfg);
-    if (h->d_out) cudaFree(h->d_out);
-    h->d_cfg = h->d_out = nullptr;
+    h->d_cfg = nullptr;
     h->scratch_cfg = 0;
-    cudaError_t e = cudaMalloc((void**)&h->d_cfg, sizeof(double) * 9 * (size_t)n_cfg);
+    const cudaError_t e = cudaMalloc((void**)&h->d_cfg, sizeof(double) * 9 * (size_t)n_cfg);
     if (e != cudaSuccess) { cuda_fail(e, "cudaMalloc(cfg scratch)"); return NO_ERR_ALLOC; }
-    e = cudaMalloc((void**)&h->d_out, sizeof(double) * 512 * (size_t)n_cfg);
-    if (e != cudaSuccess) { cudaFree(h->d_cfg); h->d_cfg = nullptr; cuda_fail(e, "cudaMalloc(out scratch)"); return NO_ERR_ALLOC; }
     h->scratch_cfg = n_cfg;
+  }
+  if (need_out > h->scratch_out) {
+    if (h->d_out) cudaFree(h->d_out);
+    h->d_out = nullptr;
+    h->scratch_out = 0;
+    const cudaError_t e = cudaMalloc((void**)&h->d_out, sizeof(double) * (size_t)need_out);
+    if (e != cudaSuccess) { cuda_fail(e, "cudaMalloc(out scratch)"); return NO_ERR_ALLOC; }
+    h->scratch_out = need_out;
   }
   if (!h->host_path_ready) {
     NO_CUDA(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
@@ -416,13 +435,65 @@ int no_eval_host(no_handle* h, const double* h_cfg, long long n_cfg, double* h_o
     }
     h->host_path_ready = true;
   }
-  const int rc = host_path(h, h_cfg, n_cfg, h_out, s);
+  const int rc = host_path(h, h_cfg, n_cfg, h_out, s, mode);
   if (rc != NO_OK) {
     // nothing of this call may still be writing into the caller's buffers or the scratch when it returns
     cudaStreamSynchronize(h->copy_stream);
     cudaStreamSynchronize(s);
   }
   return rc;
+}
+
+}  // namespace
+
+int no_eval_host(no_handle* h, const double* h_cfg, long long n_cfg, double* h_out, void* cuda_stream) {
+  if (!h || n_cfg < 0) return NO_ERR_INVALID;
+  return eval_host_mode(h, h_cfg, n_cfg, h_out, cuda_stream, kModeFull);
+}
+
+int no_eval_host_packed(no_handle* h, int format, const double* h_cfg, long long n_cfg, double* h_packed,
+                        void* cuda_stream) {
+  if (!h || n_cfg < 0) return NO_ERR_INVALID;
+  const int mode = packed_mode(h, format);
+  if (mode < 0) return NO_ERR_INVALID;
+  return eval_host_mode(h, h_cfg, n_cfg, h_packed, cuda_stream, mode);
+}
+
+int no_packed_doubles(const no_handle* h, int format) {
+  if (!h) return 0;
+  const int mode = packed_mode(h, format);
+  return mode < 0 ? 0 : no3n::out_doubles(mode);
+}
+
+int no_eval_packed(const no_handle* h, int format, const double* d_cfg, long long n_cfg, double* d_packed,
+                   void* cuda_stream) {
+  if (!h || n_cfg < 0) return NO_ERR_INVALID;
+  const int mode = packed_mode(h, format);
+  if (mode < 0) return NO_ERR_INVALID;
+  if (n_cfg == 0) return NO_OK;
+  if (!d_cfg || !d_packed) return NO_ERR_INVALID;
+  if ((reinterpret_cast<uintptr_t>(d_cfg) & 7u) || (reinterpret_cast<uintptr_t>(d_packed) & 15u)) return NO_ERR_INVALID;
+  DeviceGuard guard(h->device);
+  if (!guard.ok) return cuda_fail(cudaGetLastError(), "cudaSetDevice");
+  return launch(h, d_cfg, n_cfg, d_packed, static_cast<cudaStream_t>(cuda_stream), resolve_layout(h, n_cfg), mode);
+}
+
+int no_unpack(int format, const double* d_packed, long long n_cfg, double* d_out, void* cuda_stream) {
+  if (n_cfg < 0 || (format != NO_PACK_CHARGE && format != NO_PACK_ISOSPIN)) return NO_ERR_INVALID;
+  if (n_cfg == 0) return NO_OK;
+  if (!d_packed || !d_out) return NO_ERR_INVALID;
+  if ((reinterpret_cast<uintptr_t>(d_packed) & 15u) || (reinterpret_cast<uintptr_t>(d_out) & 15u)) return NO_ERR_INVALID;
+  // runs on the device that owns the pointers (the caller's current device), like a memcpy
+  const int mode = format == NO_PACK_CHARGE ? kModePacked : kModeIso;
+  const long long pd = no3n::out_doubles(mode);
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  for (long long c0 = 0; c0 < n_cfg; c0 += kMaxGrid) {
+    const long long cnt = n_cfg - c0 < kMaxGrid ? n_cfg - c0 : kMaxGrid;
+    unpack_kernel<<<(unsigned)cnt, 256, 0, s>>>(reinterpret_cast<const double2*>(d_packed + pd * c0), cnt,
+                                                reinterpret_cast<double2*>(d_out + 512 * c0), mode);
+    NO_CUDA(cudaGetLastError());
+  }
+  return NO_OK;
 }
 
 int no_free(no_handle* h) {

@@ -20,6 +20,12 @@ namespace no3n {
 
 constexpr int kModeFull = 0;   // out[n_cfg][16][16][2]
 constexpr int kModeDiag = 1;   // out[n_cfg][4]
+constexpr int kModePacked = 2; // out[n_cfg][16 spin elements][6 charge-conserving isospin blocks][2]   (include/no.h NO_PACK_CHARGE)
+constexpr int kModeIso = 3;    // out[n_cfg][16 spin elements][(pn,pn), (pn,np)][2], isospin-symmetric matter (NO_PACK_ISOSPIN)
+
+__host__ __device__ constexpr int out_doubles(int mode) {
+  return mode == kModeDiag ? 4 : (mode == kModePacked ? 192 : (mode == kModeIso ? 64 : 512));
+}
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return static_cast<uint32_t>(__cvta_generic_to_shared(p));
@@ -245,10 +251,28 @@ no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg,
     if (lane < 4) out[ic * 4 + lane] = re;
     return;
   }
-  double2* o = reinterpret_cast<double2*>(out) + ic * 256;
   P3Lane pl;
   phase3_lane_setup(lane, pl);
   const int h = lane & 1;
+  if (mode == kModePacked) {
+    // only the 96 entries that charge conservation allows, [spin element][block]
+    double2* o = reinterpret_cast<double2*>(out) + ic * 96 + (lane >> 1) * 6 + h;
+#pragma unroll
+    for (int it = 0; it < 3; ++it) {
+      double re, im;
+      phase3_block(coef, pl, 2 * it + h, re, im);
+      o[2 * it] = make_double2(re, im);
+    }
+    return;
+  }
+  if (mode == kModeIso) {
+    // isospin-symmetric matter: the (pn,pn) and (pn,np) blocks determine the other four (pin P9); one 512-byte warp store
+    double re, im;
+    phase3_block(coef, pl, h ? 4 : 1, re, im);
+    reinterpret_cast<double2*>(out)[ic * 32 + lane] = make_double2(re, im);
+    return;
+  }
+  double2* o = reinterpret_cast<double2*>(out) + ic * 256;
 #pragma unroll
   for (int it = 0; it < 3; ++it) {
     double re, im;
@@ -257,6 +281,27 @@ no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg,
   }
 #pragma unroll
   for (int it = 0; it < 5; ++it) o[phase3_zero_off(pl, 2 * it + h)] = make_double2(0.0, 0.0);
+}
+
+// ---- reconstruction of the 16x16 matrix from a packed form ----
+// one thread per element of the full matrix: charge-violating entries are 0; format kModeIso fills the four other
+// charge-conserving blocks from isospin symmetry, (pp,pp) = (nn,nn) = (pn,pn) + (pn,np), (np,np) = (pn,pn), (np,pn) = (pn,np)
+__global__ void __launch_bounds__(256) unpack_kernel(const double2* __restrict__ packed, long long n_cfg,
+                                                     double2* __restrict__ out, int mode) {
+  const long long c = blockIdx.x;
+  const int e = threadIdx.x, row = e >> 4, col = e & 15;
+  const int sp = 4 * (row >> 2) + (col >> 2), nb = iso_block(row & 3, col & 3);
+  double2 v = make_double2(0.0, 0.0);
+  if (nb >= 0) {
+    if (mode == kModePacked) {
+      v = packed[c * 96 + 6 * sp + nb];
+    } else {
+      const double2 d = packed[c * 32 + 2 * sp], x = packed[c * 32 + 2 * sp + 1];
+      if (nb == 0 || nb == 3) v = make_double2(d.x + x.x, d.y + x.y);
+      else v = nb < 3 ? d : x;
+    }
+  }
+  if (c < n_cfg) out[c * 256 + e] = v;
 }
 
 // ---- Hartree-Fock contraction helpers ----

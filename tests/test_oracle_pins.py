@@ -589,3 +589,41 @@ def test_sp_energy_cE_closed_form():
     pref = -(-0.5) * kF ** 3 / (math.pi ** 2 * (92.4 / hbarc) ** 4 * (700.0 / hbarc))
     sig = O.sp_energy(np.array([[0.3, -0.2, 0.5], [2.0, 1.0, -3.0]]), 3, 2, 2, **kw)
     assert np.allclose(sig, pref * kF ** 3 / (4 * math.pi ** 2), rtol=1e-12, atol=0)
+
+
+# ----------------------------------------------------------------------------------------------
+# Packed, symmetry-reduced matrix, oracle functions pack / unpack
+# ----------------------------------------------------------------------------------------------
+def test_pack_format1_is_exactly_the_96_charge_conserving_entries():
+    """"only up to 4^A C(2A,A) matrix elements can be non-zero": the index map of format 1 hits each of
+    the 96 allowed (row, column) pairs once and nothing else (checked on a matrix of distinct labels, independent of the physics)."""
+    label = (np.arange(256).reshape(1, 16, 16) + 1).astype(complex)
+    P = O.pack(label, O.PACK_CHARGE)[0].real.astype(int) - 1
+    assert len(set(P.tolist())) == 96 == 4 ** 2 * math.comb(4, 2)
+    for e in P:
+        r, c = divmod(int(e), 16)
+        assert ((r >> 1) & 1) + (r & 1) == ((c >> 1) & 1) + (c & 1)
+    # the element order: spin element major, then (pp,pp) (pn,pn) (np,np) (nn,nn) (pn,np) (np,pn)
+    assert P[0] == 16 * idx(0, 0, 0, 0) + idx(0, 0, 0, 0) and P[4] == 16 * idx(0, 0, 0, 1) + idx(0, 0, 1, 0)
+    assert P[6 * 7 + 5] == 16 * idx(0, 1, 1, 0) + idx(1, 1, 0, 1)
+    U = O.unpack(O.pack(label, O.PACK_CHARGE), O.PACK_CHARGE)[0]
+    allowed = U != 0
+    assert allowed.sum() == 96 and (U[allowed] == label[0][allowed]).all()
+
+
+@pytest.mark.parametrize("matter", ["snm", "pnm", "asym"])
+def test_unpack_of_pack_reproduces_the_oracle_matrix(matter):
+    """Format 1 loses nothing in any matter (P6); format 2 reconstructs the matrix only in isospin-symmetric matter
+    (P9: pp = nn = T=1 combination, pn/np blocks equal) and must NOT be used elsewhere (pp != nn there)."""
+    kf = {"snm": (1.1, 1.1), "pnm": (1.3, 0.0), "asym": (1.2, 0.9)}[matter]
+    kw = dict(PHYS, c4=5.4, kf_n=kf[0], kf_p=kf[1], n_r=3, n_cos=3, n_phi=4)
+    M = O.normal_order(rand_cfg(3, 1.5), **kw)
+    scale = np.abs(M).max(axis=(1, 2), keepdims=True)
+    U1 = O.unpack(O.pack(M, O.PACK_CHARGE), O.PACK_CHARGE)
+    assert np.abs(U1 - M).max() <= 1e-16 * scale.max()        # only the O(1e-17) structural zeros of the oracle differ
+    U2 = O.unpack(O.pack(M, O.PACK_ISOSPIN), O.PACK_ISOSPIN)
+    err = (np.abs(U2 - M) / scale).max()
+    if matter == "snm":
+        assert err < 4e-16
+    else:
+        assert err > 1e-3

@@ -320,7 +320,8 @@ def test_batches_larger_than_one_grid_are_cut_into_several_launches(monkeypatch)
         assert np.array_equal(no(cfg).cpu().numpy(), ref[layout])
         assert np.array_equal(no.diag(cfg).cpu().numpy(), ref[layout, "diag"])
         h_out = np.empty((37, 16, 16, 2))
-        binding.no_eval_host(no._h, run.configurations().ctypes.data, 37, h_out.ctypes.data, None)
+        h_cfg = run.configurations()                     # kept alive across the call (a raw pointer is passed)
+        binding.no_eval_host(no._h, h_cfg.ctypes.data, 37, h_out.ctypes.data, None)
         assert np.array_equal(h_out[..., 0] + 1j * h_out[..., 1], ref[layout])
         no.close()
 
@@ -526,3 +527,96 @@ def test_fp64_probe_reports_a_sane_peak():
 def test_native_library_is_the_one_loaded():
     maps = open(f"/proc/{os.getpid()}/maps").read()
     assert "libno3n.so" in maps
+
+
+# ----------------------------------------------------------------------------------------------
+# packed, symmetry-reduced output and its reconstruction
+# ----------------------------------------------------------------------------------------------
+def _check_packed(got, want, label):
+    """same criterion as _check, on packed rows: relative 1e-10 above 1e-12 of the row maximum"""
+    mx = np.abs(want).max(axis=1, keepdims=True)
+    mask = np.abs(want) > MAG_FLOOR * mx
+    rel = np.abs(got - want)[mask] / np.abs(want)[mask]
+    worst = rel.max() if rel.size else 0.0
+    assert worst < REL_TOL, f"{label}: max rel err {worst:.3e}"
+    return worst
+
+
+@pytest.mark.parametrize("layout", [1, 2])
+@pytest.mark.parametrize("matter", ["snm", "pnm", "asym", "snm_c4_lebedev"])
+def test_packed_output_and_unpack_match_the_oracle(matter, layout):
+    from paper_2603_24532_b200 import angular_rules
+    kf = {"snm": (1.33, 1.33), "pnm": (1.2, 0.0), "asym": (1.3, 0.9), "snm_c4_lebedev": (1.1, 1.1)}[matter]
+    kw = dict(PHYS, kf_n=kf[0], kf_p=kf[1], n_r=6, n_cos=7, n_phi=5)
+    dirs = None
+    if matter == "snm_c4_lebedev":
+        kw.update(c4=5.4, n_cos=1, n_phi=1)
+        dirs = angular_rules.octahedral_rule(7)
+    cfg = W.momentum_configurations(11, 0, 37, 2.5, 2.0 * max(kf))
+    want = O.normal_order(cfg, dirs=dirs, **kw)
+    no = NormalOrdering(device=0, layout=layout, angular=dirs, **kw)
+    d_cfg = torch.from_numpy(cfg).cuda()
+    full = no(d_cfg)
+    formats = [binding.NO_PACK_CHARGE] + ([binding.NO_PACK_ISOSPIN] if kf[0] == kf[1] else [])
+    for fmt in formats:
+        packed = no.packed(d_cfg, fmt)
+        torch.cuda.synchronize()
+        assert packed.shape == (37, O.PACKED_COMPLEX[fmt]) and binding.no_packed_doubles(no._h, fmt) == 2 * O.PACKED_COMPLEX[fmt]
+        worst = _check_packed(packed.cpu().numpy(), O.pack(want, fmt), f"{matter} packed fmt {fmt}")
+        rebuilt = NormalOrdering.unpack(packed, fmt)
+        torch.cuda.synchronize()
+        worst = max(worst, _check(rebuilt.cpu().numpy(), want, f"{matter} unpack fmt {fmt}"))
+        # the oracle's own reconstruction of the oracle's packed form is the same matrix
+        _check(rebuilt.cpu().numpy(), O.unpack(O.pack(want, fmt), fmt), f"{matter} unpack vs oracle unpack fmt {fmt}")
+        if fmt == binding.NO_PACK_CHARGE:
+            assert torch.equal(rebuilt, full)                    # format 1 loses nothing: bit for bit no_eval
+        # the host path ships the same packed bits
+        host = no.packed(torch.from_numpy(cfg), fmt)
+        assert torch.equal(host, packed.cpu())
+        print(f"{matter} layout {layout} fmt {fmt}: max rel err {worst:.2e}")
+    if kf[0] != kf[1]:
+        assert binding.no_packed_doubles(no._h, binding.NO_PACK_ISOSPIN) == 0
+        with pytest.raises(binding.NoError):
+            out = torch.empty((37, 32, 2), dtype=torch.float64, device="cuda")
+            binding.no_eval_packed(no._h, binding.NO_PACK_ISOSPIN, d_cfg.data_ptr(), 37, out.data_ptr(), 0)
+    no.close()
+
+
+def test_packed_abi_argument_checks_and_full_size_launch():
+    """raw C-ABI calls: bad formats, null / misaligned pointers, n = 0; then the bench-size paper-quadrature launch in
+    packed form against the full no_eval launch (every configuration, bit for bit) and sampled against the oracle."""
+    lib = binding.load()
+    run = W.workload("paper").runs[0]
+    no = NormalOrdering(device=0, angular=run.angular(), **run.params())
+    h = no._h
+    n = run.n_cfg
+    cfg = run.configurations()
+    d_cfg = torch.from_numpy(cfg).cuda()
+    pk = torch.empty((n, 32, 2), dtype=torch.float64, device="cuda")
+    vp = ctypes.c_void_p
+    assert lib.no_eval_packed(h, 3, vp(d_cfg.data_ptr()), n, vp(pk.data_ptr()), None) == binding.NO_ERR_INVALID
+    assert lib.no_eval_packed(h, 0, vp(d_cfg.data_ptr()), n, vp(pk.data_ptr()), None) == binding.NO_ERR_INVALID
+    assert lib.no_eval_packed(h, 2, vp(d_cfg.data_ptr()), -1, vp(pk.data_ptr()), None) == binding.NO_ERR_INVALID
+    assert lib.no_eval_packed(h, 2, None, n, vp(pk.data_ptr()), None) == binding.NO_ERR_INVALID
+    assert lib.no_eval_packed(h, 2, vp(d_cfg.data_ptr()), n, vp(pk.data_ptr() + 8), None) == binding.NO_ERR_INVALID
+    assert lib.no_eval_packed(h, 2, None, 0, None, None) == binding.NO_OK
+    assert lib.no_unpack(5, vp(pk.data_ptr()), n, vp(pk.data_ptr()), None) == binding.NO_ERR_INVALID
+    assert lib.no_unpack(2, None, 0, None, None) == binding.NO_OK
+    assert lib.no_packed_doubles(h, 1) == 192 and lib.no_packed_doubles(h, 2) == 64 and lib.no_packed_doubles(h, 7) == 0
+    assert lib.no_packed_doubles(None, 1) == 0
+    # full size, isospin-reduced form (the paper workload is SNM)
+    assert lib.no_eval_packed(h, 2, vp(d_cfg.data_ptr()), n, vp(pk.data_ptr()), None) == binding.NO_OK
+    full = torch.empty((n, 16, 16, 2), dtype=torch.float64, device="cuda")
+    no.eval_into(d_cfg, full)
+    torch.cuda.synchronize()
+    F = torch.view_as_complex(full)
+    P = torch.view_as_complex(pk)
+    sp = torch.arange(16, device="cuda")
+    rows, cols = 4 * (sp >> 2), 4 * (sp & 3)
+    assert torch.equal(P[:, 0::2], F[:, rows + 1, cols + 1]) and torch.equal(P[:, 1::2], F[:, rows + 1, cols + 2])
+    idx = sample_indices(n, 16)
+    want = O.normal_order(cfg[idx], dirs=run.angular(), **run.params())
+    rebuilt = NormalOrdering.unpack(P[idx].contiguous(), 2).cpu().numpy()
+    worst = _check(rebuilt, want, "paper packed")
+    print(f"paper packed (isospin form, {n} configurations): max rel err {worst:.2e} on {len(idx)} sampled")
+    no.close()
