@@ -23,6 +23,8 @@ def build(force: bool = False) -> str:
         cmd = ["g++", "-O2", "-fopenmp", "-fcx-limited-range", "-shared", "-fPIC", "-Wall", "-Wextra",
                "-o", _LIB, _SRC]
         subprocess.run(cmd, check=True)
+    from . import trace
+    trace.build(force)          # the second oracle (spin-isospin trace, oracle/trace_oracle.c)
     return _LIB
 
 

@@ -15,8 +15,9 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libno3n.so")
-SOURCES = ["no_api.cu"]
-HEADERS = ["no_core.h", "no_host.h", "no_kernel.cuh", os.path.join("..", "..", "include", "no.h")]
+SOURCES = ["no_api.cu", "no_trace.cu"]
+HEADERS = ["no_core.h", "no_host.h", "no_kernel.cuh", "no_tma.cuh", "no_trace_host.h",
+           os.path.join("..", "..", "include", "no.h"), os.path.join("..", "..", "include", "no_trace.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
 

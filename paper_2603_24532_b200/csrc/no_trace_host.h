@@ -1,0 +1,245 @@
+// no_trace_host.h -- host-side planning of the spin-isospin trace kernel (PAPER.md:155-157 and
+// Appendix B): turns a diagram topology into a short program of tensor contractions.
+// Plain C++ (no CUDA calls) so that the CPU tests can drive it through tests/trace_emu.cpp.  Nothing here is shared
+// with oracle/.
+//
+// The trace of a closed two-body diagram,
+//     T = sum over the labels x_j = 2 s_j + t_j of its 2 n lines of prod_v V_v[pair(o1, o2)][pair(i1, i2)],
+// is the full contraction of a tensor network whose nodes are the vertex matrices.  The paper loops over the labels
+// (restricted to charge-conserving isospin assignments) with the most connected vertex pair innermost
+// (PAPER.md:643-651).  Here the network is contracted vertex by vertex instead: the partial result R carries the
+// labels of the lines that are cut by the frontier ("open" lines, at most kMaxOpen = 4, i.e. 256 complex numbers that
+// live in shared memory), and absorbing a vertex is one small complex matrix product
+//     R'[a, b] = sum_g R[a, g] W_v[g, b]        a: labels of the open lines that stay open  (nA = 4^kept values)
+//                                                g: labels of the lines the vertex closes     (nC = 4^closed)
+//                                                b: labels of the lines the vertex opens      (nB = 4^new)
+// which turns the exponential label sum (4^(2n) terms) into n products of at most 16 x 16 x 16.  Topologies whose
+// frontier would exceed four lines are handled by "slicing": the labels of up to kMaxSlice lines are fixed in an outer
+// loop (a line that starts and ends on the same vertex is always sliced).  The order of the vertices and the sliced
+// lines are chosen here, on the host, by exhaustive search for the fewest complex multiply-adds.
+//
+// All index arithmetic of the kernel is tabulated here: with x the label of a line attached to slot q of a vertex
+// (q = 0, 1: outgoing 1, 2; q = 2, 3: incoming 1, 2) the element offset inside the 16 x 16 matrix of include/no.h
+// (row = outgoing pair, column = incoming pair, pair index 8 s1 + 4 s2 + 2 t1 + t2) is the sum over the four slots of
+// slot_off(q, x); offsets into R are sums of label * 4^(position of the line in the open list).
+#pragma once
+
+#include <stdint.h>
+
+#include <algorithm>
+#include <vector>
+
+namespace no3n {
+
+constexpr int kTrMaxVertex = 6;
+constexpr int kTrMaxLines = 2 * kTrMaxVertex;
+constexpr int kTrMaxOpen = 4;        // open lines of the partial result: 4^4 = 256 complex numbers
+constexpr int kTrMaxSlice = 3;       // lines whose labels are fixed in the outer loop
+constexpr int kTrTab = 256;
+
+inline int slot_off(int slot, int x) {
+  const int s = x >> 1, t = x & 1;
+  switch (slot) {
+    case 0: return 16 * (8 * s + 2 * t);    // outgoing 1: row bits s1, t1
+    case 1: return 16 * (4 * s + t);        // outgoing 2: row bits s2, t2
+    case 2: return 8 * s + 2 * t;           // incoming 1: column bits
+    default: return 4 * s + t;              // incoming 2
+  }
+}
+
+// one absorption step, as the kernel runs it (offsets in complex elements)
+struct TraceStep {
+  int vertex;                 // which vertex matrix of the sample
+  int nA, nB, nC;             // kept, opened, closed label combinations (powers of 4); nA * nB <= 256
+  uint16_t baseR[kTrTab];     // [a]  offset of the kept labels in R
+  uint16_t offR[kTrTab];      // [g]  offset of the closed labels in R
+  uint16_t baseW[kTrTab];     // [b]  offset of the opened labels in the vertex matrix
+  uint16_t offW[kTrTab];      // [g]  offset of the closed labels in the vertex matrix
+  uint16_t sliceW[64];        // [outer iteration] offset of the sliced labels in the vertex matrix
+};
+
+struct TracePlan {
+  int n_vertex;
+  int n_slice_iter;           // 4^(number of sliced lines)
+  int n_sliced;
+  int sliced[kTrMaxSlice];    // line ids
+  int order[kTrMaxVertex];    // vertices in absorption order
+  int max_open;               // widest frontier
+  long long cmacs;            // complex multiply-adds per sample (all outer iterations)
+  long long n_isospin;        // charge-conserving isospin assignments of the lines, for information
+  TraceStep steps[kTrMaxVertex];
+};
+
+inline bool trace_topology_valid(int n, const int* topo) {
+  if (n < 1 || n > kTrMaxVertex) return false;
+  int outs[kTrMaxLines] = {0}, ins[kTrMaxLines] = {0};
+  for (int v = 0; v < n; ++v)
+    for (int q = 0; q < 4; ++q) {
+      const int l = topo[4 * v + q];
+      if (l < 0 || l >= 2 * n) return false;
+      (q < 2 ? outs : ins)[l]++;
+    }
+  for (int l = 0; l < 2 * n; ++l) if (outs[l] != 1 || ins[l] != 1) return false;
+  return true;
+}
+
+namespace trace_detail {
+
+// frontier simulation of one (order, sliced set); returns the cost or -1 if the frontier exceeds kTrMaxOpen
+inline long long simulate(int n, const int* topo, const int* order, unsigned sliced_mask, int* max_open) {
+  int open[kTrMaxLines], n_open = 0;
+  long long cost = 0;
+  *max_open = 0;
+  for (int k = 0; k < n; ++k) {
+    const int v = order[k];
+    int closed = 0, opened = 0;
+    for (int q = 0; q < 4; ++q) {
+      const int l = topo[4 * v + q];
+      if (sliced_mask >> l & 1) continue;
+      bool is_open = false;
+      for (int j = 0; j < n_open; ++j) is_open |= open[j] == l;
+      if (is_open) ++closed; else ++opened;
+    }
+    // a line opened twice by the same vertex is a self-loop that was not sliced
+    for (int q = 0; q < 4; ++q)
+      for (int r = q + 1; r < 4; ++r)
+        if (topo[4 * v + q] == topo[4 * v + r] && !(sliced_mask >> topo[4 * v + q] & 1)) return -1;
+    const int kept = n_open - closed;
+    if (kept + opened > kTrMaxOpen) return -1;
+    cost += (1LL << (2 * kept)) * (1LL << (2 * opened)) * (1LL << (2 * closed));
+    // new frontier: kept lines in their old order, then the opened lines in slot order
+    int next[kTrMaxLines], m = 0;
+    for (int j = 0; j < n_open; ++j) {
+      bool closes = false;
+      for (int q = 0; q < 4; ++q) closes |= topo[4 * v + q] == open[j];
+      if (!closes) next[m++] = open[j];
+    }
+    for (int q = 0; q < 4; ++q) {
+      const int l = topo[4 * v + q];
+      if (sliced_mask >> l & 1) continue;
+      bool was_open = false;
+      for (int j = 0; j < n_open; ++j) was_open |= open[j] == l;
+      if (!was_open) next[m++] = l;
+    }
+    n_open = m;
+    for (int j = 0; j < m; ++j) open[j] = next[j];
+    if (n_open > *max_open) *max_open = n_open;
+  }
+  return n_open == 0 ? cost : -1;
+}
+
+inline int popcount(unsigned m) { int c = 0; for (; m; m &= m - 1) ++c; return c; }
+
+}  // namespace trace_detail
+
+// 0 on success; 1 if the topology is malformed or cannot be contracted within the limits above
+inline int build_trace_plan(int n, const int* topo, TracePlan& plan) {
+  using namespace trace_detail;
+  if (!trace_topology_valid(n, topo)) return 1;
+  const int L = 2 * n;
+  plan = TracePlan();
+  plan.n_vertex = n;
+
+  // charge-conserving isospin assignments (information only)
+  plan.n_isospin = 0;
+  for (unsigned m = 0; m < (1u << L); ++m) {
+    bool ok = true;
+    for (int v = 0; v < n && ok; ++v) {
+      const int* t = topo + 4 * v;
+      ok = (int)(m >> t[0] & 1) + (int)(m >> t[1] & 1) == (int)(m >> t[2] & 1) + (int)(m >> t[3] & 1);
+    }
+    plan.n_isospin += ok;
+  }
+
+  // exhaustive search: sliced sets of at most kTrMaxSlice lines x all vertex orders, fewest multiply-adds wins
+  // (ties: fewer sliced lines, then the first order in lexicographic enumeration -- deterministic)
+  long long best = -1;
+  unsigned best_mask = 0;
+  int best_order[kTrMaxVertex] = {0}, best_open = 0;
+  for (int ns = 0; ns <= kTrMaxSlice; ++ns)
+    for (unsigned mask = 0; mask < (1u << L); ++mask) {
+      if (popcount(mask) != ns) continue;
+      int order[kTrMaxVertex];
+      for (int v = 0; v < n; ++v) order[v] = v;
+      do {
+        int mo = 0;
+        const long long c = simulate(n, topo, order, mask, &mo);
+        if (c < 0) continue;
+        const long long total = c << (2 * ns);
+        if (best < 0 || total < best) {
+          best = total; best_mask = mask; best_open = mo;
+          for (int v = 0; v < n; ++v) best_order[v] = order[v];
+        }
+      } while (std::next_permutation(order, order + n));
+    }
+  if (best < 0) return 1;
+  plan.cmacs = best;
+  plan.max_open = best_open;
+  plan.n_sliced = 0;
+  for (int l = 0; l < L; ++l) if (best_mask >> l & 1) plan.sliced[plan.n_sliced++] = l;
+  plan.n_slice_iter = 1 << (2 * plan.n_sliced);
+  for (int v = 0; v < n; ++v) plan.order[v] = best_order[v];
+
+  // tables of every step
+  int open[kTrMaxLines], n_open = 0;
+  for (int k = 0; k < n; ++k) {
+    const int v = plan.order[k];
+    TraceStep& s = plan.steps[k];
+    s.vertex = v;
+    int kept_pos[kTrMaxOpen], n_kept = 0;            // positions (in the old open list) of the lines that stay open
+    int closed_pos[4], closed_slot[4], n_closed = 0;  // closed lines: position in the old list, slot of this vertex
+    int opened_slot[4], opened_line[4], n_opened = 0;
+    for (int j = 0; j < n_open; ++j) {
+      int slot = -1;
+      for (int q = 0; q < 4; ++q) if (topo[4 * v + q] == open[j]) slot = q;
+      if (slot < 0) kept_pos[n_kept++] = j;
+      else { closed_pos[n_closed] = j; closed_slot[n_closed++] = slot; }
+    }
+    for (int q = 0; q < 4; ++q) {
+      const int l = topo[4 * v + q];
+      if (best_mask >> l & 1) continue;
+      bool was_open = false;
+      for (int j = 0; j < n_open; ++j) was_open |= open[j] == l;
+      if (!was_open) { opened_slot[n_opened] = q; opened_line[n_opened++] = l; }
+    }
+    s.nA = 1 << (2 * n_kept);
+    s.nB = 1 << (2 * n_opened);
+    s.nC = 1 << (2 * n_closed);
+    for (int a = 0; a < kTrTab; ++a) {
+      int off = 0;
+      for (int j = 0; j < n_kept; ++j) off += ((a >> (2 * j)) & 3) << (2 * kept_pos[j]);
+      s.baseR[a] = (uint16_t)(a < s.nA ? off : 0);
+    }
+    for (int g = 0; g < kTrTab; ++g) {
+      int offr = 0, offw = 0;
+      for (int j = 0; j < n_closed; ++j) {
+        const int x = (g >> (2 * j)) & 3;
+        offr += x << (2 * closed_pos[j]);
+        offw += slot_off(closed_slot[j], x);
+      }
+      s.offR[g] = (uint16_t)(g < s.nC ? offr : 0);
+      s.offW[g] = (uint16_t)(g < s.nC ? offw : 0);
+    }
+    for (int b = 0; b < kTrTab; ++b) {
+      int off = 0;
+      for (int j = 0; j < n_opened; ++j) off += slot_off(opened_slot[j], (b >> (2 * j)) & 3);
+      s.baseW[b] = (uint16_t)(b < s.nB ? off : 0);
+    }
+    for (int it = 0; it < 64; ++it) {
+      int off = 0;
+      for (int i = 0; i < plan.n_sliced; ++i)
+        for (int q = 0; q < 4; ++q)
+          if (topo[4 * v + q] == plan.sliced[i]) off += slot_off(q, (it >> (2 * i)) & 3);
+      s.sliceW[it] = (uint16_t)(it < plan.n_slice_iter ? off : 0);
+    }
+    // new frontier: kept lines in their old order, then the opened lines in slot order: R'[a + nA b]
+    int next[kTrMaxLines], m = 0;
+    for (int j = 0; j < n_kept; ++j) next[m++] = open[kept_pos[j]];
+    for (int j = 0; j < n_opened; ++j) next[m++] = opened_line[j];
+    n_open = m;
+    for (int j = 0; j < m; ++j) open[j] = next[j];
+  }
+  return n_open == 0 ? 0 : 1;
+}
+
+}  // namespace no3n
