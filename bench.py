@@ -33,8 +33,9 @@ UNIT = "evals/s"
 FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum per launch (mean over the launches of one step) of the workload's
 # kernel, from the ncu capture named beside it (profiles/); None = no capture of that workload exists
-NCU_DRAM_BYTES_PER_LAUNCH = {}
-NCU_DRAM_SOURCE = {}
+NCU_DRAM_BYTES_PER_LAUNCH = {"cfg5": 1675959125}
+NCU_DRAM_SOURCE = {"cfg5": "profiles/r02a.md (r02a_cfg5_dram.csv: all six launches of one cfg5 step, 10.06 GB of DRAM "
+                           "traffic against 9.83 GB algorithmic: 4.4 GB of output per 2^20-configuration launch cannot stay in the 126 MB L2)"}
 
 
 def flops_per_eval(n_reg: int, regulated: bool, forward: bool = False) -> float:
@@ -60,7 +61,7 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="cfg5", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "c4", "paper", "hf"])
+    ap.add_argument("--workload", default="cfg5", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "c4", "paper", "hf", "trace5"])
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg")
@@ -505,10 +506,187 @@ def run_hf(args):
         "cpu_baseline": cpu}), flush=True)
 
 
+# --------------------------------------------------------------------------------------------
+# the spin-isospin trace (no_trace_eval) as a workload of its own
+# --------------------------------------------------------------------------------------------
+TRACE_BENCH = dict(n_vertex=5, n_sample=1 << 18, seed=7)      # fifth-order ring, 5.4 GB of vertex matrices (> L2)
+TRACE_METRIC = "spin-isospin trace samples/s (fifth-order ring diagram, FP64 complex) on 1 B200"
+
+
+def hbm_peak_gbs():
+    """measured HBM copy bandwidth of this pool's B200s (driver-written MEASURED_PEAKS.json), else the guide's fallback"""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except (OSError, KeyError, ValueError):
+        return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+def run_trace(args):
+    """One step = one no_trace_eval launch over 2^18 samples of 5 vertex matrices (20 KiB per sample, read once)."""
+    from paper_2603_24532_b200 import trace_workloads as TW
+    n, n_sample = TRACE_BENCH["n_vertex"], TRACE_BENCH["n_sample"]
+    topo = TW.ring(n)
+    labels = 4 ** (2 * n)
+    if args.impl == "reference":
+        if int(os.environ.get("RANK", "0")) != 0:
+            return
+        if int(os.environ.get("WORLD_SIZE", "1")) > 1 and os.environ.get("OMP_NUM_THREADS") == "1":
+            os.environ["OMP_NUM_THREADS"] = str(os.cpu_count() or 1)
+        from oracle import trace as T
+        T.build()
+        m = args.cpu_sample or 256
+        V = TW.vertex_matrices(m, n, seed=TRACE_BENCH["seed"])
+        for _ in range(args.warmup):
+            T.trace_bruteforce(topo, V[:16])
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            T.trace_bruteforce(topo, V)
+        dt = (time.perf_counter() - t0) / args.steps
+        sample = f"first {m} samples of the workload, brute-force sum over all 4^10 label configurations each"
+        print(json.dumps({"impl": "reference", "metric": TRACE_METRIC, "value": m / dt, "unit": "samples/s",
+                          "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3,
+                          "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                          "config": {"workload": "trace5", "sample": sample},
+                          "cpu_baseline": {"value": m / dt, "unit": "samples/s", "cores": os.cpu_count(), "kind": "oracle (brute force)",
+                                           "sample": sample},
+                          "e2e": {"value": m / dt, "unit": "samples/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                          "gpu_launches": 0}), flush=True)
+        return
+    import torch
+
+    from paper_2603_24532_b200 import binding, build, replicas, workloads
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        torch.distributed.init_process_group("nccl", device_id=torch.device("cuda", local))
+    build.build()
+    binding.load()
+    dev = torch.device("cuda", local)
+    stream = torch.cuda.current_stream(dev)
+    plan = binding.no_trace_init(topo, local)
+    info = binding.no_trace_info(plan, n)
+    V = TW.vertex_matrices(n_sample, n, seed=TRACE_BENCH["seed"])
+    d_V = torch.from_numpy(V).to(dev)
+    d_out = torch.empty((n_sample,), dtype=torch.complex128, device=dev)
+    flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)
+
+    def barrier():
+        replicas.barrier()
+        torch.cuda.synchronize(dev)
+
+    warmup = max(args.warmup, 3)
+    for _ in range(warmup):
+        binding.no_trace_eval(plan, d_V.data_ptr(), n_sample, d_out.data_ptr(), stream.cuda_stream)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.25)
+    steps = max(args.steps, 20)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for a, b in ev:
+        flush.zero_()
+        a.record(stream)
+        binding.no_trace_eval(plan, d_V.data_ptr(), n_sample, d_out.data_ptr(), stream.cuda_stream)
+        b.record(stream)
+    barrier()
+    time.sleep(0.25)
+    clocks = sampler.stop()
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    t_dev = replicas.max_over_ranks(sum(step_ms) * 1e-3, dev)
+    value = replicas.whole_job_rate(n_sample, steps, t_dev)
+    bytes_step = n_sample * (n * 4096 + 16)
+    peak, peak_src = hbm_peak_gbs()
+    achieved = bytes_step * steps / (sum(step_ms) * 1e-3) / 1e9
+    flops_step = 8.0 * info["cmacs_per_sample"] * n_sample
+
+    # ---- end to end: HOST momentum configurations -> no_eval (the vertices are produced on the device, where the
+    # trace consumes them: the paper's pipeline, PAPER.md:176,186) -> no_trace_eval -> HOST traces ----
+    e2e = None
+    if not args.no_e2e:
+        m = 1 << 15                                            # samples of the pipeline leg (5 x 2^15 configurations)
+        run = workloads.workload("cfg3").runs[0].shrunk(n * m, 16)
+        h_cfg = torch.from_numpy(run.configurations()).pin_memory()
+        h_res = torch.empty((m,), dtype=torch.complex128).pin_memory()
+        d_cfg = torch.empty((n * m, 9), dtype=torch.float64, device=dev)
+        d_M = torch.empty((n * m, 16, 16, 2), dtype=torch.float64, device=dev)
+        d_res = torch.empty((m,), dtype=torch.complex128, device=dev)
+        h = binding.no_init(device=local, **run.params())
+
+        def pipeline():
+            d_cfg.copy_(h_cfg, non_blocking=True)
+            binding.no_eval(h, d_cfg.data_ptr(), n * m, d_M.data_ptr(), stream.cuda_stream)
+            binding.no_trace_eval(plan, d_M.data_ptr(), m, d_res.data_ptr(), stream.cuda_stream)
+            h_res.copy_(d_res, non_blocking=True)
+            torch.cuda.synchronize(dev)
+
+        pipeline()
+        barrier()
+        k = 5
+        t0 = time.perf_counter()
+        for _ in range(k):
+            pipeline()
+        barrier()
+        t_e2e = replicas.max_over_ranks((time.perf_counter() - t0) / k, dev)
+        # share of the trace inside the pipeline, device-timed
+        ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ea.record(stream)
+        binding.no_trace_eval(plan, d_M.data_ptr(), m, d_res.data_ptr(), stream.cuda_stream)
+        eb.record(stream)
+        torch.cuda.synchronize(dev)
+        e2e = {"value": world * m / t_e2e, "unit": "samples/s", "h2d_bytes_per_step": int(h_cfg.numel() * 8),
+               "d2h_bytes_per_step": int(m * 16), "ms_per_step": t_e2e * 1e3, "steps": k,
+               "checksum": float(h_res.abs().sum()),
+               "trace_ms_inside": ea.elapsed_time(eb),
+               "api": f"host configurations -> no_eval (SNM kF=1.33, 16^3 k3 grid, {n * m} vertices) -> no_trace_eval "
+                      f"({m} samples) -> host traces"}
+        binding.no_free(h)
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        from oracle import trace as T
+        mcpu = args.cpu_sample or 1024
+        t0 = time.perf_counter()
+        T.trace_bruteforce(topo, V[:mcpu])
+        dt = time.perf_counter() - t0
+        cpu = {"value": mcpu / dt, "unit": "samples/s", "cores": os.cpu_count(), "kind": "oracle (brute force over 4^10 label configurations, long double)",
+               "sample": f"first {mcpu} samples of the workload ({dt:.1f} s)"}
+    binding.no_trace_free(plan)
+    if world > 1:
+        torch.distributed.destroy_process_group()
+    if rank != 0:
+        return
+    print(json.dumps({
+        "metric": TRACE_METRIC, "value": value, "unit": "samples/s", "n_gpus": world, "steps": steps, "warmup": warmup,
+        "ms_per_step": t_dev / steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "trace5", "description": "spin-isospin trace of a fifth-order ring diagram (5 vertices, 10 lines, "
+                   "4^10 label configurations per sample), 2^18 samples of seeded charge-conserving complex 16x16 vertex matrices",
+                   "n_sample": n_sample, "label_configurations_per_s": value * labels, "plan": info,
+                   "l2": "256 MiB buffer rewritten between timed steps (L2 flush); the input (5.4 GB) exceeds L2",
+                   "parallelism": "replicas only: every rank traces the whole batch"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": steps,
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get("trace5"), "traffic_source": NCU_DRAM_SOURCE.get("trace5"),
+                     "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_step,
+                     "bytes_per_sample": n * 4096 + 16, "kernel": "trace_kernel", "avg_launch_ms": sum(step_ms) / steps,
+                     "fp64_tflops": flops_step * steps / (sum(step_ms) * 1e-3) / 1e12,
+                     "fp64_frac_of_nominal": flops_step * steps / (sum(step_ms) * 1e-3) / 1e12 / FP64_PEAK_NOMINAL_TFLOPS,
+                     "flops_per_sample": 8.0 * info["cmacs_per_sample"]},
+        "cpu_baseline": cpu}), flush=True)
+
+
 def main():
     args = parse_args()
     if args.workload == "hf":
         run_hf(args)
+        return
+    if args.workload == "trace5":
+        run_trace(args)
         return
     from paper_2603_24532_b200 import workloads
     wl = workloads.workload(args.workload)

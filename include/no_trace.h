@@ -62,6 +62,9 @@ int no_trace_eval(const no_trace_plan *plan, const double *d_vertices, long long
 int no_trace_info(const no_trace_plan *plan, long long *cmacs_per_sample, int *max_open, int *n_sliced,
                   long long *n_isospin_configs, int *order);
 
+/* Text of the last CUDA error seen by the calling thread in a no_trace_* call ("" if none). */
+const char *no_trace_last_cuda_error(void);
+
 /* Release the plan.  NULL is a no-op. */
 int no_trace_free(no_trace_plan *plan);
 

@@ -106,3 +106,47 @@ class NormalOrdering:
                 binding.no_eval_host(self._h, cfg.data_ptr(), n, out.data_ptr(),
                                      torch.cuda.current_stream(self.device).cuda_stream)
         return torch.view_as_complex(out)
+
+
+class SpinIsospinTrace:
+    """`SpinIsospinTrace(topo)`; `__call__(vertices)` -> complex128 [n_sample] on the device.
+
+    topo: int array [n_vertex, 4] = line ids (out 1, out 2, in 1, in 2) of every vertex (include/no_trace.h).
+    vertices: complex128 CUDA tensor [n_sample, n_vertex, 16, 16] (e.g. NormalOrdering output reshaped), contiguous.
+    """
+
+    def __init__(self, topo, device: int = 0):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2603_24532_b200 needs a CUDA device (no CPU fallback)")
+        self.device = device
+        self._p = binding.no_trace_init(topo, device)
+        self.n_vertex = len(topo)
+
+    def info(self) -> dict:
+        return binding.no_trace_info(self._p, self.n_vertex)
+
+    def eval_into(self, vertices: torch.Tensor, out: torch.Tensor, stream: torch.cuda.Stream | None = None) -> None:
+        assert vertices.is_cuda and out.is_cuda and vertices.is_contiguous() and out.is_contiguous()
+        assert vertices.dtype == torch.complex128 and out.dtype == torch.complex128
+        n = out.numel()
+        assert vertices.numel() == n * self.n_vertex * 256
+        s = stream if stream is not None else torch.cuda.current_stream(vertices.device)
+        binding.no_trace_eval(self._p, vertices.data_ptr(), n, out.data_ptr(), s.cuda_stream)
+
+    def __call__(self, vertices: torch.Tensor) -> torch.Tensor:
+        vertices = vertices.contiguous()
+        n = vertices.numel() // (self.n_vertex * 256)
+        out = torch.empty((n,), dtype=torch.complex128, device=vertices.device)
+        self.eval_into(vertices, out)
+        return out
+
+    def close(self):
+        if getattr(self, "_p", None) is not None:
+            binding.no_trace_free(self._p)
+            self._p = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

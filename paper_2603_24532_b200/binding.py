@@ -21,6 +21,8 @@ EXPORTS = ("no_init", "no_init_angular", "no_eval", "no_eval_host", "no_eval_dia
 
 NO_PACK_CHARGE, NO_PACK_ISOSPIN = 1, 2
 
+TRACE_EXPORTS = ("no_trace_init", "no_trace_eval", "no_trace_info", "no_trace_free", "no_trace_last_cuda_error")
+
 
 class no_params(ctypes.Structure):
     """struct no_params of include/no.h."""
@@ -77,6 +79,13 @@ def load() -> ctypes.CDLL:
                                            ctypes.c_void_p]
         for name in ("no_init", "no_init_angular", "no_eval", "no_eval_host", "no_eval_diag", "no_hf_energy", "no_sp_energy", "no_set_layout", "no_free", "no_kernel_info",
                      "no_probe_fp64_peak", "no_packed_doubles", "no_eval_packed", "no_unpack", "no_eval_host_packed"):
+            getattr(lib, name).restype = ctypes.c_int
+        lib.no_trace_init.argtypes = [ctypes.POINTER(H), ctypes.c_int, ctypes.c_void_p, ctypes.c_int]
+        lib.no_trace_eval.argtypes = [H, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]
+        lib.no_trace_info.argtypes = [H, ctypes.POINTER(ctypes.c_longlong), ip, ip, ctypes.POINTER(ctypes.c_longlong), ip]
+        lib.no_trace_free.argtypes = [H]
+        lib.no_trace_last_cuda_error.restype = ctypes.c_char_p
+        for name in ("no_trace_init", "no_trace_eval", "no_trace_info", "no_trace_free"):
             getattr(lib, name).restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -213,3 +222,40 @@ def no_probe_fp64_peak(device: int = 0, millis: int = 200, stream_ptr: Optional[
     if rc != NO_OK:
         raise NoError(rc, "no_probe_fp64_peak")
     return {"tflops": t.value, "n_sm": n.value}
+
+
+# ---- include/no_trace.h: spin-isospin trace of a closed diagram ----
+def no_trace_init(topo, device: int = 0) -> ctypes.c_void_p:
+    """no_trace_init: topo host int array [n_vertex, 4] = line ids (out 1, out 2, in 1, in 2); returns the plan."""
+    import numpy as np
+    t = np.ascontiguousarray(topo, dtype=np.int32).reshape(-1, 4)
+    h = ctypes.c_void_p()
+    rc = load().no_trace_init(ctypes.byref(h), t.shape[0], ctypes.c_void_p(t.ctypes.data), device)
+    if rc != NO_OK:
+        raise NoError(rc, "no_trace_init")
+    return h
+
+
+def no_trace_eval(plan, d_vertices_ptr: int, n_sample: int, d_out_ptr: int, stream_ptr: Optional[int] = None) -> None:
+    """no_trace_eval with raw DEVICE pointers: vertices [n_sample][n_vertex][16][16][2], out [n_sample][2]."""
+    rc = load().no_trace_eval(plan, ctypes.c_void_p(d_vertices_ptr), n_sample, ctypes.c_void_p(d_out_ptr),
+                              ctypes.c_void_p(stream_ptr or 0))
+    if rc != NO_OK:
+        raise NoError(rc, "no_trace_eval")
+
+
+def no_trace_info(plan, n_vertex: int) -> dict:
+    cm, iso = ctypes.c_longlong(), ctypes.c_longlong()
+    mo, ns = ctypes.c_int(), ctypes.c_int()
+    order = (ctypes.c_int * 8)()
+    rc = load().no_trace_info(plan, ctypes.byref(cm), ctypes.byref(mo), ctypes.byref(ns), ctypes.byref(iso), order)
+    if rc != NO_OK:
+        raise NoError(rc, "no_trace_info")
+    return {"cmacs_per_sample": cm.value, "max_open": mo.value, "n_sliced": ns.value, "n_isospin_configs": iso.value,
+            "order": [order[i] for i in range(n_vertex)]}
+
+
+def no_trace_free(plan) -> None:
+    rc = load().no_trace_free(plan)
+    if rc != NO_OK:
+        raise NoError(rc, "no_trace_free")

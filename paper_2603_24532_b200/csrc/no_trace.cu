@@ -1,14 +1,15 @@
 // no_trace.cu -- spin-isospin trace kernel and its C ABI (include/no_trace.h; PAPER.md:155-157,
 // 639-653).  One warp contracts the tensor network of one Monte-Carlo sample: the n vertex matrices of the sample
-// (n x 4 KiB, contiguous in HBM) arrive in shared memory with ONE TMA bulk copy per sample (cp.async.bulk + mbarrier,
-// double buffered: the next sample's copy runs under this sample's arithmetic), the partial result (<= 256 complex
-// numbers) ping-pongs between two shared-memory buffers, and every step of the host-planned program
-// (no_trace_host.h) is a small complex matrix product whose index arithmetic is tabulated.  The dominant step shape
-// (16 x 16 x 16: ladders and rings) has a register-tiled path: a lane owns a 4 x 2 tile of the product, its operands
-// are warp-broadcast 16-byte shared-memory loads, 32 DFMA per 6 loads.  sm_100a only; there is no CPU path.
+// (n x 4 KiB, contiguous in HBM) arrive in shared memory through asynchronous 16-byte copies (cp.async, coalesced
+// 512-byte warp reads) into rows padded by one element, the partial result (<= 256 complex numbers) ping-pongs
+// between two padded shared-memory buffers, and every step of the host-planned program (no_trace_host.h) is a small
+// complex matrix product whose index arithmetic is tabulated.  The dominant step shape (16 x 16 x 16: ladders and
+// rings) runs on the FP64 tensor cores (mma.sync m8n8k4, SASS DMMA: 64 per step against 16 shared-memory fragment
+// loads); a vector-FP64 register-tiled variant of it is kept for comparison.  sm_100a only; there is no CPU path.
 #include <cuda_runtime.h>
 
 #include <cstdio>
+#include <cstdlib>
 #include <new>
 
 #include "../../include/no_trace.h"
@@ -32,19 +33,43 @@ __device__ __forceinline__ void cfma(double2& acc, const double2 a, const double
   acc.y = fma(a.y, b.x, acc.y);
 }
 
+constexpr int kTrStagesDefault = 1;
+constexpr int kTrPathDefault = 1;
+
 __device__ __forceinline__ double2 shfl_xor2(double2 v, int m) {
   return make_double2(__shfl_xor_sync(0xffffffffu, v.x, m), __shfl_xor_sync(0xffffffffu, v.y, m));
 }
 
-constexpr int kTrStages = 2;     // vertex buffers per warp (TMA double buffering)
+// m8n8k4 FP64 tensor-core product D = A B + C (SASS DMMA): lane l holds A[l / 4][l % 4], B[l % 4][l / 4] and
+// C[l / 4][2 (l % 4)], C[l / 4][2 (l % 4) + 1]
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+               : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
 
-// shared memory: plan (n_vertex steps) | per warp: mbarriers (16 B) | vertex buffers [kTrStages][n][256] complex | R [2][256] complex
+// shared memory: plan (n_vertex steps) | per warp: (16 B unused) | vertex buffers [stages][n][16][17] complex | R [2][16][17] complex
 __host__ __device__ inline size_t trace_plan_bytes(int n) { return 16 + (size_t)n * sizeof(TraceStep); }
-__host__ __device__ inline size_t trace_warp_bytes(int n) { return 16 + (size_t)kTrStages * n * 4096 + 2 * 4096; }
+__host__ __device__ inline size_t trace_warp_bytes(int n, int stages) {
+  return 16 + (size_t)(stages * n + 2) * kTrMat * 16;
+}
 
+// request one sample: n x 256 complex numbers, one 16-byte cp.async (LDGSTS) per lane and element -- coalesced 512-byte
+// warp reads from HBM, written into the padded rows of buffer `dst`, no registers held while in flight.  (One TMA bulk
+// copy per sample cannot pad the rows, and one per row is bound by the TMA issue rate: 80 descriptors per sample ran
+// at 1.17e8 samples/s, profiles/r02b.md.)
+__device__ __forceinline__ void request_sample(double2* dst, const double2* src, int n, int lane) {
+  for (int e = lane; e < 256 * n; e += 32) {
+    const int rc = e & 255;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;"
+                 ::"r"(smem_u32(dst + (e >> 8) * kTrMat + rc + (rc >> 4))), "l"(src + e) : "memory");
+  }
+  asm volatile("cp.async.commit_group;" ::: "memory");
+}
+
+// path: 0 = vector FP64 (DFMA) register tiles, 1 = FP64 tensor cores (DMMA m8n8k4) for the 16 x 16 x 16 steps
 __global__ void __launch_bounds__(512, 1)
 trace_kernel(const DevTracePlan* __restrict__ plan_g, const double2* __restrict__ V, long long n_sample,
-             double2* __restrict__ out) {
+             double2* __restrict__ out, int stages, int path) {
   extern __shared__ __align__(128) unsigned char tsm[];
   const int n = plan_g->n_vertex, n_iter = plan_g->n_slice_iter;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
@@ -56,63 +81,83 @@ trace_kernel(const DevTracePlan* __restrict__ plan_g, const double2* __restrict_
     for (int i = threadIdx.x; i < n16; i += blockDim.x) dst[i] = src[i];
   }
   const TraceStep* steps = reinterpret_cast<const TraceStep*>(tsm + 16);
-  unsigned char* wb = tsm + trace_plan_bytes(n) + (size_t)warp * trace_warp_bytes(n);
-  uint64_t* bar = reinterpret_cast<uint64_t*>(wb);                       // [kTrStages]
-  double2* vbuf = reinterpret_cast<double2*>(wb + 16);                   // [kTrStages][n][256]
-  double2* Rb = vbuf + (size_t)kTrStages * n * 256;                      // [2][256]
-  const uint32_t sample_bytes = (uint32_t)n * 4096u;
-  if (lane == 0)
-    for (int s = 0; s < kTrStages; ++s) mbar_init(bar + s, 1);
+  unsigned char* wb = tsm + trace_plan_bytes(n) + (size_t)warp * trace_warp_bytes(n, stages);
+  double2* vbuf = reinterpret_cast<double2*>(wb + 16);                   // [stages][n][16][17]
+  double2* Rb = vbuf + (size_t)stages * n * kTrMat;                      // [2][16][17]
   __syncthreads();
 
   const long long first = (long long)blockIdx.x * n_warps + warp, stride = (long long)gridDim.x * n_warps;
-  // prologue: request the first sample
-  if (lane == 0 && first < n_sample) {
-    mbar_expect_tx(bar, sample_bytes);
-    tma_bulk_g2s(vbuf, V + first * n * 256, sample_bytes, bar);
-  }
-  uint32_t phase[kTrStages] = {0, 0};
+  if (first < n_sample) request_sample(vbuf, V + first * n * 256, n, lane);
   int stage = 0;
   for (long long smp = first; smp < n_sample; smp += stride) {
-    // request the next sample into the other buffer (its last reader finished before the __syncwarp that ended
-    // the previous iteration; the proxy fence orders those generic-proxy reads before the async-proxy write)
     const long long nxt = smp + stride;
-    if (lane == 0 && nxt < n_sample) {
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-      mbar_expect_tx(bar + (stage ^ 1), sample_bytes);
-      tma_bulk_g2s(vbuf + (size_t)(stage ^ 1) * n * 256, V + nxt * n * 256, sample_bytes, bar + (stage ^ 1));
+    if (stages == 2 && nxt < n_sample) {
+      // the other buffer's last readers finished before the __syncwarp that ended the previous iteration
+      request_sample(vbuf + (size_t)(stage ^ 1) * n * kTrMat, V + nxt * n * 256, n, lane);
+      asm volatile("cp.async.wait_group 1;" ::: "memory");      // this sample has landed; the next one is in flight
+    } else {
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
     }
-    mbar_wait(bar + stage, phase[stage]);
-    phase[stage] ^= 1;
-    const double2* W = vbuf + (size_t)stage * n * 256;
+    __syncwarp();
+    const double2* W = vbuf + (size_t)stage * n * kTrMat;
 
     double2 total = make_double2(0.0, 0.0);
     for (int it = 0; it < n_iter; ++it) {
       double2* Rin = Rb;
-      double2* Rout = Rb + 256;
+      double2* Rout = Rb + kTrMat;
       double2 last = make_double2(0.0, 0.0);
+      if (lane == 0) Rin[0] = make_double2(1.0, 0.0);     // nothing open, nothing contracted yet: the scalar 1
+      __syncwarp();
       for (int k = 0; k < n; ++k) {
         const TraceStep& s = steps[k];
-        const double2* Wv = W + s.vertex * 256 + s.sliceW[it];
+        const double2* Wv = W + s.vertex * kTrMat + s.sliceW[it];
         const int nA = s.nA, nB = s.nB, nC = s.nC, nOut = nA * nB;
-        if (nA == 1 && nC == 1) {
-          // nothing is open on the input side (first vertex of a component): R' = the vertex's own entries,
-          // times the scalar carried so far (1 at the start; the trace of the finished components otherwise)
-          const double2 c = k == 0 ? make_double2(1.0, 0.0) : Rin[0];
-          for (int o = lane; o < nB; o += 32) {
-            double2 v = make_double2(0.0, 0.0);
-            cfma(v, c, Wv[s.baseW[o]]);
-            if (nB == 1) last = v;
-            Rout[o] = v;
+        if (nA == 16 && nB == 16 && nC == 16 && path == 1) {
+          // 16 x 16 x 16 complex product on the FP64 tensor cores: four real products per (8 x 8 tile, k-step of 4),
+          // Re = Re Re - Im Im, Im = Re Im + Im Re; fragments come straight from the tabulated offsets
+          const int r = lane >> 2, c = lane & 3;
+          int aR[2], bW[2], gR[4], gW[4];
+#pragma unroll
+          for (int t = 0; t < 2; ++t) { aR[t] = s.baseR[8 * t + r]; bW[t] = s.baseW[8 * t + r]; }
+#pragma unroll
+          for (int ks = 0; ks < 4; ++ks) { gR[ks] = s.offR[4 * ks + c]; gW[ks] = s.offW[4 * ks + c]; }
+          double cre[2][2][2], cim[2][2][2];
+#pragma unroll
+          for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+            for (int nt = 0; nt < 2; ++nt) cre[mt][nt][0] = cre[mt][nt][1] = cim[mt][nt][0] = cim[mt][nt][1] = 0.0;
+#pragma unroll
+          for (int ks = 0; ks < 4; ++ks) {
+            double2 A[2], B[2];
+#pragma unroll
+            for (int t = 0; t < 2; ++t) { A[t] = Rin[aR[t] + gR[ks]]; B[t] = Wv[gW[ks] + bW[t]]; }
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+              for (int nt = 0; nt < 2; ++nt) {
+                dmma884(cre[mt][nt][0], cre[mt][nt][1], A[mt].x, B[nt].x);
+                dmma884(cim[mt][nt][0], cim[mt][nt][1], A[mt].x, B[nt].y);
+                dmma884(cre[mt][nt][0], cre[mt][nt][1], -A[mt].y, B[nt].y);
+                dmma884(cim[mt][nt][0], cim[mt][nt][1], A[mt].y, B[nt].x);
+              }
           }
+#pragma unroll
+          for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+            for (int nt = 0; nt < 2; ++nt)
+#pragma unroll
+              for (int e = 0; e < 2; ++e) {
+                const int o = (8 * mt + r) + 16 * (8 * nt + 2 * c + e);
+                Rout[o + (o >> 4)] = make_double2(cre[mt][nt][e], cim[mt][nt][e]);
+              }
         } else if (nA == 16 && nB == 16 && nC == 16) {
-          // register-tiled 16 x 16 x 16 complex product: lane (la, lb) owns a = 4 la + i, b = 2 lb + j
+          // register-tiled 16 x 16 x 16 complex product: lane (la, lb) owns a = la + 4 i, b = lb + 8 j
           const int la = lane >> 3, lb = lane & 7;
           int rA[4], wB[2];
 #pragma unroll
-          for (int i = 0; i < 4; ++i) rA[i] = s.baseR[4 * la + i];
+          for (int i = 0; i < 4; ++i) rA[i] = s.baseR[la + 4 * i];
 #pragma unroll
-          for (int j = 0; j < 2; ++j) wB[j] = s.baseW[2 * lb + j];
+          for (int j = 0; j < 2; ++j) wB[j] = s.baseW[lb + 8 * j];
           double2 acc[4][2];
 #pragma unroll
           for (int i = 0; i < 4; ++i) acc[i][0] = acc[i][1] = make_double2(0.0, 0.0);
@@ -131,17 +176,19 @@ trace_kernel(const DevTracePlan* __restrict__ plan_g, const double2* __restrict_
             }
           }
 #pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            Rout[(4 * la + i) + 16 * (2 * lb)] = acc[i][0];
-            Rout[(4 * la + i) + 16 * (2 * lb + 1)] = acc[i][1];
-          }
+          for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+              const int o = (la + 4 * i) + 16 * (lb + 8 * j);
+              Rout[o + (o >> 4)] = acc[i][j];
+            }
         } else if (nOut >= 32) {
           const int mA = nA - 1, shA = 31 - __clz(nA);
           for (int o = lane; o < nOut; o += 32) {
             const int rA = s.baseR[o & mA], wB = s.baseW[o >> shA];
             double2 v = make_double2(0.0, 0.0);
             for (int g = 0; g < nC; ++g) cfma(v, Rin[rA + s.offR[g]], Wv[wB + s.offW[g]]);
-            Rout[o] = v;
+            Rout[o + (o >> 4)] = v;
           }
         } else {
           // fewer outputs than lanes: P = 32 / nOut lanes share one output, each sums every P-th closed label,
@@ -155,7 +202,7 @@ trace_kernel(const DevTracePlan* __restrict__ plan_g, const double2* __restrict_
             const double2 u = shfl_xor2(v, m);
             v.x += u.x; v.y += u.y;
           }
-          if (part == 0) Rout[o] = v;
+          if (part == 0) Rout[o + (o >> 4)] = v;
           if (nOut == 1) last = v;
         }
         __syncwarp();
@@ -165,7 +212,11 @@ trace_kernel(const DevTracePlan* __restrict__ plan_g, const double2* __restrict_
     }
     if (lane == 0) out[smp] = total;
     __syncwarp();
-    stage ^= 1;
+    if (stages == 2) {
+      stage ^= 1;
+    } else if (nxt < n_sample) {
+      request_sample(vbuf, V + nxt * n * 256, n, lane);
+    }
   }
 }
 
@@ -195,7 +246,8 @@ struct no_trace_plan {
   DevTracePlan* d_plan;
   int warps;        // warps per CTA
   int n_sm;
-  size_t smem;
+  int stages;       // vertex buffers per warp: 2 = the next sample's copy runs under this sample's arithmetic
+  int path;         // 0 vector FP64 tiles, 1 FP64 tensor cores for the 16 x 16 x 16 steps
 };
 
 extern "C" {
@@ -220,12 +272,16 @@ int no_trace_init(no_trace_plan** out, int n_vertex, const int* topo, int device
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, device);
   if (e != cudaSuccess) { delete p; return trace_cuda_fail(e, "cudaDeviceGetAttribute"); }
   // one CTA per SM, as many warps (samples in flight) as its shared memory holds
+  p->stages = kTrStagesDefault;
+  p->path = kTrPathDefault;
+  if (const char* e = getenv("NO3N_TRACE_STAGES")) { const int v = atoi(e); if (v == 1 || v == 2) p->stages = v; }   // tuning knobs
+  if (const char* e = getenv("NO3N_TRACE_PATH")) { const int v = atoi(e); if (v == 0 || v == 1) p->path = v; }
   const size_t avail = (size_t)smem_optin - trace_plan_bytes(n_vertex) - 128;
-  int warps = (int)(avail / trace_warp_bytes(n_vertex));
+  int warps = (int)(avail / trace_warp_bytes(n_vertex, p->stages));
   if (warps > 16) warps = 16;
+  if (const char* e = getenv("NO3N_TRACE_WARPS")) { const int v = atoi(e); if (v >= 1 && v < warps) warps = v; }
   if (warps < 1) { delete p; return NO_ERR_INVALID; }
   p->warps = warps;
-  p->smem = trace_plan_bytes(n_vertex) + (size_t)warps * trace_warp_bytes(n_vertex);
   e = cudaFuncSetAttribute((const void*)trace_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);
   if (e != cudaSuccess) { delete p; return trace_cuda_fail(e, "cudaFuncSetAttribute(smem)"); }
   DevTracePlan hp;
@@ -257,9 +313,10 @@ int no_trace_eval(const no_trace_plan* p, const double* d_vertices, long long n_
   } else {
     blocks = p->n_sm;
   }
-  const size_t smem = trace_plan_bytes(p->plan.n_vertex) + (size_t)warps * trace_warp_bytes(p->plan.n_vertex);
+  const size_t smem = trace_plan_bytes(p->plan.n_vertex) + (size_t)warps * trace_warp_bytes(p->plan.n_vertex, p->stages);
   trace_kernel<<<(unsigned)blocks, warps * 32, smem, static_cast<cudaStream_t>(cuda_stream)>>>(
-      p->d_plan, reinterpret_cast<const double2*>(d_vertices), n_sample, reinterpret_cast<double2*>(d_out));
+      p->d_plan, reinterpret_cast<const double2*>(d_vertices), n_sample, reinterpret_cast<double2*>(d_out), p->stages,
+      p->path);
   const cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return trace_cuda_fail(e, "trace_kernel launch");
   return NO_OK;

@@ -15,13 +15,14 @@
 //                                                b: labels of the lines the vertex opens      (nB = 4^new)
 // which turns the exponential label sum (4^(2n) terms) into n products of at most 16 x 16 x 16.  Topologies whose
 // frontier would exceed four lines are handled by "slicing": the labels of up to kMaxSlice lines are fixed in an outer
-// loop (a line that starts and ends on the same vertex is always sliced).  The order of the vertices and the sliced
+// loop; a line that starts and ends on the same vertex is summed inside that vertex's step.  The order of the vertices and the sliced
 // lines are chosen here, on the host, by exhaustive search for the fewest complex multiply-adds.
 //
 // All index arithmetic of the kernel is tabulated here: with x the label of a line attached to slot q of a vertex
 // (q = 0, 1: outgoing 1, 2; q = 2, 3: incoming 1, 2) the element offset inside the 16 x 16 matrix of include/no.h
 // (row = outgoing pair, column = incoming pair, pair index 8 s1 + 4 s2 + 2 t1 + t2) is the sum over the four slots of
-// slot_off(q, x); offsets into R are sums of label * 4^(position of the line in the open list).
+// slot_off(q, x); offsets into R are sums of label * 4^(position of the line in the open list); the new partial result
+// is stored at index a + nA b (kept labels, then opened labels).
 #pragma once
 
 #include <stdint.h>
@@ -37,13 +38,21 @@ constexpr int kTrMaxOpen = 4;        // open lines of the partial result: 4^4 = 
 constexpr int kTrMaxSlice = 3;       // lines whose labels are fixed in the outer loop
 constexpr int kTrTab = 256;
 
+// Shared-memory layouts (complex elements).  Both the vertex matrices and the partial result are held as 16 rows of
+// kTrRow = 17 elements (one element of padding per row): consecutive rows start one 16-byte bank group apart, so a
+// warp access whose lanes differ in row AND column bits spreads over all banks.  Padding is additive on offsets
+// that occupy disjoint digits, so every table below holds padded offsets and the kernel only adds them.
+constexpr int kTrRow = 17;
+constexpr int kTrMat = 16 * kTrRow;  // elements of one padded 16 x 16 matrix
+inline int tr_pad(int idx) { return idx + (idx >> 4); }   // canonical index (16 row + col) -> padded offset
+
 inline int slot_off(int slot, int x) {
   const int s = x >> 1, t = x & 1;
   switch (slot) {
-    case 0: return 16 * (8 * s + 2 * t);    // outgoing 1: row bits s1, t1
-    case 1: return 16 * (4 * s + t);        // outgoing 2: row bits s2, t2
-    case 2: return 8 * s + 2 * t;           // incoming 1: column bits
-    default: return 4 * s + t;              // incoming 2
+    case 0: return kTrRow * (8 * s + 2 * t);    // outgoing 1: row bits s1, t1
+    case 1: return kTrRow * (4 * s + t);        // outgoing 2: row bits s2, t2
+    case 2: return 8 * s + 2 * t;               // incoming 1: column bits
+    default: return 4 * s + t;                  // incoming 2
   }
 }
 
@@ -51,7 +60,7 @@ inline int slot_off(int slot, int x) {
 struct TraceStep {
   int vertex;                 // which vertex matrix of the sample
   int nA, nB, nC;             // kept, opened, closed label combinations (powers of 4); nA * nB <= 256
-  uint16_t baseR[kTrTab];     // [a]  offset of the kept labels in R
+  uint16_t baseR[kTrTab];     // [a]  offset of the kept labels in R (all offsets padded, see kTrRow)
   uint16_t offR[kTrTab];      // [g]  offset of the closed labels in R
   uint16_t baseW[kTrTab];     // [b]  offset of the opened labels in the vertex matrix
   uint16_t offW[kTrTab];      // [g]  offset of the closed labels in the vertex matrix
@@ -92,21 +101,20 @@ inline long long simulate(int n, const int* topo, const int* order, unsigned sli
   *max_open = 0;
   for (int k = 0; k < n; ++k) {
     const int v = order[k];
-    int closed = 0, opened = 0;
+    int closed = 0, opened = 0, self = 0;
     for (int q = 0; q < 4; ++q) {
       const int l = topo[4 * v + q];
       if (sliced_mask >> l & 1) continue;
+      bool twice = false;                      // a line that leaves and enters this vertex: summed inside the step
+      for (int r = 0; r < 4; ++r) twice |= r != q && topo[4 * v + r] == l;
+      if (twice) { self += q < 2; continue; }
       bool is_open = false;
       for (int j = 0; j < n_open; ++j) is_open |= open[j] == l;
       if (is_open) ++closed; else ++opened;
     }
-    // a line opened twice by the same vertex is a self-loop that was not sliced
-    for (int q = 0; q < 4; ++q)
-      for (int r = q + 1; r < 4; ++r)
-        if (topo[4 * v + q] == topo[4 * v + r] && !(sliced_mask >> topo[4 * v + q] & 1)) return -1;
     const int kept = n_open - closed;
     if (kept + opened > kTrMaxOpen) return -1;
-    cost += (1LL << (2 * kept)) * (1LL << (2 * opened)) * (1LL << (2 * closed));
+    cost += (1LL << (2 * kept)) * (1LL << (2 * opened)) * (1LL << (2 * (closed + self)));
     // new frontier: kept lines in their old order, then the opened lines in slot order
     int next[kTrMaxLines], m = 0;
     for (int j = 0; j < n_open; ++j) {
@@ -117,9 +125,10 @@ inline long long simulate(int n, const int* topo, const int* order, unsigned sli
     for (int q = 0; q < 4; ++q) {
       const int l = topo[4 * v + q];
       if (sliced_mask >> l & 1) continue;
-      bool was_open = false;
+      bool twice = false, was_open = false;
+      for (int r = 0; r < 4; ++r) twice |= r != q && topo[4 * v + r] == l;
       for (int j = 0; j < n_open; ++j) was_open |= open[j] == l;
-      if (!was_open) next[m++] = l;
+      if (!was_open && !twice) next[m++] = l;
     }
     n_open = m;
     for (int j = 0; j < m; ++j) open[j] = next[j];
@@ -187,17 +196,25 @@ inline int build_trace_plan(int n, const int* topo, TracePlan& plan) {
     TraceStep& s = plan.steps[k];
     s.vertex = v;
     int kept_pos[kTrMaxOpen], n_kept = 0;            // positions (in the old open list) of the lines that stay open
-    int closed_pos[4], closed_slot[4], n_closed = 0;  // closed lines: position in the old list, slot of this vertex
+    // closed lines: position in the old list (-1: a line that leaves and enters this vertex, it has no index in R),
+    // slot of this vertex (and the second slot of such a self-loop, else -1)
+    int closed_pos[4], closed_slot[4], closed_slot2[4], n_closed = 0;
     int opened_slot[4], opened_line[4], n_opened = 0;
     for (int j = 0; j < n_open; ++j) {
       int slot = -1;
       for (int q = 0; q < 4; ++q) if (topo[4 * v + q] == open[j]) slot = q;
       if (slot < 0) kept_pos[n_kept++] = j;
-      else { closed_pos[n_closed] = j; closed_slot[n_closed++] = slot; }
+      else { closed_pos[n_closed] = j; closed_slot[n_closed] = slot; closed_slot2[n_closed++] = -1; }
     }
     for (int q = 0; q < 4; ++q) {
       const int l = topo[4 * v + q];
       if (best_mask >> l & 1) continue;
+      int twin = -1;
+      for (int r = 0; r < 4; ++r) if (r != q && topo[4 * v + r] == l) twin = r;
+      if (twin >= 0) {
+        if (q < twin) { closed_pos[n_closed] = -1; closed_slot[n_closed] = q; closed_slot2[n_closed++] = twin; }
+        continue;
+      }
       bool was_open = false;
       for (int j = 0; j < n_open; ++j) was_open |= open[j] == l;
       if (!was_open) { opened_slot[n_opened] = q; opened_line[n_opened++] = l; }
@@ -208,16 +225,17 @@ inline int build_trace_plan(int n, const int* topo, TracePlan& plan) {
     for (int a = 0; a < kTrTab; ++a) {
       int off = 0;
       for (int j = 0; j < n_kept; ++j) off += ((a >> (2 * j)) & 3) << (2 * kept_pos[j]);
-      s.baseR[a] = (uint16_t)(a < s.nA ? off : 0);
+      s.baseR[a] = (uint16_t)(a < s.nA ? tr_pad(off) : 0);
     }
     for (int g = 0; g < kTrTab; ++g) {
       int offr = 0, offw = 0;
       for (int j = 0; j < n_closed; ++j) {
         const int x = (g >> (2 * j)) & 3;
-        offr += x << (2 * closed_pos[j]);
+        if (closed_pos[j] >= 0) offr += x << (2 * closed_pos[j]);
         offw += slot_off(closed_slot[j], x);
+        if (closed_slot2[j] >= 0) offw += slot_off(closed_slot2[j], x);
       }
-      s.offR[g] = (uint16_t)(g < s.nC ? offr : 0);
+      s.offR[g] = (uint16_t)(g < s.nC ? tr_pad(offr) : 0);
       s.offW[g] = (uint16_t)(g < s.nC ? offw : 0);
     }
     for (int b = 0; b < kTrTab; ++b) {

@@ -17,8 +17,8 @@ def lib():
     return binding.load()
 
 
-def declared_symbols():
-    text = open(os.path.join(ROOT, "include", "no.h")).read()
+def declared_symbols(header="no.h"):
+    text = open(os.path.join(ROOT, "include", header)).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(no_[a-z0-9_]+)\s*\(", text)))
 
@@ -28,10 +28,11 @@ def test_header_declares_the_boundary():
     for required in ("no_init", "no_eval", "no_free"):          # north_star (a)
         assert required in syms
     assert set(syms) == set(binding.EXPORTS)
+    assert set(declared_symbols("no_trace.h")) == set(binding.TRACE_EXPORTS)
 
 
 def test_every_declared_symbol_is_exported(lib):
-    for name in declared_symbols():
+    for name in declared_symbols() + declared_symbols("no_trace.h"):
         assert hasattr(lib, name), name
 
 
@@ -59,6 +60,24 @@ def test_error_strings_and_null_handling(lib):
     assert lib.no_init(None, None) == binding.NO_ERR_INVALID
     assert lib.no_eval(None, None, 0, None, None) == binding.NO_ERR_INVALID
     assert lib.no_evals_per_cfg(None) == 0
+    assert lib.no_trace_free(None) == binding.NO_OK
+    assert lib.no_trace_init(None, 2, None, 0) == binding.NO_ERR_INVALID
+    assert lib.no_trace_eval(None, None, 0, None, None) == binding.NO_ERR_INVALID
+    assert lib.no_trace_info(None, None, None, None, None, None) == binding.NO_ERR_INVALID
+
+
+def test_malformed_trace_topologies_are_rejected_before_any_cuda_call(lib):
+    import numpy as np
+    for topo in ([[0, 1, 0, 0]],                        # a line entering twice
+                 [[0, 1, 2, 3], [2, 3, 0, 4]],          # id out of range
+                 [[0, 1, 2, 3], [2, 2, 0, 1]]):         # a line leaving twice
+        t = np.array(topo, dtype=np.int32)
+        h = ctypes.c_void_p()
+        assert lib.no_trace_init(ctypes.byref(h), t.shape[0], ctypes.c_void_p(t.ctypes.data), 0) == binding.NO_ERR_INVALID
+        assert not h.value
+    t = np.zeros((7, 4), dtype=np.int32)
+    h = ctypes.c_void_p()
+    assert lib.no_trace_init(ctypes.byref(h), 7, ctypes.c_void_p(t.ctypes.data), 0) == binding.NO_ERR_INVALID
 
 
 GOOD = dict(kf_n=1.0, kf_p=0.0, c1=-0.81, c3=-3.2, c4=0.0, cD=1.0, cE=-0.5, gA=1.27, fpi=92.4, mpi=138.04,
@@ -95,4 +114,4 @@ def test_product_never_imports_the_oracle():
             if f.endswith((".py", ".h", ".cuh", ".cu", ".cpp")):
                 src = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(from|import)\s+oracle", src, flags=re.M), f
-                assert "no_oracle" not in src and "liboracle" not in src, f
+                assert "no_oracle" not in src and "liboracle" not in src and "trace_oracle" not in src, f
