@@ -110,78 +110,105 @@ trace_kernel(const DevTracePlan* __restrict__ plan_g, const double2* __restrict_
       __syncwarp();
       for (int k = 0; k < n; ++k) {
         const TraceStep& s = steps[k];
+        if (s.skip) continue;                           // folded into a neighbouring step (warp uniform)
         const double2* Wv = W + s.vertex * kTrMat + s.sliceW[it];
         const int nA = s.nA, nB = s.nB, nC = s.nC, nOut = nA * nB;
-        if (nA == 16 && nB == 16 && nC == 16 && path == 1) {
-          // 16 x 16 x 16 complex product on the FP64 tensor cores: four real products per (8 x 8 tile, k-step of 4),
-          // Re = Re Re - Im Im, Im = Re Im + Im Re; fragments come straight from the tabulated offsets
-          const int r = lane >> 2, c = lane & 3;
-          int aR[2], bW[2], gR[4], gW[4];
+        if (nA == 16 && nB == 16 && nC == 16) {
+          // R of this step: the partial result, or (first vertex folded in) the first vertex's matrix itself
+          const double2* Rs = s.r_vertex >= 0 ? W + s.r_vertex * kTrMat + steps[0].sliceW[it] : Rin;
+          // last vertex folded in: it closes all four lines, T = sum_o R'[o] W_last[lastW[o]]
+          const double2* Wl = s.fuse_last ? W + steps[n - 1].vertex * kTrMat + steps[n - 1].sliceW[it] : nullptr;
+          double2 dot = make_double2(0.0, 0.0);
+          if (path == 1) {
+            // 16 x 16 x 16 complex product on the FP64 tensor cores: four real products per (8 x 8 tile, k-step of 4),
+            // Re = Re Re - Im Im, Im = Re Im + Im Re; fragments come straight from the tabulated offsets
+            const int r = lane >> 2, c = lane & 3;
+            int aR[2], bW[2], gR[4], gW[4];
 #pragma unroll
-          for (int t = 0; t < 2; ++t) { aR[t] = s.baseR[8 * t + r]; bW[t] = s.baseW[8 * t + r]; }
+            for (int t = 0; t < 2; ++t) { aR[t] = s.baseR[8 * t + r]; bW[t] = s.baseW[8 * t + r]; }
 #pragma unroll
-          for (int ks = 0; ks < 4; ++ks) { gR[ks] = s.offR[4 * ks + c]; gW[ks] = s.offW[4 * ks + c]; }
-          double cre[2][2][2], cim[2][2][2];
-#pragma unroll
-          for (int mt = 0; mt < 2; ++mt)
-#pragma unroll
-            for (int nt = 0; nt < 2; ++nt) cre[mt][nt][0] = cre[mt][nt][1] = cim[mt][nt][0] = cim[mt][nt][1] = 0.0;
-#pragma unroll
-          for (int ks = 0; ks < 4; ++ks) {
-            double2 A[2], B[2];
-#pragma unroll
-            for (int t = 0; t < 2; ++t) { A[t] = Rin[aR[t] + gR[ks]]; B[t] = Wv[gW[ks] + bW[t]]; }
+            for (int ks = 0; ks < 4; ++ks) { gR[ks] = s.offR[4 * ks + c]; gW[ks] = s.offW[4 * ks + c]; }
+            double cre[2][2][2], cim[2][2][2];
 #pragma unroll
             for (int mt = 0; mt < 2; ++mt)
 #pragma unroll
-              for (int nt = 0; nt < 2; ++nt) {
-                dmma884(cre[mt][nt][0], cre[mt][nt][1], A[mt].x, B[nt].x);
-                dmma884(cim[mt][nt][0], cim[mt][nt][1], A[mt].x, B[nt].y);
-                dmma884(cre[mt][nt][0], cre[mt][nt][1], -A[mt].y, B[nt].y);
-                dmma884(cim[mt][nt][0], cim[mt][nt][1], A[mt].y, B[nt].x);
-              }
-          }
+              for (int nt = 0; nt < 2; ++nt) cre[mt][nt][0] = cre[mt][nt][1] = cim[mt][nt][0] = cim[mt][nt][1] = 0.0;
 #pragma unroll
-          for (int mt = 0; mt < 2; ++mt)
+            for (int ks = 0; ks < 4; ++ks) {
+              double2 A[2], B[2];
 #pragma unroll
-            for (int nt = 0; nt < 2; ++nt)
+              for (int t = 0; t < 2; ++t) { A[t] = Rs[aR[t] + gR[ks]]; B[t] = Wv[gW[ks] + bW[t]]; }
+              // one term over all four tiles before the next: dependent DMMAs are eight apart
 #pragma unroll
-              for (int e = 0; e < 2; ++e) {
-                const int o = (8 * mt + r) + 16 * (8 * nt + 2 * c + e);
-                Rout[o + (o >> 4)] = make_double2(cre[mt][nt][e], cim[mt][nt][e]);
-              }
-        } else if (nA == 16 && nB == 16 && nC == 16) {
-          // register-tiled 16 x 16 x 16 complex product: lane (la, lb) owns a = la + 4 i, b = lb + 8 j
-          const int la = lane >> 3, lb = lane & 7;
-          int rA[4], wB[2];
+              for (int mt = 0; mt < 2; ++mt)
 #pragma unroll
-          for (int i = 0; i < 4; ++i) rA[i] = s.baseR[la + 4 * i];
+                for (int nt = 0; nt < 2; ++nt) dmma884(cre[mt][nt][0], cre[mt][nt][1], A[mt].x, B[nt].x);
 #pragma unroll
-          for (int j = 0; j < 2; ++j) wB[j] = s.baseW[lb + 8 * j];
-          double2 acc[4][2];
+              for (int mt = 0; mt < 2; ++mt)
 #pragma unroll
-          for (int i = 0; i < 4; ++i) acc[i][0] = acc[i][1] = make_double2(0.0, 0.0);
+                for (int nt = 0; nt < 2; ++nt) dmma884(cim[mt][nt][0], cim[mt][nt][1], A[mt].x, B[nt].y);
+#pragma unroll
+              for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+                for (int nt = 0; nt < 2; ++nt) dmma884(cre[mt][nt][0], cre[mt][nt][1], -A[mt].y, B[nt].y);
+#pragma unroll
+              for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+                for (int nt = 0; nt < 2; ++nt) dmma884(cim[mt][nt][0], cim[mt][nt][1], A[mt].y, B[nt].x);
+            }
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+              for (int nt = 0; nt < 2; ++nt)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                  const int o = (8 * mt + r) + 16 * (8 * nt + 2 * c + e);
+                  const double2 v = make_double2(cre[mt][nt][e], cim[mt][nt][e]);
+                  if (Wl) cfma(dot, v, Wl[s.lastW[o]]);
+                  else Rout[o + (o >> 4)] = v;
+                }
+          } else {
+            // vector FP64 variant: lane (la, lb) owns the 4 x 2 tile a = la + 4 i, b = lb + 8 j
+            const int la = lane >> 3, lb = lane & 7;
+            int rA[4], wB[2];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) rA[i] = s.baseR[la + 4 * i];
+#pragma unroll
+            for (int j = 0; j < 2; ++j) wB[j] = s.baseW[lb + 8 * j];
+            double2 acc[4][2];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) acc[i][0] = acc[i][1] = make_double2(0.0, 0.0);
 #pragma unroll 4
-          for (int g = 0; g < 16; ++g) {
-            const int oR = s.offR[g], oW = s.offW[g];
-            double2 r[4], w[2];
+            for (int g = 0; g < 16; ++g) {
+              const int oR = s.offR[g], oW = s.offW[g];
+              double2 rr[4], w[2];
 #pragma unroll
-            for (int i = 0; i < 4; ++i) r[i] = Rin[rA[i] + oR];
+              for (int i = 0; i < 4; ++i) rr[i] = Rs[rA[i] + oR];
 #pragma unroll
-            for (int j = 0; j < 2; ++j) w[j] = Wv[wB[j] + oW];
+              for (int j = 0; j < 2; ++j) w[j] = Wv[wB[j] + oW];
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
-              cfma(acc[i][0], r[i], w[0]);
-              cfma(acc[i][1], r[i], w[1]);
+              for (int i = 0; i < 4; ++i) {
+                cfma(acc[i][0], rr[i], w[0]);
+                cfma(acc[i][1], rr[i], w[1]);
+              }
             }
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+              for (int j = 0; j < 2; ++j) {
+                const int o = (la + 4 * i) + 16 * (lb + 8 * j);
+                if (Wl) cfma(dot, acc[i][j], Wl[s.lastW[o]]);
+                else Rout[o + (o >> 4)] = acc[i][j];
+              }
           }
+          if (Wl) {                                     // add the 32 partial dot products (fixed butterfly)
 #pragma unroll
-          for (int i = 0; i < 4; ++i)
-#pragma unroll
-            for (int j = 0; j < 2; ++j) {
-              const int o = (la + 4 * i) + 16 * (lb + 8 * j);
-              Rout[o + (o >> 4)] = acc[i][j];
+            for (int m = 16; m > 0; m >>= 1) {
+              const double2 u = shfl_xor2(dot, m);
+              dot.x += u.x; dot.y += u.y;
             }
+            last = dot;
+          }
         } else if (nOut >= 32) {
           const int mA = nA - 1, shA = 31 - __clz(nA);
           for (int o = lane; o < nOut; o += 32) {

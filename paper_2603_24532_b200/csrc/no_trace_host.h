@@ -60,11 +60,17 @@ inline int slot_off(int slot, int x) {
 struct TraceStep {
   int vertex;                 // which vertex matrix of the sample
   int nA, nB, nC;             // kept, opened, closed label combinations (powers of 4); nA * nB <= 256
+  int skip;                   // 1: this step only copies its vertex into R and the next step reads the vertex directly
+  int r_vertex;               // >= 0: R of this step IS that vertex matrix (baseR, offR hold offsets into it); -1: R
+  int fuse_last;              // 1: the next (last) step closes all four lines: its sum is folded into this step,
+                              //    lastW[o] = offset in the LAST vertex of the element that multiplies R'[o]
+  int pad_;
   uint16_t baseR[kTrTab];     // [a]  offset of the kept labels in R (all offsets padded, see kTrRow)
   uint16_t offR[kTrTab];      // [g]  offset of the closed labels in R
   uint16_t baseW[kTrTab];     // [b]  offset of the opened labels in the vertex matrix
   uint16_t offW[kTrTab];      // [g]  offset of the closed labels in the vertex matrix
   uint16_t sliceW[64];        // [outer iteration] offset of the sliced labels in the vertex matrix
+  uint16_t lastW[kTrTab];     // [o = a + 16 b] see fuse_last
 };
 
 struct TracePlan {
@@ -257,7 +263,35 @@ inline int build_trace_plan(int n, const int* topo, TracePlan& plan) {
     n_open = m;
     for (int j = 0; j < m; ++j) open[j] = next[j];
   }
-  return n_open == 0 ? 0 : 1;
+  if (n_open != 0) return 1;
+
+  // fusions around the 16 x 16 x 16 steps (what ladders and rings consist of)
+  for (int k = 0; k < n; ++k) { plan.steps[k].skip = 0; plan.steps[k].r_vertex = -1; plan.steps[k].fuse_last = 0; }
+  auto is_big = [&](int k) { return plan.steps[k].nA == 16 && plan.steps[k].nB == 16 && plan.steps[k].nC == 16; };
+  // (1) first vertex: step 0 would copy its 256 entries into R (R[pad(b)] = W_0[baseW_0[b]], b = canonical index of
+  //     the four opened lines).  Offsets are additive over disjoint digits, so step 1 can address the vertex itself.
+  if (n >= 3 && plan.steps[0].nA == 1 && plan.steps[0].nC == 1 && plan.steps[0].nB == 256 && is_big(1)) {
+    TraceStep& s0 = plan.steps[0];
+    TraceStep& s1 = plan.steps[1];
+    auto unpad = [](int p) { return p - p / kTrRow; };      // padded offset -> canonical index
+    for (int a = 0; a < 16; ++a) s1.baseR[a] = s0.baseW[unpad(s1.baseR[a])];
+    for (int g = 0; g < 16; ++g) s1.offR[g] = s0.baseW[unpad(s1.offR[g])];
+    s1.r_vertex = s0.vertex;
+    s0.skip = 1;
+  }
+  // (2) last vertex: it closes all four open lines, T = sum_o R'[o] W_last[offW_last[g(o)]] with g(o) the closed-label
+  //     combination whose R offset is o: folded into the step that produces R'.
+  if (n >= 3 && plan.steps[n - 1].nA == 1 && plan.steps[n - 1].nB == 1 && plan.steps[n - 1].nC == 256 && is_big(n - 2)) {
+    TraceStep& sl = plan.steps[n - 1];
+    TraceStep& sp = plan.steps[n - 2];
+    for (int g = 0; g < 256; ++g) {
+      const int o = sl.offR[g] - sl.offR[g] / kTrRow;          // canonical index of R'
+      sp.lastW[o] = sl.offW[g];
+    }
+    sp.fuse_last = 1;
+    sl.skip = 1;
+  }
+  return 0;
 }
 
 }  // namespace no3n

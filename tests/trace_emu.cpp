@@ -43,14 +43,23 @@ int trace_emu_eval(int n, const int* topo, const double* V, long long n_sample, 
       R[0] = 1.0;
       for (int k = 0; k < n; ++k) {
         const TraceStep& s = plan.steps[k];
+        if (s.skip) continue;                         // folded into a neighbouring step
         const cplx* Wv = W.data() + s.vertex * kTrMat + s.sliceW[it];
+        const cplx* Rsrc = s.r_vertex >= 0 ? W.data() + s.r_vertex * kTrMat + plan.steps[0].sliceW[it] : R.data();
         for (int b = 0; b < s.nB; ++b)
           for (int a = 0; a < s.nA; ++a) {
             cplx v = 0;
-            for (int g = 0; g < s.nC; ++g) v += R[s.baseR[a] + s.offR[g]] * Wv[s.baseW[b] + s.offW[g]];
+            for (int g = 0; g < s.nC; ++g) v += Rsrc[s.baseR[a] + s.offR[g]] * Wv[s.baseW[b] + s.offW[g]];
             Rn[tr_pad(a + s.nA * b)] = v;
           }
         R.swap(Rn);
+        if (s.fuse_last) {                            // the last vertex closes everything: one dot product
+          const TraceStep& sl = plan.steps[n - 1];
+          const cplx* Wl = W.data() + sl.vertex * kTrMat + sl.sliceW[it];
+          cplx t = 0;
+          for (int o = 0; o < 256; ++o) t += R[tr_pad(o)] * Wl[s.lastW[o]];
+          R[0] = t;
+        }
       }
       total += R[0];
     }
