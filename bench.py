@@ -241,6 +241,49 @@ def timed_steps(dw, stream, dev, flush, steps, warmup, barrier):
     return [a.elapsed_time(b) for a, b in ev]
 
 
+def small_batch_rates(dw, dev):
+    """Small transactions (cfg1: 256 configurations per launch, the paper's per-diagram transaction size):
+    launches back to back on one stream, and the same launches spread over 4 streams and replayed as ONE CUDA graph
+    (many host threads sharing the GPU through streams, without the host-side launch cost)."""
+    import torch
+    h, c, o, r = dw.handles[0], dw.d_cfg[0], dw.d_out[0], dw.runs[0]
+    evals = dw.binding.no_evals_per_cfg(h) * r.n_cfg
+    reps = 64
+    main = torch.cuda.current_stream(dev)
+    outs = [torch.empty_like(o) for _ in range(4)]
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for _ in range(8):
+        dw.binding.no_eval(h, c.data_ptr(), r.n_cfg, o.data_ptr(), main.cuda_stream)
+    a.record(main)
+    for _ in range(reps):
+        dw.binding.no_eval(h, c.data_ptr(), r.n_cfg, o.data_ptr(), main.cuda_stream)
+    b.record(main)
+    torch.cuda.synchronize(dev)
+    serial = evals * reps / (a.elapsed_time(b) * 1e-3)
+    streams = [torch.cuda.Stream(dev) for _ in range(4)]
+    g = torch.cuda.CUDAGraph()
+    cap = torch.cuda.Stream(dev)
+    with torch.cuda.stream(cap):
+        with torch.cuda.graph(g, stream=cap):
+            for k in range(reps):
+                st = streams[k % 4]
+                st.wait_stream(cap)
+                dw.binding.no_eval(h, c.data_ptr(), r.n_cfg, outs[k % 4].data_ptr(), st.cuda_stream)
+            for st in streams:
+                cap.wait_stream(st)
+    for _ in range(3):
+        g.replay()
+    torch.cuda.synchronize(dev)
+    a.record(main)
+    for _ in range(4):
+        g.replay()
+    b.record(main)
+    torch.cuda.synchronize(dev)
+    graph = evals * reps * 4 / (a.elapsed_time(b) * 1e-3)
+    assert torch.equal(outs[0], o)
+    return {"back_to_back_one_stream_evals_per_s": serial, "graph_4_streams_evals_per_s": graph, "launches": reps}
+
+
 def run_b200(args, workload):
     import torch
     import torch.distributed as dist
@@ -345,6 +388,7 @@ def run_b200(args, workload):
                 "kernel": "no3n::no3n_kernel", "avg_launch_ms": launch_ms, "launches_per_step": len(runs),
                 "algorithmic_bytes_per_launch": int(sum(r.n_cfg * (72 + 4096) for r in runs) / len(runs)),
                 "kernel_info": info}
+    small = small_batch_rates(dw, dev) if workload.name == "cfg1" and world == 1 else None
     dw.close()
 
     # ---- the other BASELINE configs, a few steps each in the same run (not the headline) ----
@@ -361,7 +405,8 @@ def run_b200(args, workload):
             ms = timed_steps(d2, stream, dev, flush, 3, 3, barrier)
             rate = wl.evals * len(ms) / (sum(ms) * 1e-3)
             fl = d2.flops_step / wl.evals
-            per_config[name] = {"evals_per_s": rate, "cfg_per_s": wl.n_cfg * len(ms) / (sum(ms) * 1e-3),
+            extra = small_batch_rates(d2, dev) if name == "cfg1" else None
+            per_config[name] = {"small_transactions": extra, "evals_per_s": rate, "cfg_per_s": wl.n_cfg * len(ms) / (sum(ms) * 1e-3),
                                 "ms_per_step": sum(ms) / len(ms), "steps": len(ms), "flops_per_eval": fl,
                                 "frac": rate * fl / 1e12 / FP64_PEAK_NOMINAL_TFLOPS}
             d2.close()
@@ -384,7 +429,7 @@ def run_b200(args, workload):
                        "cfg_per_s": world * workload.n_cfg * args.steps / t_dev,
                        "l2": "256 MiB buffer rewritten between timed steps (L2 flush); the kernel is ALU bound",
                        "parallelism": "replicas only: every rank integrates the whole workload",
-                       "per_config": per_config},
+                       "per_config": per_config, "small_transactions": small},
             "clocks": clocks, "e2e": e2e, "e2e_full_matrices": e2e_full, "gpu_launches": n_launch, "roofline": roofline, "cpu_baseline": cpu,
             "wall_s_timed_region": t_wall}
     print(json.dumps(line), flush=True)
@@ -568,7 +613,8 @@ def run_trace(args):
     binding.load()
     dev = torch.device("cuda", local)
     stream = torch.cuda.current_stream(dev)
-    plan = binding.no_trace_init(topo, local)
+    # the vertices are charge conserving (as no_eval output is): the plan skips the structurally zero blocks
+    plan = binding.no_trace_init(topo, local, binding.NO_TRACE_CHARGE_CONSERVING)
     info = binding.no_trace_info(plan, n)
     V = TW.vertex_matrices(n_sample, n, seed=TRACE_BENCH["seed"])
     d_V = torch.from_numpy(V).to(dev)
@@ -599,10 +645,26 @@ def run_trace(args):
     step_ms = [a.elapsed_time(b) for a, b in ev]
     t_dev = replicas.max_over_ranks(sum(step_ms) * 1e-3, dev)
     value = replicas.whole_job_rate(n_sample, steps, t_dev)
+    # the same launch with a plan for arbitrary (dense) vertex matrices, for comparison
+    plan_d = binding.no_trace_init(topo, local, 0)
+    for _ in range(3):
+        binding.no_trace_eval(plan_d, d_V.data_ptr(), n_sample, d_out.data_ptr(), stream.cuda_stream)
+    ed = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(5)]
+    for a, b in ed:
+        flush.zero_()
+        a.record(stream)
+        binding.no_trace_eval(plan_d, d_V.data_ptr(), n_sample, d_out.data_ptr(), stream.cuda_stream)
+        b.record(stream)
+    torch.cuda.synchronize(dev)
+    dense_rate = n_sample * len(ed) / (sum(a.elapsed_time(b) for a, b in ed) * 1e-3)
+    binding.no_trace_free(plan_d)
     bytes_step = n_sample * (n * 4096 + 16)
     peak, peak_src = hbm_peak_gbs()
     achieved = bytes_step * steps / (sum(step_ms) * 1e-3) / 1e9
-    flops_step = 8.0 * info["cmacs_per_sample"] * n_sample
+    # FP64 work actually issued: 8x8x4 tensor-core products (512 flops each) of the 16x16x16 steps + the folded last
+    # vertex (256 complex multiply-adds)
+    flops_sample = 512.0 * info["tensor_products_per_sample"] + 8.0 * 256
+    flops_step = flops_sample * n_sample
 
     # ---- end to end: HOST momentum configurations -> no_eval (the vertices are produced on the device, where the
     # trace consumes them: the paper's pipeline) -> no_trace_eval -> HOST traces ----
@@ -676,7 +738,9 @@ def run_trace(args):
                      "bytes_per_sample": n * 4096 + 16, "kernel": "trace_kernel", "avg_launch_ms": sum(step_ms) / steps,
                      "fp64_tflops": flops_step * steps / (sum(step_ms) * 1e-3) / 1e12,
                      "fp64_frac_of_nominal": flops_step * steps / (sum(step_ms) * 1e-3) / 1e12 / FP64_PEAK_NOMINAL_TFLOPS,
-                     "flops_per_sample": 8.0 * info["cmacs_per_sample"]},
+                     "flops_per_sample": flops_sample,
+                     "dense_plan_samples_per_s": dense_rate,
+                     "dense_plan_flops_per_sample": 8.0 * info["cmacs_per_sample"]},
         "cpu_baseline": cpu}), flush=True)
 
 

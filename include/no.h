@@ -206,6 +206,13 @@ long long no_evals_per_cfg(const no_handle *h);
  * FP64 peak next to the nominal one. */
 int no_probe_fp64_peak(int device, int millis, double *tflops, int *n_sm, void *cuda_stream);
 
+/* FP64 operand-delivery probe (the rule the hot loop is written around): the same 16
+ * independent DFMA chains per thread, once with two fresh register operands per instruction (the other two loop
+ * invariant) and once with three distinct 64-bit register operands per instruction; writes both rates in TFLOP/s.
+ * On B200 the second runs at about two thirds of the first (3 instead of 2 pipe cycles per instruction). */
+int no_probe_fp64_operands(int device, int millis, double *tflops_two_operands, double *tflops_three_operands,
+                           void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -37,14 +37,23 @@ typedef struct no_trace_plan no_trace_plan;   /* opaque; owns its device tables 
 
 #define NO_TRACE_MAX_VERTEX 6
 
+/* flags of no_trace_init */
+#define NO_TRACE_CHARGE_CONSERVING 1   /* the caller promises that every vertex matrix is EXACTLY zero outside the 96
+                                          charge-conserving entries, t_o1 + t_o2 = t_i1 + t_i2 (what no_eval
+                                          writes).  The plan then skips the blocks that isospin conservation at each vertex
+                                          empties ("the subset of isospin configurations consistent with isospin conservation
+                                          at each vertex"): a quarter of the tensor-core products of a ladder
+                                          or ring remain.  With matrices that break the promise the result is unspecified. */
+
 /* Plan the trace of one topology and upload its tables to device `device`.
  *   n_vertex : 1..NO_TRACE_MAX_VERTEX (the MBPT order at the two-body level)
  *   topo     : HOST, const, [n_vertex][4] ints = line ids (out 1, out 2, in 1, in 2) of every vertex; every id
  *              0 .. 2 n_vertex - 1 must appear exactly once among the outgoing and once among the incoming slots
- * NO_ERR_INVALID: malformed topology, or one that cannot be contracted with at most four open lines after fixing
+ *   flags    : 0 (arbitrary complex vertex matrices) or NO_TRACE_CHARGE_CONSERVING
+ * NO_ERR_INVALID: unknown flag, malformed topology, or one that cannot be contracted with at most four open lines after fixing
  * the labels of at most three lines in an outer loop (every ladder, ring and fifth-order diagram tested fits;
  * disconnected diagrams are accepted).  *plan is written only on success. */
-int no_trace_init(no_trace_plan **plan, int n_vertex, const int *topo, int device);
+int no_trace_init(no_trace_plan **plan, int n_vertex, const int *topo, int flags, int device);
 
 /* Enqueue the trace of n_sample samples on `cuda_stream` (a cudaStream_t; NULL is the default stream).  No
  * synchronisation inside; one plan may be used from several streams and host threads at once.
@@ -57,10 +66,11 @@ int no_trace_eval(const no_trace_plan *plan, const double *d_vertices, long long
 
 /* Facts about a plan (each pointer may be NULL): complex multiply-adds per sample of the planned contraction,
  * widest frontier (open lines), number of sliced lines, number of charge-conserving isospin assignments of the lines
- * ("the subset of isospin configurations consistent with isospin conservation at each vertex"), and the
- * vertex order (n_vertex ints). */
+ * ("the subset of isospin configurations consistent with isospin conservation at each vertex"), the
+ * vertex order (n_vertex ints), and the number of 8x8x4 FP64 tensor-core products per sample that the 16x16x16 steps
+ * issue (64 per step for arbitrary vertices, 16 with NO_TRACE_CHARGE_CONSERVING). */
 int no_trace_info(const no_trace_plan *plan, long long *cmacs_per_sample, int *max_open, int *n_sliced,
-                  long long *n_isospin_configs, int *order);
+                  long long *n_isospin_configs, int *order, long long *tensor_products_per_sample);
 
 /* Text of the last CUDA error seen by the calling thread in a no_trace_* call ("" if none). */
 const char *no_trace_last_cuda_error(void);

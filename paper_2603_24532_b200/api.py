@@ -115,11 +115,13 @@ class SpinIsospinTrace:
     vertices: complex128 CUDA tensor [n_sample, n_vertex, 16, 16] (e.g. NormalOrdering output reshaped), contiguous.
     """
 
-    def __init__(self, topo, device: int = 0):
+    def __init__(self, topo, device: int = 0, charge_conserving: bool = False):
+        """charge_conserving: the vertex matrices are exactly zero outside the 96 charge-conserving entries (true for
+        NormalOrdering output): structurally zero blocks are skipped (NO_TRACE_CHARGE_CONSERVING)."""
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2603_24532_b200 needs a CUDA device (no CPU fallback)")
         self.device = device
-        self._p = binding.no_trace_init(topo, device)
+        self._p = binding.no_trace_init(topo, device, binding.NO_TRACE_CHARGE_CONSERVING if charge_conserving else 0)
         self.n_vertex = len(topo)
 
     def info(self) -> dict:

@@ -17,7 +17,7 @@ NO_OK, NO_ERR_INVALID, NO_ERR_CUDA, NO_ERR_ALLOC = 0, 1, 2, 3
 
 EXPORTS = ("no_init", "no_init_angular", "no_eval", "no_eval_host", "no_eval_diag", "no_hf_energy", "no_sp_energy", "no_set_layout", "no_free", "no_strerror", "no_last_cuda_error",
            "no_kernel_info", "no_evals_per_cfg", "no_probe_fp64_peak",
-           "no_packed_doubles", "no_eval_packed", "no_unpack", "no_eval_host_packed")
+           "no_packed_doubles", "no_eval_packed", "no_unpack", "no_eval_host_packed", "no_probe_fp64_operands")
 
 NO_PACK_CHARGE, NO_PACK_ISOSPIN = 1, 2
 
@@ -80,9 +80,13 @@ def load() -> ctypes.CDLL:
         for name in ("no_init", "no_init_angular", "no_eval", "no_eval_host", "no_eval_diag", "no_hf_energy", "no_sp_energy", "no_set_layout", "no_free", "no_kernel_info",
                      "no_probe_fp64_peak", "no_packed_doubles", "no_eval_packed", "no_unpack", "no_eval_host_packed"):
             getattr(lib, name).restype = ctypes.c_int
-        lib.no_trace_init.argtypes = [ctypes.POINTER(H), ctypes.c_int, ctypes.c_void_p, ctypes.c_int]
+        lib.no_probe_fp64_operands.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double),
+                                               ctypes.POINTER(ctypes.c_double), ctypes.c_void_p]
+        lib.no_probe_fp64_operands.restype = ctypes.c_int
+        lib.no_trace_init.argtypes = [ctypes.POINTER(H), ctypes.c_int, ctypes.c_void_p, ctypes.c_int, ctypes.c_int]
         lib.no_trace_eval.argtypes = [H, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]
-        lib.no_trace_info.argtypes = [H, ctypes.POINTER(ctypes.c_longlong), ip, ip, ctypes.POINTER(ctypes.c_longlong), ip]
+        lib.no_trace_info.argtypes = [H, ctypes.POINTER(ctypes.c_longlong), ip, ip, ctypes.POINTER(ctypes.c_longlong), ip,
+                                      ctypes.POINTER(ctypes.c_longlong)]
         lib.no_trace_free.argtypes = [H]
         lib.no_trace_last_cuda_error.restype = ctypes.c_char_p
         for name in ("no_trace_init", "no_trace_eval", "no_trace_info", "no_trace_free"):
@@ -224,13 +228,26 @@ def no_probe_fp64_peak(device: int = 0, millis: int = 200, stream_ptr: Optional[
     return {"tflops": t.value, "n_sm": n.value}
 
 
+def no_probe_fp64_operands(device: int = 0, millis: int = 100, stream_ptr: Optional[int] = None) -> dict:
+    """DFMA rate (TFLOP/s) with two and with three fresh register operands per instruction (include/no.h)."""
+    a, b = ctypes.c_double(), ctypes.c_double()
+    rc = load().no_probe_fp64_operands(device, millis, ctypes.byref(a), ctypes.byref(b), ctypes.c_void_p(stream_ptr or 0))
+    if rc != NO_OK:
+        raise NoError(rc, "no_probe_fp64_operands")
+    return {"two_operands_tflops": a.value, "three_operands_tflops": b.value}
+
+
 # ---- include/no_trace.h: spin-isospin trace of a closed diagram (SURVEY.md 8(f) f4) ----
-def no_trace_init(topo, device: int = 0) -> ctypes.c_void_p:
-    """no_trace_init: topo host int array [n_vertex, 4] = line ids (out 1, out 2, in 1, in 2); returns the plan."""
+NO_TRACE_CHARGE_CONSERVING = 1
+
+
+def no_trace_init(topo, device: int = 0, flags: int = 0) -> ctypes.c_void_p:
+    """no_trace_init: topo host int array [n_vertex, 4] = line ids (out 1, out 2, in 1, in 2); returns the plan.
+    flags: 0 or NO_TRACE_CHARGE_CONSERVING (vertex matrices exactly zero outside the 96 charge-conserving entries)."""
     import numpy as np
     t = np.ascontiguousarray(topo, dtype=np.int32).reshape(-1, 4)
     h = ctypes.c_void_p()
-    rc = load().no_trace_init(ctypes.byref(h), t.shape[0], ctypes.c_void_p(t.ctypes.data), device)
+    rc = load().no_trace_init(ctypes.byref(h), t.shape[0], ctypes.c_void_p(t.ctypes.data), flags, device)
     if rc != NO_OK:
         raise NoError(rc, "no_trace_init")
     return h
@@ -245,14 +262,15 @@ def no_trace_eval(plan, d_vertices_ptr: int, n_sample: int, d_out_ptr: int, stre
 
 
 def no_trace_info(plan, n_vertex: int) -> dict:
-    cm, iso = ctypes.c_longlong(), ctypes.c_longlong()
+    cm, iso, tp = ctypes.c_longlong(), ctypes.c_longlong(), ctypes.c_longlong()
     mo, ns = ctypes.c_int(), ctypes.c_int()
     order = (ctypes.c_int * 8)()
-    rc = load().no_trace_info(plan, ctypes.byref(cm), ctypes.byref(mo), ctypes.byref(ns), ctypes.byref(iso), order)
+    rc = load().no_trace_info(plan, ctypes.byref(cm), ctypes.byref(mo), ctypes.byref(ns), ctypes.byref(iso), order,
+                              ctypes.byref(tp))
     if rc != NO_OK:
         raise NoError(rc, "no_trace_info")
     return {"cmacs_per_sample": cm.value, "max_open": mo.value, "n_sliced": ns.value, "n_isospin_configs": iso.value,
-            "order": [order[i] for i in range(n_vertex)]}
+            "order": [order[i] for i in range(n_vertex)], "tensor_products_per_sample": tp.value}
 
 
 def no_trace_free(plan) -> None:

@@ -595,4 +595,52 @@ int no_probe_fp64_peak(int device, int millis, double* tflops, int* n_sm, void* 
   return NO_OK;
 }
 
+int no_probe_fp64_operands(int device, int millis, double* tflops_two, double* tflops_three, void* cuda_stream) {
+  if (!tflops_two || !tflops_three || millis < 1) return NO_ERR_INVALID;
+  int n_dev = 0;
+  NO_CUDA(cudaGetDeviceCount(&n_dev));
+  if (device < 0 || device >= n_dev) return NO_ERR_INVALID;
+  DeviceGuard guard(device);
+  if (!guard.ok) return cuda_fail(cudaGetLastError(), "cudaSetDevice");
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  int sms = 0;
+  NO_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device));
+  const int threads = 256, blocks = sms * 4;
+  struct Res {
+    double* sink = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    ~Res() {
+      if (e0) cudaEventDestroy(e0);
+      if (e1) cudaEventDestroy(e1);
+      if (sink) cudaFree(sink);
+    }
+  } r;
+  NO_CUDA(cudaMalloc((void**)&r.sink, sizeof(double) * threads * blocks));
+  NO_CUDA(cudaEventCreate(&r.e0));
+  NO_CUDA(cudaEventCreate(&r.e1));
+  double* res[2] = {tflops_two, tflops_three};
+  for (int variant = 0; variant < 2; ++variant) {
+    int iters = 1 << 12;
+    double best = 0.0;
+    float ms = 0.f;
+    for (int rep = 0; rep < 24; ++rep) {
+      NO_CUDA(cudaEventRecord(r.e0, s));
+      if (variant) dfma_operand_probe_kernel<true><<<blocks, threads, 0, s>>>(r.sink, iters, 1.0);
+      else dfma_operand_probe_kernel<false><<<blocks, threads, 0, s>>>(r.sink, iters, 1.0);
+      NO_CUDA(cudaGetLastError());
+      NO_CUDA(cudaEventRecord(r.e1, s));
+      NO_CUDA(cudaEventSynchronize(r.e1));
+      NO_CUDA(cudaEventElapsedTime(&ms, r.e0, r.e1));
+      const double rate = 2.0 * 16.0 * (double)iters * threads * (double)blocks / (ms * 1e-3) * 1e-12;
+      if (ms >= 0.5f * millis) {
+        if (rate > best) best = rate;
+        if (rep >= 3 && ms >= (float)millis) break;
+      }
+      if (ms < (float)millis && iters < (1 << 28)) iters *= 2;
+    }
+    *res[variant] = best;
+  }
+  return NO_OK;
+}
+
 }  // extern "C"

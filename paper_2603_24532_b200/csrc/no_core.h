@@ -115,7 +115,7 @@ struct CfgConst {
   double cpair[4];    // |kappa_x - kappa_y|^2/2 + mpi^2
   double E0;          // k3-independent part of the regulator exponent
   double rs[kMaxRegPoly];  // s = -64 log2(e) dE = sum_k rs[k-1] (d^2)^k, k = 1..n
-  double smin;        // lower bound of s over the Fermi spheres (s at d^2 = (kF_max + |P/2|)^2); NaN if cfg is not finite
+  double smin;        // lower bound of s over the Fermi spheres (s at d^2 = 2 (kF_max^2 + |P/2|^2)); NaN if cfg is not finite
   double pad_[2];     // 40 doubles: keeps what follows in shared memory 32-byte aligned
 };
 constexpr int kCfgDoubles = sizeof(CfgConst) / sizeof(double);
@@ -169,8 +169,10 @@ NO_HD void cfg_setup(const DevParams& P, const double* cfg, CfgConst& c) {
       c.rs[k - 1] = scale * (binom * (px0[n - k] + px1[n - k]) * ps3[k]);
     }
     c.E0 = px0[n] + px1[n];
-    // s = d2 h(d2) decreases with d2 (all rs <= 0); d2 = |k3 - P/2|^2 <= (kF_max + |P/2|)^2
-    const double dmax = P.kf_max + sqrt(c.gamd), d2max = dmax * dmax;
+    // s = d2 h(d2) decreases with d2 (all rs <= 0); d2 = |k3 - P/2|^2 <= (kF_max + |P/2|)^2 <= 2 (kF_max^2 + |P/2|^2)
+    // (the second bound needs no square root: 21 dependent FP64 instructions less in every prologue; it is only used
+    //  to decide whether the hot loop needs its underflow guard)
+    const double d2max = 2.0 * fma(P.kf_max, P.kf_max, c.gamd);
     double h = c.rs[n - 1];
     for (int k = n - 2; k >= 0; --k) h = fma(d2max, h, c.rs[k]);
     c.smin = d2max * h;

@@ -360,4 +360,28 @@ __global__ void __launch_bounds__(256) dfma_probe_kernel(double* sink, int iters
   if (s == 123.456) sink[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
+// ---- FP64 operand-delivery probe: the same 16 DFMA chains with TWO or THREE fresh register operands ----
+// two:   a[k] = fma(a[k], x, y)        x, y loop invariant (one register-file read per instruction after reuse)
+// three: a[k] = fma(b[k], c[k'], a[k]) three distinct 64-bit registers per instruction (b, c rotate so that no
+//        operand-reuse slot hits)
+template <bool THREE>
+__global__ void __launch_bounds__(256) dfma_operand_probe_kernel(double* sink, int iters, double seed) {
+  double a[16], b[16], c[16];
+#pragma unroll
+  for (int k = 0; k < 16; ++k) {
+    a[k] = seed + k + threadIdx.x;
+    b[k] = 1.0 - 1e-9 * (seed + k + threadIdx.x);       // thread dependent: plain registers, not uniform ones
+    c[k] = 1e-9 * (k + 1 + threadIdx.x);
+  }
+  const double x = 1.0 - 1e-9 * seed, y = 1e-9;
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int k = 0; k < 16; ++k) a[k] = THREE ? fma(b[k], c[(k + 5) & 15], a[k]) : fma(a[k], x, y);
+  }
+  double s = 0;
+#pragma unroll
+  for (int k = 0; k < 16; ++k) s += a[k] + (THREE ? b[k] + c[k] : 0.0);
+  if (s == 123.456) sink[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
 }  // namespace no3n

@@ -21,7 +21,8 @@ using namespace no3n;
 namespace {
 
 struct DevTracePlan {
-  int n_vertex, n_slice_iter, pad_[2];
+  int n_vertex, n_slice_iter;
+  uint8_t n_groups, vgrp[kTrMaxVertex], pad_;     // load pipeline: executed steps, and which of them reads vertex v
   TraceStep steps[kTrMaxVertex];
 };
 static_assert(sizeof(TraceStep) % 16 == 0 && sizeof(DevTracePlan) % 16 == 0, "plan is staged with 16-byte copies");
@@ -53,17 +54,38 @@ __host__ __device__ inline size_t trace_warp_bytes(int n, int stages) {
   return 16 + (size_t)(stages * n + 2) * kTrMat * 16;
 }
 
-// request one sample: n x 256 complex numbers, one 16-byte cp.async (LDGSTS) per lane and element -- coalesced 512-byte
-// warp reads from HBM, written into the padded rows of buffer `dst`, no registers held while in flight.  (One TMA bulk
-// copy per sample cannot pad the rows, and one per row is bound by the TMA issue rate: 80 descriptors per sample ran
-// at 1.17e8 samples/s, profiles/r02b.md.)
-__device__ __forceinline__ void request_sample(double2* dst, const double2* src, int n, int lane) {
-  for (int e = lane; e < 256 * n; e += 32) {
-    const int rc = e & 255;
+// request vertex matrix v of a sample: 256 complex numbers, one 16-byte cp.async (LDGSTS) per lane and element --
+// coalesced 512-byte warp reads from HBM, written into the padded rows of the vertex's slot, no registers held while in
+// flight.  (One TMA bulk copy per sample cannot pad the rows, and one per row is bound by the TMA issue rate: 80
+// descriptors per sample ran at 1.17e8 samples/s, profiles/r02b.md.)
+__device__ __forceinline__ void request_vertex(double2* dst, const double2* src, int v, int lane) {
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    const int rc = lane + 32 * j;
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;"
-                 ::"r"(smem_u32(dst + (e >> 8) * kTrMat + rc + (rc >> 4))), "l"(src + e) : "memory");
+                 ::"r"(smem_u32(dst + v * kTrMat + rc + (rc >> 4))), "l"(src + v * 256 + rc) : "memory");
   }
+}
+
+// the vertices read by executed step g (all of them if g < 0) of the sample at src, as ONE cp.async group
+__device__ __forceinline__ void request_group(double2* dst, const double2* src, int n, const uint8_t* vgrp, int g, bool valid,
+                                              int lane) {
+  if (valid)
+    for (int v = 0; v < n; ++v)
+      if (g < 0 || vgrp[v] == g) request_vertex(dst, src, v, lane);
   asm volatile("cp.async.commit_group;" ::: "memory");
+}
+
+// wait until at most `pending` of this thread's most recent cp.async groups are still in flight
+__device__ __forceinline__ void wait_groups(int pending) {
+  switch (pending) {
+    case 0: asm volatile("cp.async.wait_group 0;" ::: "memory"); break;
+    case 1: asm volatile("cp.async.wait_group 1;" ::: "memory"); break;
+    case 2: asm volatile("cp.async.wait_group 2;" ::: "memory"); break;
+    case 3: asm volatile("cp.async.wait_group 3;" ::: "memory"); break;
+    case 4: asm volatile("cp.async.wait_group 4;" ::: "memory"); break;
+    default: asm volatile("cp.async.wait_group 5;" ::: "memory"); break;
+  }
 }
 
 // path: 0 = vector FP64 (DFMA) register tiles, 1 = FP64 tensor cores (DMMA m8n8k4) for the 16 x 16 x 16 steps
@@ -87,18 +109,33 @@ trace_kernel(const DevTracePlan* __restrict__ plan_g, const double2* __restrict_
   __syncthreads();
 
   const long long first = (long long)blockIdx.x * n_warps + warp, stride = (long long)gridDim.x * n_warps;
-  if (first < n_sample) request_sample(vbuf, V + first * n * 256, n, lane);
+  // Load pipeline.  stages == 1 (default): ONE set of vertex slots per warp.  A vertex is read by exactly one executed
+  // step, so right after step g of this sample the copies of the NEXT sample's vertices of step g are issued into
+  // the same slots (one cp.async group per executed step); before step g of the next sample at most n_groups - 1
+  // younger groups may still be in flight.  The copies of a sample thus run under the arithmetic of the previous one
+  // without a second buffer (shared memory decides how many samples an SM keeps in flight).  With sliced lines every
+  // vertex is read in every outer iteration: the whole sample is one group, requested after the last iteration.
+  const uint8_t* vgrp = reinterpret_cast<const DevTracePlan*>(tsm)->vgrp;
+  const int n_groups = n_iter == 1 && stages == 1 ? reinterpret_cast<const DevTracePlan*>(tsm)->n_groups : 1;
+  const bool piped = n_groups > 1;
+  if (piped) {
+    for (int g = 0; g < n_groups; ++g) request_group(vbuf, V + first * n * 256, n, vgrp, g, first < n_sample, lane);
+  } else {
+    request_group(vbuf, V + first * n * 256, n, vgrp, -1, first < n_sample, lane);
+  }
   int stage = 0;
   for (long long smp = first; smp < n_sample; smp += stride) {
     const long long nxt = smp + stride;
-    if (stages == 2 && nxt < n_sample) {
-      // the other buffer's last readers finished before the __syncwarp that ended the previous iteration
-      request_sample(vbuf + (size_t)(stage ^ 1) * n * kTrMat, V + nxt * n * 256, n, lane);
-      asm volatile("cp.async.wait_group 1;" ::: "memory");      // this sample has landed; the next one is in flight
-    } else {
-      asm volatile("cp.async.wait_group 0;" ::: "memory");
+    if (!piped) {
+      if (stages == 2) {
+        // the other buffer's last readers finished before the __syncwarp that ended the previous iteration
+        request_group(vbuf + (size_t)(stage ^ 1) * n * kTrMat, V + nxt * n * 256, n, vgrp, -1, nxt < n_sample, lane);
+        wait_groups(1);                                  // this sample has landed; the next one is in flight
+      } else {
+        wait_groups(0);
+      }
+      __syncwarp();
     }
-    __syncwarp();
     const double2* W = vbuf + (size_t)stage * n * kTrMat;
 
     double2 total = make_double2(0.0, 0.0);
@@ -111,15 +148,52 @@ trace_kernel(const DevTracePlan* __restrict__ plan_g, const double2* __restrict_
       for (int k = 0; k < n; ++k) {
         const TraceStep& s = steps[k];
         if (s.skip) continue;                           // folded into a neighbouring step (warp uniform)
+        if (piped) {                                    // the vertices of this step have landed
+          wait_groups(n_groups - 1);
+          __syncwarp();
+        }
         const double2* Wv = W + s.vertex * kTrMat + s.sliceW[it];
         const int nA = s.nA, nB = s.nB, nC = s.nC, nOut = nA * nB;
-        if (nA == 16 && nB == 16 && nC == 16) {
+        if (s.big) {
           // R of this step: the partial result, or (first vertex folded in) the first vertex's matrix itself
           const double2* Rs = s.r_vertex >= 0 ? W + s.r_vertex * kTrMat + steps[0].sliceW[it] : Rin;
-          // last vertex folded in: it closes all four lines, T = sum_o R'[o] W_last[lastW[o]]
+          // last vertex folded in: it closes all four lines, T = sum_{a,b} R'[a,b] W_last[lastW[a + 16 b]]
           const double2* Wl = s.fuse_last ? W + steps[n - 1].vertex * kTrMat + steps[n - 1].sliceW[it] : nullptr;
           double2 dot = make_double2(0.0, 0.0);
-          if (path == 1) {
+          if (path == 1 && s.block_diag) {
+            // charge-conserving vertices: the product is block diagonal in the isospin-pair enumeration, two 8 x 8 x 8
+            // complex blocks (k-steps 2 p, 2 p + 1 -> output tile (p, p)); 16 tensor-core products instead of 64
+            const int r = lane >> 2, c = lane & 3, valid = s.ks_valid;
+            double cre[2][2] = {{0.0, 0.0}, {0.0, 0.0}}, cim[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
+#pragma unroll
+            for (int p = 0; p < 2; ++p) {
+              const int aR = s.baseR[8 * p + r], bW = s.baseW[8 * p + r];
+#pragma unroll
+              for (int j = 0; j < 2; ++j) {
+                const int ks = 2 * p + j;
+                if (!(valid >> ks & 1)) continue;           // warp uniform
+                const double2 A = Rs[aR + s.offR[4 * ks + c]], B = Wv[s.offW[4 * ks + c] + bW];
+                dmma884(cre[p][0], cre[p][1], A.x, B.x);
+                dmma884(cim[p][0], cim[p][1], A.x, B.y);
+                dmma884(cre[p][0], cre[p][1], -A.y, B.y);
+                dmma884(cim[p][0], cim[p][1], A.y, B.x);
+              }
+            }
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+              for (int nt = 0; nt < 2; ++nt)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                  const int a = 8 * mt + r, b = 8 * nt + 2 * c + e;
+                  if (Wl) {
+                    if (mt == nt) cfma(dot, make_double2(cre[mt][e], cim[mt][e]), Wl[s.lastW[a + 16 * b]]);
+                  } else {
+                    // the off-diagonal tiles are stored as zeros: the next step reads whole tiles
+                    Rout[s.outA[a] + s.outB[b]] = mt == nt ? make_double2(cre[mt][e], cim[mt][e]) : make_double2(0.0, 0.0);
+                  }
+                }
+          } else if (path == 1) {
             // 16 x 16 x 16 complex product on the FP64 tensor cores: four real products per (8 x 8 tile, k-step of 4),
             // Re = Re Re - Im Im, Im = Re Im + Im Re; fragments come straight from the tabulated offsets
             const int r = lane >> 2, c = lane & 3;
@@ -162,10 +236,10 @@ trace_kernel(const DevTracePlan* __restrict__ plan_g, const double2* __restrict_
               for (int nt = 0; nt < 2; ++nt)
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
-                  const int o = (8 * mt + r) + 16 * (8 * nt + 2 * c + e);
+                  const int a = 8 * mt + r, b = 8 * nt + 2 * c + e;
                   const double2 v = make_double2(cre[mt][nt][e], cim[mt][nt][e]);
-                  if (Wl) cfma(dot, v, Wl[s.lastW[o]]);
-                  else Rout[o + (o >> 4)] = v;
+                  if (Wl) cfma(dot, v, Wl[s.lastW[a + 16 * b]]);
+                  else Rout[s.outA[a] + s.outB[b]] = v;
                 }
           } else {
             // vector FP64 variant: lane (la, lb) owns the 4 x 2 tile a = la + 4 i, b = lb + 8 j
@@ -196,9 +270,9 @@ trace_kernel(const DevTracePlan* __restrict__ plan_g, const double2* __restrict_
             for (int i = 0; i < 4; ++i)
 #pragma unroll
               for (int j = 0; j < 2; ++j) {
-                const int o = (la + 4 * i) + 16 * (lb + 8 * j);
-                if (Wl) cfma(dot, acc[i][j], Wl[s.lastW[o]]);
-                else Rout[o + (o >> 4)] = acc[i][j];
+                const int a = la + 4 * i, b = lb + 8 * j;
+                if (Wl) cfma(dot, acc[i][j], Wl[s.lastW[a + 16 * b]]);
+                else Rout[s.outA[a] + s.outB[b]] = acc[i][j];
               }
           }
           if (Wl) {                                     // add the 32 partial dot products (fixed butterfly)
@@ -233,17 +307,16 @@ trace_kernel(const DevTracePlan* __restrict__ plan_g, const double2* __restrict_
           if (nOut == 1) last = v;
         }
         __syncwarp();
+        // the slots this step read are free: request the same vertices of the warp's next sample
+        if (piped) request_group(vbuf, V + nxt * n * 256, n, vgrp, s.grp, nxt < n_sample, lane);
         double2* t = Rin; Rin = Rout; Rout = t;
       }
       total.x += last.x; total.y += last.y;
     }
     if (lane == 0) out[smp] = total;
     __syncwarp();
-    if (stages == 2) {
-      stage ^= 1;
-    } else if (nxt < n_sample) {
-      request_sample(vbuf, V + nxt * n * 256, n, lane);
-    }
+    if (stages == 2) stage ^= 1;
+    else if (!piped) request_group(vbuf, V + nxt * n * 256, n, vgrp, -1, nxt < n_sample, lane);
   }
 }
 
@@ -281,12 +354,12 @@ extern "C" {
 
 const char* no_trace_last_cuda_error(void) { return g_trace_err; }
 
-int no_trace_init(no_trace_plan** out, int n_vertex, const int* topo, int device) {
-  if (!out || !topo) return NO_ERR_INVALID;
+int no_trace_init(no_trace_plan** out, int n_vertex, const int* topo, int flags, int device) {
+  if (!out || !topo || (flags & ~NO_TRACE_CHARGE_CONSERVING)) return NO_ERR_INVALID;
   no_trace_plan* p = new (std::nothrow) no_trace_plan();
   if (!p) return NO_ERR_ALLOC;
   p->d_plan = nullptr;
-  if (build_trace_plan(n_vertex, topo, p->plan) != 0) { delete p; return NO_ERR_INVALID; }
+  if (build_trace_plan(n_vertex, topo, p->plan, (flags & NO_TRACE_CHARGE_CONSERVING) != 0) != 0) { delete p; return NO_ERR_INVALID; }
   int n_dev = 0;
   cudaError_t e = cudaGetDeviceCount(&n_dev);
   if (e != cudaSuccess) { delete p; return trace_cuda_fail(e, "cudaGetDeviceCount"); }
@@ -314,7 +387,9 @@ int no_trace_init(no_trace_plan** out, int n_vertex, const int* topo, int device
   DevTracePlan hp;
   hp.n_vertex = p->plan.n_vertex;
   hp.n_slice_iter = p->plan.n_slice_iter;
-  hp.pad_[0] = hp.pad_[1] = 0;
+  hp.n_groups = (uint8_t)p->plan.n_groups;
+  for (int v = 0; v < kTrMaxVertex; ++v) hp.vgrp[v] = (uint8_t)(v < p->plan.n_vertex ? p->plan.vgrp[v] : 255);
+  hp.pad_ = 0;
   for (int k = 0; k < kTrMaxVertex; ++k) hp.steps[k] = p->plan.steps[k];
   e = cudaMalloc((void**)&p->d_plan, sizeof(DevTracePlan));
   if (e != cudaSuccess) { delete p; trace_cuda_fail(e, "cudaMalloc(trace plan)"); return NO_ERR_ALLOC; }
@@ -349,9 +424,11 @@ int no_trace_eval(const no_trace_plan* p, const double* d_vertices, long long n_
   return NO_OK;
 }
 
-int no_trace_info(const no_trace_plan* p, long long* cmacs, int* max_open, int* n_sliced, long long* n_iso, int* order) {
+int no_trace_info(const no_trace_plan* p, long long* cmacs, int* max_open, int* n_sliced, long long* n_iso, int* order,
+                  long long* tensor_products) {
   if (!p) return NO_ERR_INVALID;
   if (cmacs) *cmacs = p->plan.cmacs;
+  if (tensor_products) *tensor_products = p->plan.dmma_products;
   if (max_open) *max_open = p->plan.max_open;
   if (n_sliced) *n_sliced = p->plan.n_sliced;
   if (n_iso) *n_iso = p->plan.n_isospin;

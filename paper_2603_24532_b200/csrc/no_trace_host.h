@@ -64,13 +64,26 @@ struct TraceStep {
   int r_vertex;               // >= 0: R of this step IS that vertex matrix (baseR, offR hold offsets into it); -1: R
   int fuse_last;              // 1: the next (last) step closes all four lines: its sum is folded into this step,
                               //    lastW[o] = offset in the LAST vertex of the element that multiplies R'[o]
-  int pad_;
+  int big;                    // 1: 16 x 16 x 16 step (two kept, two closed, two opened lines), tile tables below are valid
   uint16_t baseR[kTrTab];     // [a]  offset of the kept labels in R (all offsets padded, see kTrRow)
   uint16_t offR[kTrTab];      // [g]  offset of the closed labels in R
   uint16_t baseW[kTrTab];     // [b]  offset of the opened labels in the vertex matrix
   uint16_t offW[kTrTab];      // [g]  offset of the closed labels in the vertex matrix
   uint16_t sliceW[64];        // [outer iteration] offset of the sliced labels in the vertex matrix
   uint16_t lastW[kTrTab];     // [o = a + 16 b] see fuse_last
+  // 16 x 16 x 16 steps only.  The 16 label combinations of a line pair are enumerated isospin-major,
+  // e = 4 iso + spin, iso over (t1,t2) = (0,1) (1,0) (0,0) (1,1), spin = s1 + 2 s2: a tensor-core tile of 8 holds
+  // two isospin combinations, a k-step of 4 holds one.  R'[a, b] is stored at outA[a] + outB[b] (padded offsets of
+  // the canonical index); lastW is indexed by a + 16 b of this enumeration.
+  uint16_t outA[16], outB[16];
+  // tile_mask[ks] bit (2 mt + nt): the 8 x 8 x 4 product of m-tile mt, n-tile nt, k-step ks can be non-zero; all
+  // ones unless the plan was made for charge-conserving vertices.  There the product is block diagonal: k-steps 0, 1
+  // feed output tile (0, 0), k-steps 2, 3 feed tile (1, 1), the off-diagonal tiles are zero (block_diag = 1,
+  // ks_valid bit ks: the k-step contributes).
+  uint8_t tile_mask[4];
+  uint8_t block_diag, ks_valid;
+  uint8_t grp;                // index of this step among the executed (not skipped) steps
+  uint8_t pad2_[9];
 };
 
 struct TracePlan {
@@ -82,6 +95,12 @@ struct TracePlan {
   int max_open;               // widest frontier
   long long cmacs;            // complex multiply-adds per sample (all outer iterations)
   long long n_isospin;        // charge-conserving isospin assignments of the lines, for information
+  long long dmma_products;    // 8 x 8 x 4 real tensor-core products per sample in the 16 x 16 x 16 steps (after skipping)
+  int charge;                 // 1: planned for charge-conserving vertices (structurally zero tiles are skipped)
+  // load pipeline of the kernel: a vertex matrix is read by exactly one executed step, so its shared-memory slot is
+  // free for the NEXT sample's copy as soon as that step is done: n_groups executed steps, vgrp[v] = the one reading v
+  int n_groups;
+  int vgrp[kTrMaxVertex];
   TraceStep steps[kTrMaxVertex];
 };
 
@@ -148,7 +167,12 @@ inline int popcount(unsigned m) { int c = 0; for (; m; m &= m - 1) ++c; return c
 }  // namespace trace_detail
 
 // 0 on success; 1 if the topology is malformed or cannot be contracted within the limits above
-inline int build_trace_plan(int n, const int* topo, TracePlan& plan) {
+// charge: the caller promises that every vertex matrix is exactly zero outside the 96 charge-conserving entries
+// (t_o1 + t_o2 = t_i1 + t_i2, what no_eval writes).  Then R[open labels] vanishes unless
+// sum over the open lines of sigma_l t_l = 0 (sigma = +1: the line leaves the absorbed part, i.e. was opened at an
+// outgoing slot; -1: it enters it) and the products of structurally zero tiles are skipped ("the
+// subset of isospin configurations consistent with isospin conservation at each vertex").
+inline int build_trace_plan(int n, const int* topo, TracePlan& plan, bool charge = false) {
   using namespace trace_detail;
   if (!trace_topology_valid(n, topo)) return 1;
   const int L = 2 * n;
@@ -195,8 +219,14 @@ inline int build_trace_plan(int n, const int* topo, TracePlan& plan) {
   plan.n_slice_iter = 1 << (2 * plan.n_sliced);
   for (int v = 0; v < n; ++v) plan.order[v] = best_order[v];
 
+  plan.charge = charge ? 1 : 0;
+  plan.dmma_products = 0;
+  // isospin-major enumeration of a pair of line labels (16 x 16 x 16 steps): digit j of enumeration e
+  static const int iso_t[4][2] = {{0, 1}, {1, 0}, {0, 0}, {1, 1}};
+  auto big_digit = [](int e, int j) { return 2 * (((e & 3) >> j) & 1) + iso_t[e >> 2][j]; };
+
   // tables of every step
-  int open[kTrMaxLines], n_open = 0;
+  int open[kTrMaxLines], open_sigma[kTrMaxLines], n_open = 0;
   for (int k = 0; k < n; ++k) {
     const int v = plan.order[k];
     TraceStep& s = plan.steps[k];
@@ -228,15 +258,18 @@ inline int build_trace_plan(int n, const int* topo, TracePlan& plan) {
     s.nA = 1 << (2 * n_kept);
     s.nB = 1 << (2 * n_opened);
     s.nC = 1 << (2 * n_closed);
+    const bool big = n_kept == 2 && n_opened == 2 && n_closed == 2 && closed_slot2[0] < 0 && closed_slot2[1] < 0;
+    s.big = big ? 1 : 0;
+    auto digit = [&](int e, int j) { return big ? big_digit(e, j) : (e >> (2 * j)) & 3; };
     for (int a = 0; a < kTrTab; ++a) {
       int off = 0;
-      for (int j = 0; j < n_kept; ++j) off += ((a >> (2 * j)) & 3) << (2 * kept_pos[j]);
+      for (int j = 0; j < n_kept; ++j) off += digit(a, j) << (2 * kept_pos[j]);
       s.baseR[a] = (uint16_t)(a < s.nA ? tr_pad(off) : 0);
     }
     for (int g = 0; g < kTrTab; ++g) {
       int offr = 0, offw = 0;
       for (int j = 0; j < n_closed; ++j) {
-        const int x = (g >> (2 * j)) & 3;
+        const int x = digit(g, j);
         if (closed_pos[j] >= 0) offr += x << (2 * closed_pos[j]);
         offw += slot_off(closed_slot[j], x);
         if (closed_slot2[j] >= 0) offw += slot_off(closed_slot2[j], x);
@@ -246,9 +279,48 @@ inline int build_trace_plan(int n, const int* topo, TracePlan& plan) {
     }
     for (int b = 0; b < kTrTab; ++b) {
       int off = 0;
-      for (int j = 0; j < n_opened; ++j) off += slot_off(opened_slot[j], (b >> (2 * j)) & 3);
+      for (int j = 0; j < n_opened; ++j) off += slot_off(opened_slot[j], digit(b, j));
       s.baseW[b] = (uint16_t)(b < s.nB ? off : 0);
     }
+    for (int e = 0; e < 16; ++e) {
+      const int canon = big ? big_digit(e, 0) + 4 * big_digit(e, 1) : e;
+      s.outA[e] = (uint16_t)tr_pad(canon);
+      s.outB[e] = (uint16_t)tr_pad(16 * canon);
+    }
+    for (int ks = 0; ks < 4; ++ks) s.tile_mask[ks] = 0xF;
+    s.block_diag = 0;
+    s.ks_valid = 0xF;
+    if (big && charge && plan.n_sliced == 0) {
+      // signed charges: R side sigma (orientation of the open line), vertex side tau (+1 outgoing slot, -1 incoming)
+      const int sk[2] = {open_sigma[kept_pos[0]], open_sigma[kept_pos[1]]};
+      const int sc[2] = {open_sigma[closed_pos[0]], open_sigma[closed_pos[1]]};
+      const int tc[2] = {closed_slot[0] < 2 ? 1 : -1, closed_slot[1] < 2 ? 1 : -1};
+      const int to[2] = {opened_slot[0] < 2 ? 1 : -1, opened_slot[1] < 2 ? 1 : -1};
+      uint8_t masks[4];
+      bool diag = true;
+      for (int ks = 0; ks < 4; ++ks) {
+        const int qRg = sc[0] * iso_t[ks][0] + sc[1] * iso_t[ks][1], qWg = tc[0] * iso_t[ks][0] + tc[1] * iso_t[ks][1];
+        int mset = 0, nset = 0;
+        for (int i = 0; i < 4; ++i) {
+          if (sk[0] * iso_t[i][0] + sk[1] * iso_t[i][1] + qRg == 0) mset |= 1 << (i >> 1);
+          if (to[0] * iso_t[i][0] + to[1] * iso_t[i][1] + qWg == 0) nset |= 1 << (i >> 1);
+        }
+        int mask = 0;
+        for (int mt = 0; mt < 2; ++mt)
+          for (int nt = 0; nt < 2; ++nt)
+            if ((mset >> mt & 1) && (nset >> nt & 1)) mask |= 1 << (2 * mt + nt);
+        masks[ks] = (uint8_t)mask;
+        // the isospin pairs {(0,1),(1,0)} and {(0,0),(1,1)} are mapped onto themselves by charge matching
+        diag = diag && (mask == 0 || mask == (ks < 2 ? 1 : 8));
+      }
+      if (diag) {
+        s.block_diag = 1;
+        s.ks_valid = 0;
+        for (int ks = 0; ks < 4; ++ks) { s.tile_mask[ks] = masks[ks]; if (masks[ks]) s.ks_valid |= (uint8_t)(1 << ks); }
+      }
+    }
+    if (big)
+      for (int ks = 0; ks < 4; ++ks) plan.dmma_products += 4LL * popcount(s.tile_mask[ks]) * plan.n_slice_iter;
     for (int it = 0; it < 64; ++it) {
       int off = 0;
       for (int i = 0; i < plan.n_sliced; ++i)
@@ -258,16 +330,17 @@ inline int build_trace_plan(int n, const int* topo, TracePlan& plan) {
     }
     // new frontier: kept lines in their old order, then the opened lines in slot order: R'[a + nA b]
     int next[kTrMaxLines], m = 0;
-    for (int j = 0; j < n_kept; ++j) next[m++] = open[kept_pos[j]];
-    for (int j = 0; j < n_opened; ++j) next[m++] = opened_line[j];
+    int next_sigma[kTrMaxLines];
+    for (int j = 0; j < n_kept; ++j) { next_sigma[m] = open_sigma[kept_pos[j]]; next[m++] = open[kept_pos[j]]; }
+    for (int j = 0; j < n_opened; ++j) { next_sigma[m] = opened_slot[j] < 2 ? 1 : -1; next[m++] = opened_line[j]; }
     n_open = m;
-    for (int j = 0; j < m; ++j) open[j] = next[j];
+    for (int j = 0; j < m; ++j) { open[j] = next[j]; open_sigma[j] = next_sigma[j]; }
   }
   if (n_open != 0) return 1;
 
   // fusions around the 16 x 16 x 16 steps (what ladders and rings consist of)
   for (int k = 0; k < n; ++k) { plan.steps[k].skip = 0; plan.steps[k].r_vertex = -1; plan.steps[k].fuse_last = 0; }
-  auto is_big = [&](int k) { return plan.steps[k].nA == 16 && plan.steps[k].nB == 16 && plan.steps[k].nC == 16; };
+  auto is_big = [&](int k) { return plan.steps[k].big == 1; };
   // (1) first vertex: step 0 would copy its 256 entries into R (R[pad(b)] = W_0[baseW_0[b]], b = canonical index of
   //     the four opened lines).  Offsets are additive over disjoint digits, so step 1 can address the vertex itself.
   if (n >= 3 && plan.steps[0].nA == 1 && plan.steps[0].nC == 1 && plan.steps[0].nB == 256 && is_big(1)) {
@@ -284,12 +357,22 @@ inline int build_trace_plan(int n, const int* topo, TracePlan& plan) {
   if (n >= 3 && plan.steps[n - 1].nA == 1 && plan.steps[n - 1].nB == 1 && plan.steps[n - 1].nC == 256 && is_big(n - 2)) {
     TraceStep& sl = plan.steps[n - 1];
     TraceStep& sp = plan.steps[n - 2];
-    for (int g = 0; g < 256; ++g) {
-      const int o = sl.offR[g] - sl.offR[g] / kTrRow;          // canonical index of R'
-      sp.lastW[o] = sl.offW[g];
-    }
+    uint16_t by_offset[kTrMat] = {0};                          // padded offset in R' -> offset in the last vertex
+    for (int g = 0; g < 256; ++g) by_offset[sl.offR[g]] = sl.offW[g];
+    for (int a = 0; a < 16; ++a)
+      for (int b = 0; b < 16; ++b) sp.lastW[a + 16 * b] = by_offset[sp.outA[a] + sp.outB[b]];
     sp.fuse_last = 1;
     sl.skip = 1;
+  }
+  plan.n_groups = 0;
+  for (int k = 0; k < n; ++k) {
+    TraceStep& st = plan.steps[k];
+    st.grp = 0;
+    if (st.skip) continue;
+    st.grp = (uint8_t)plan.n_groups++;
+    plan.vgrp[st.vertex] = st.grp;
+    if (st.r_vertex >= 0) plan.vgrp[st.r_vertex] = st.grp;
+    if (st.fuse_last) plan.vgrp[plan.steps[n - 1].vertex] = st.grp;
   }
   return 0;
 }

@@ -61,9 +61,9 @@ def test_error_strings_and_null_handling(lib):
     assert lib.no_eval(None, None, 0, None, None) == binding.NO_ERR_INVALID
     assert lib.no_evals_per_cfg(None) == 0
     assert lib.no_trace_free(None) == binding.NO_OK
-    assert lib.no_trace_init(None, 2, None, 0) == binding.NO_ERR_INVALID
+    assert lib.no_trace_init(None, 2, None, 0, 0) == binding.NO_ERR_INVALID
     assert lib.no_trace_eval(None, None, 0, None, None) == binding.NO_ERR_INVALID
-    assert lib.no_trace_info(None, None, None, None, None, None) == binding.NO_ERR_INVALID
+    assert lib.no_trace_info(None, None, None, None, None, None, None) == binding.NO_ERR_INVALID
 
 
 def test_malformed_trace_topologies_are_rejected_before_any_cuda_call(lib):
@@ -73,11 +73,13 @@ def test_malformed_trace_topologies_are_rejected_before_any_cuda_call(lib):
                  [[0, 1, 2, 3], [2, 2, 0, 1]]):         # a line leaving twice
         t = np.array(topo, dtype=np.int32)
         h = ctypes.c_void_p()
-        assert lib.no_trace_init(ctypes.byref(h), t.shape[0], ctypes.c_void_p(t.ctypes.data), 0) == binding.NO_ERR_INVALID
+        assert lib.no_trace_init(ctypes.byref(h), t.shape[0], ctypes.c_void_p(t.ctypes.data), 0, 0) == binding.NO_ERR_INVALID
         assert not h.value
     t = np.zeros((7, 4), dtype=np.int32)
     h = ctypes.c_void_p()
-    assert lib.no_trace_init(ctypes.byref(h), 7, ctypes.c_void_p(t.ctypes.data), 0) == binding.NO_ERR_INVALID
+    assert lib.no_trace_init(ctypes.byref(h), 7, ctypes.c_void_p(t.ctypes.data), 0, 0) == binding.NO_ERR_INVALID
+    t2 = np.array([[0, 1, 2, 3], [2, 3, 0, 1]], dtype=np.int32)
+    assert lib.no_trace_init(ctypes.byref(h), 2, ctypes.c_void_p(t2.ctypes.data), 8, 0) == binding.NO_ERR_INVALID   # unknown flag
 
 
 GOOD = dict(kf_n=1.0, kf_p=0.0, c1=-0.81, c3=-3.2, c4=0.0, cD=1.0, cE=-0.5, gA=1.27, fpi=92.4, mpi=138.04,

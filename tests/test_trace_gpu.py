@@ -35,8 +35,8 @@ def check(got, want, label=""):
     return worst
 
 
-def gpu_trace(topo, V):
-    tr = SpinIsospinTrace(topo)
+def gpu_trace(topo, V, charge=False):
+    tr = SpinIsospinTrace(topo, charge_conserving=charge)
     out = tr(torch.from_numpy(V).cuda())
     torch.cuda.synchronize()
     info = tr.info()
@@ -72,6 +72,11 @@ def test_trace_matches_the_unoptimized_trace(name, topo):
         got, info = gpu_trace(topo, V)
         want = T.trace_bruteforce(topo, V)
         worst = check(got, want, f"{name} dense={dense}")
+        if not dense:
+            # plan for charge-conserving vertices (NO_TRACE_CHARGE_CONSERVING): structurally zero blocks skipped
+            got_c, info_c = gpu_trace(topo, V, charge=True)
+            worst = max(worst, check(got_c, want, f"{name} charge-conserving plan"))
+            assert info_c["tensor_products_per_sample"] <= info["tensor_products_per_sample"]
     assert info["n_isospin_configs"] == T.isospin_configs(topo)
     print(f"{name}: {info}, max rel err {worst:.2e}")
 
@@ -116,13 +121,14 @@ def test_trace_abi_argument_checks():
     assert float(out.abs().sum()) == 0.0
     h = ctypes.c_void_p()
     t = np.ascontiguousarray(topo)
-    assert lib.no_trace_init(ctypes.byref(h), 3, vp(t.ctypes.data), 99) == binding.NO_ERR_INVALID
+    assert lib.no_trace_init(ctypes.byref(h), 3, vp(t.ctypes.data), 0, 99) == binding.NO_ERR_INVALID
     binding.no_trace_free(p)
-    # NaN in one sample stays in that sample
+    # NaN in one sample stays in that sample (both kinds of plan)
     Vn = TW.vertex_matrices(6, 3, seed=6)
     Vn[2, 1, 0, 0] = np.nan
-    got, _ = gpu_trace(topo, Vn)
-    assert np.isnan(got[2]) and np.isfinite(np.delete(got, 2)).all()
+    for charge in (False, True):
+        got, _ = gpu_trace(topo, Vn, charge=charge)
+        assert np.isnan(got[2]) and np.isfinite(np.delete(got, 2)).all()
 
 
 def test_normal_ordering_feeds_the_trace_on_the_device():
@@ -134,7 +140,7 @@ def test_normal_ordering_feeds_the_trace_on_the_device():
     no = NormalOrdering(device=0, **run.params())
     M = no(torch.from_numpy(cfg).cuda())                      # [n n_sample, 16, 16] complex
     topo = TW.ring(n)
-    tr = SpinIsospinTrace(topo)
+    tr = SpinIsospinTrace(topo, charge_conserving=True)       # no_eval writes exact zeros outside the 96 entries
     got = tr(M.reshape(n_sample, n, 16, 16)).cpu().numpy()
     torch.cuda.synchronize()
     want = T.trace_bruteforce(topo, O.normal_order(cfg, **run.params()).reshape(n_sample, n, 16, 16))
@@ -149,10 +155,15 @@ def test_bench_size_launch_sampled_against_the_oracle():
     topo = TW.ring(TRACE_BENCH["n_vertex"])
     n_sample = TRACE_BENCH["n_sample"]
     V = TW.vertex_matrices(n_sample, 5, seed=TRACE_BENCH["seed"])
-    tr = SpinIsospinTrace(topo)
-    out = tr(torch.from_numpy(V).cuda()).cpu().numpy()
+    tr = SpinIsospinTrace(topo, charge_conserving=True)       # as bench.py runs it
+    d_V = torch.from_numpy(V).cuda()
+    out = tr(d_V).cpu().numpy()
     torch.cuda.synchronize()
     assert np.isfinite(out.view(np.float64)).all()
+    dense_plan = SpinIsospinTrace(topo)
+    out_d = dense_plan(d_V).cpu().numpy()
+    assert np.abs(out - out_d).max() <= 1e-12 * np.abs(out_d).max()      # both plans, every sample
+    dense_plan.close()
     idx = sorted(set(list(range(32)) + [int(i) for i in np.linspace(0, n_sample - 1, 33)]))
     worst = check(out[idx], T.trace_bruteforce(topo, V[idx]), "trace5 bench launch")
     print(f"trace5: {n_sample} samples, {len(idx)} compared, max rel err {worst:.2e}, plan {tr.info()}")

@@ -23,7 +23,14 @@ def test_planned_program_equals_the_brute_force_trace_on_chains(name, topo):
     want = T.trace_bruteforce(topo, V)
     got = E.evaluate(topo, V)
     assert rel_err(got, want) < 1e-12, name
+    # plan made for charge-conserving vertices: structurally zero tile products are skipped
+    assert rel_err(E.evaluate(topo, V, charge=True), want) < 1e-12, name
+    Vd = TW.vertex_matrices(2, n, seed=1, stream=50 + n, dense=True)
+    assert rel_err(E.evaluate(topo, Vd), T.trace_bruteforce(topo, Vd)) < 1e-12, name
+    pc = E.plan(topo, charge=True)
     p = E.plan(topo)
+    if n >= 3:
+        assert p["dmma_products"] == 64 * (n - 2) and pc["dmma_products"] == 16 * (n - 2), (p, pc)
     assert p["max_open"] <= 4
     if n >= 2:
         assert p["n_sliced"] == 0                                      # chains need no slicing
@@ -45,6 +52,8 @@ def test_planned_program_equals_the_brute_force_trace_on_random_topologies(n, se
     want = T.trace_bruteforce(topo, V)
     got = E.evaluate(topo, V)
     assert rel_err(got, want) < 1e-12, (topo, p)
+    Vc = V * TW.charge_conserving_mask()
+    assert rel_err(E.evaluate(topo, Vc, charge=True), T.trace_bruteforce(topo, Vc)) < 1e-12, (topo, p)
     assert p["max_open"] <= 4 and p["n_sliced"] <= 3
     assert p["n_isospin"] == T.isospin_configs(topo)
     assert sorted(p["order"]) == list(range(n))

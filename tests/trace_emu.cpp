@@ -12,10 +12,11 @@ typedef std::complex<double> cplx;
 
 extern "C" {
 
-// info: [cmacs, max_open, n_sliced, n_isospin, n_slice_iter, order[6], (nA, nB, nC)[6]]
-int trace_emu_plan(int n, const int* topo, long long* info) {
+// info: [cmacs, max_open, n_sliced, n_isospin, n_slice_iter, order[6], (nA, nB, nC)[6], dmma_products]
+int trace_emu_plan(int n, const int* topo, int charge, long long* info) {
   TracePlan plan;
-  if (build_trace_plan(n, topo, plan) != 0) return 1;
+  if (build_trace_plan(n, topo, plan, charge != 0) != 0) return 1;
+  info[29] = plan.dmma_products;
   info[0] = plan.cmacs; info[1] = plan.max_open; info[2] = plan.n_sliced; info[3] = plan.n_isospin;
   info[4] = plan.n_slice_iter;
   for (int v = 0; v < 6; ++v) info[5 + v] = v < n ? plan.order[v] : -1;
@@ -28,9 +29,9 @@ int trace_emu_plan(int n, const int* topo, long long* info) {
 }
 
 // V: [n_sample][n][16][16][2]; out: [n_sample][2]
-int trace_emu_eval(int n, const int* topo, const double* V, long long n_sample, double* out) {
+int trace_emu_eval(int n, const int* topo, int charge, const double* V, long long n_sample, double* out) {
   TracePlan plan;
-  if (build_trace_plan(n, topo, plan) != 0) return 1;
+  if (build_trace_plan(n, topo, plan, charge != 0) != 0) return 1;
   std::vector<cplx> R(kTrMat), Rn(kTrMat), W(n * kTrMat);
   for (long long smp = 0; smp < n_sample; ++smp) {
     // the kernel's shared-memory image of the sample: every matrix row padded to kTrRow elements
@@ -49,15 +50,21 @@ int trace_emu_eval(int n, const int* topo, const double* V, long long n_sample, 
         for (int b = 0; b < s.nB; ++b)
           for (int a = 0; a < s.nA; ++a) {
             cplx v = 0;
-            for (int g = 0; g < s.nC; ++g) v += Rsrc[s.baseR[a] + s.offR[g]] * Wv[s.baseW[b] + s.offW[g]];
-            Rn[tr_pad(a + s.nA * b)] = v;
+            for (int g = 0; g < s.nC; ++g) {
+              // 16 x 16 x 16 steps: only the tile products the plan keeps (all of them unless it was made for
+              // charge-conserving vertices); a, b tiles of 8, k-steps of 4 in the plan's enumeration
+              if (s.big && !(s.tile_mask[g >> 2] >> (2 * (a >> 3) + (b >> 3)) & 1)) continue;
+              v += Rsrc[s.baseR[a] + s.offR[g]] * Wv[s.baseW[b] + s.offW[g]];
+            }
+            Rn[s.big ? s.outA[a] + s.outB[b] : tr_pad(a + s.nA * b)] = v;
           }
         R.swap(Rn);
         if (s.fuse_last) {                            // the last vertex closes everything: one dot product
           const TraceStep& sl = plan.steps[n - 1];
           const cplx* Wl = W.data() + sl.vertex * kTrMat + sl.sliceW[it];
           cplx t = 0;
-          for (int o = 0; o < 256; ++o) t += R[tr_pad(o)] * Wl[s.lastW[o]];
+          for (int b = 0; b < 16; ++b)
+            for (int a = 0; a < 16; ++a) t += R[s.outA[a] + s.outB[b]] * Wl[s.lastW[a + 16 * b]];
           R[0] = t;
         }
       }

@@ -21,24 +21,24 @@ def load():
     return _lib
 
 
-def plan(topo):
+def plan(topo, charge=False):
     t = np.ascontiguousarray(topo, dtype=np.int32).reshape(-1, 4)
-    info = np.zeros(29, dtype=np.int64)
-    rc = load().trace_emu_plan(t.shape[0], ctypes.c_void_p(t.ctypes.data), ctypes.c_void_p(info.ctypes.data))
+    info = np.zeros(30, dtype=np.int64)
+    rc = load().trace_emu_plan(t.shape[0], ctypes.c_void_p(t.ctypes.data), int(charge), ctypes.c_void_p(info.ctypes.data))
     if rc != 0:
         return None
     n = t.shape[0]
     return dict(cmacs=int(info[0]), max_open=int(info[1]), n_sliced=int(info[2]), n_isospin=int(info[3]),
-                n_slice_iter=int(info[4]), order=info[5:5 + n].tolist(),
+                n_slice_iter=int(info[4]), order=info[5:5 + n].tolist(), dmma_products=int(info[29]),
                 steps=[tuple(int(x) for x in info[11 + 3 * k:14 + 3 * k]) for k in range(n)])
 
 
-def evaluate(topo, V):
+def evaluate(topo, V, charge=False):
     t = np.ascontiguousarray(topo, dtype=np.int32).reshape(-1, 4)
     V = np.asarray(V, dtype=complex)
     Vd = np.ascontiguousarray(np.stack([V.real, V.imag], axis=-1))
     out = np.zeros((V.shape[0], 2))
-    rc = load().trace_emu_eval(t.shape[0], ctypes.c_void_p(t.ctypes.data), ctypes.c_void_p(Vd.ctypes.data),
+    rc = load().trace_emu_eval(t.shape[0], ctypes.c_void_p(t.ctypes.data), int(charge), ctypes.c_void_p(Vd.ctypes.data),
                                ctypes.c_longlong(V.shape[0]), ctypes.c_void_p(out.ctypes.data))
     if rc != 0:
         raise ValueError("topology rejected")
