@@ -21,8 +21,7 @@ using namespace no3n;
 namespace {
 
 struct DevTracePlan {
-  int n_vertex, n_slice_iter;
-  uint8_t n_groups, vgrp[kTrMaxVertex], pad_;     // load pipeline: executed steps, and which of them reads vertex v
+  int n_vertex, n_slice_iter, pad_[2];
   TraceStep steps[kTrMaxVertex];
 };
 static_assert(sizeof(TraceStep) % 16 == 0 && sizeof(DevTracePlan) % 16 == 0, "plan is staged with 16-byte copies");
@@ -48,10 +47,13 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
                : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
-// shared memory: plan (n_vertex steps) | per warp: (16 B unused) | vertex buffers [stages][n][16][17] complex | R [2][16][17] complex
+// shared memory: plan (n_vertex steps) | per warp: the scalar 1 (16 B) | vertex buffers [stages][n][16][17] complex | R [1 or 2][16][17] complex
 __host__ __device__ inline size_t trace_plan_bytes(int n) { return 16 + (size_t)n * sizeof(TraceStep); }
-__host__ __device__ inline size_t trace_warp_bytes(int n, int stages) {
-  return 16 + (size_t)(stages * n + 2) * kTrMat * 16;
+// Partial results ping-pong between a dedicated buffer and, when every vertex is read only once (no sliced lines), the
+// slot of the first absorbed vertex, which is dead by the time the second buffer is first written (r_bufs = 1);
+// with sliced lines the vertices are re-read in every outer iteration and both buffers are dedicated (r_bufs = 2).
+__host__ __device__ inline size_t trace_warp_bytes(int n, int stages, int r_bufs) {
+  return 16 + (size_t)(stages * n * kTrMatW + r_bufs * kTrMat) * 16;
 }
 
 // request vertex matrix v of a sample: 256 complex numbers, one 16-byte cp.async (LDGSTS) per lane and element --
@@ -63,29 +65,15 @@ __device__ __forceinline__ void request_vertex(double2* dst, const double2* src,
   for (int j = 0; j < 8; ++j) {
     const int rc = lane + 32 * j;
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;"
-                 ::"r"(smem_u32(dst + v * kTrMat + rc + (rc >> 4))), "l"(src + v * 256 + rc) : "memory");
+                 ::"r"(smem_u32(dst + v * kTrMatW + (rc >> 4) * kTrRowW + (rc & 15))), "l"(src + v * 256 + rc) : "memory");
   }
 }
 
-// the vertices read by executed step g (all of them if g < 0) of the sample at src, as ONE cp.async group
-__device__ __forceinline__ void request_group(double2* dst, const double2* src, int n, const uint8_t* vgrp, int g, bool valid,
-                                              int lane) {
+// all n vertex matrices of the sample at src as ONE cp.async group
+__device__ __forceinline__ void request_sample(double2* dst, const double2* src, int n, bool valid, int lane) {
   if (valid)
-    for (int v = 0; v < n; ++v)
-      if (g < 0 || vgrp[v] == g) request_vertex(dst, src, v, lane);
+    for (int v = 0; v < n; ++v) request_vertex(dst, src, v, lane);
   asm volatile("cp.async.commit_group;" ::: "memory");
-}
-
-// wait until at most `pending` of this thread's most recent cp.async groups are still in flight
-__device__ __forceinline__ void wait_groups(int pending) {
-  switch (pending) {
-    case 0: asm volatile("cp.async.wait_group 0;" ::: "memory"); break;
-    case 1: asm volatile("cp.async.wait_group 1;" ::: "memory"); break;
-    case 2: asm volatile("cp.async.wait_group 2;" ::: "memory"); break;
-    case 3: asm volatile("cp.async.wait_group 3;" ::: "memory"); break;
-    case 4: asm volatile("cp.async.wait_group 4;" ::: "memory"); break;
-    default: asm volatile("cp.async.wait_group 5;" ::: "memory"); break;
-  }
 }
 
 // path: 0 = vector FP64 (DFMA) register tiles, 1 = FP64 tensor cores (DMMA m8n8k4) for the 16 x 16 x 16 steps
@@ -103,62 +91,53 @@ trace_kernel(const DevTracePlan* __restrict__ plan_g, const double2* __restrict_
     for (int i = threadIdx.x; i < n16; i += blockDim.x) dst[i] = src[i];
   }
   const TraceStep* steps = reinterpret_cast<const TraceStep*>(tsm + 16);
-  unsigned char* wb = tsm + trace_plan_bytes(n) + (size_t)warp * trace_warp_bytes(n, stages);
+  const int r_bufs = n_iter == 1 ? 1 : 2;
+  unsigned char* wb = tsm + trace_plan_bytes(n) + (size_t)warp * trace_warp_bytes(n, stages, r_bufs);
+  double2* one = reinterpret_cast<double2*>(wb);                         // the empty contraction: the scalar 1
   double2* vbuf = reinterpret_cast<double2*>(wb + 16);                   // [stages][n][16][17]
-  double2* Rb = vbuf + (size_t)stages * n * kTrMat;                      // [2][16][17]
+  double2* Rb = vbuf + (size_t)stages * n * kTrMatW;                      // [r_bufs][16][17]
+  if (lane == 0) *one = make_double2(1.0, 0.0);
   __syncthreads();
 
   const long long first = (long long)blockIdx.x * n_warps + warp, stride = (long long)gridDim.x * n_warps;
-  // Load pipeline.  stages == 1 (default): ONE set of vertex slots per warp.  A vertex is read by exactly one executed
-  // step, so right after step g of this sample the copies of the NEXT sample's vertices of step g are issued into
-  // the same slots (one cp.async group per executed step); before step g of the next sample at most n_groups - 1
-  // younger groups may still be in flight.  The copies of a sample thus run under the arithmetic of the previous one
-  // without a second buffer (shared memory decides how many samples an SM keeps in flight).  With sliced lines every
-  // vertex is read in every outer iteration: the whole sample is one group, requested after the last iteration.
-  const uint8_t* vgrp = reinterpret_cast<const DevTracePlan*>(tsm)->vgrp;
-  const int n_groups = n_iter == 1 && stages == 1 ? reinterpret_cast<const DevTracePlan*>(tsm)->n_groups : 1;
-  const bool piped = n_groups > 1;
-  if (piped) {
-    for (int g = 0; g < n_groups; ++g) request_group(vbuf, V + first * n * 256, n, vgrp, g, first < n_sample, lane);
-  } else {
-    request_group(vbuf, V + first * n * 256, n, vgrp, -1, first < n_sample, lane);
-  }
+  // Loads.  Default (stages = 1): ONE set of vertex slots per warp; the whole next sample is requested when this sample
+  // is done and awaited at the top of the loop: the other warps of the SM compute meanwhile (8 warps per SM at fifth
+  // order).  Measured alternatives, both slower (profiles/r02b.md): requesting the next sample's vertices step by step
+  // as their slots fall free (one cp.async group per executed step: -11 %, the copies compete with the fragment
+  // loads of the running steps), and stages = 2, a second set of slots per warp (4 warps per SM instead of 7).
+  request_sample(vbuf, V + first * n * 256, n, first < n_sample, lane);
   int stage = 0;
   for (long long smp = first; smp < n_sample; smp += stride) {
     const long long nxt = smp + stride;
-    if (!piped) {
-      if (stages == 2) {
-        // the other buffer's last readers finished before the __syncwarp that ended the previous iteration
-        request_group(vbuf + (size_t)(stage ^ 1) * n * kTrMat, V + nxt * n * 256, n, vgrp, -1, nxt < n_sample, lane);
-        wait_groups(1);                                  // this sample has landed; the next one is in flight
-      } else {
-        wait_groups(0);
-      }
-      __syncwarp();
+    if (stages == 2) {
+      // the other buffer's last readers finished before the __syncwarp that ended the previous iteration
+      request_sample(vbuf + (size_t)(stage ^ 1) * n * kTrMatW, V + nxt * n * 256, n, nxt < n_sample, lane);
+      asm volatile("cp.async.wait_group 1;" ::: "memory");      // this sample has landed; the next one is in flight
+    } else {
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
     }
-    const double2* W = vbuf + (size_t)stage * n * kTrMat;
+    __syncwarp();
+    const double2* W = vbuf + (size_t)stage * n * kTrMatW;
 
     double2 total = make_double2(0.0, 0.0);
     for (int it = 0; it < n_iter; ++it) {
-      double2* Rin = Rb;
-      double2* Rout = Rb + kTrMat;
+      double2* const RA = Rb;
+      // second buffer: dedicated, or the slot of the first absorbed vertex (its matrix is consumed by the first
+      // executed step, whose result goes to RA; the padded row strides of the two layouts are the same)
+      double2* const RB = r_bufs == 2 ? Rb + kTrMat : vbuf + ((size_t)stage * n + steps[0].vertex) * kTrMatW;
+      const double2* Rin = one;                         // nothing open, nothing contracted yet
       double2 last = make_double2(0.0, 0.0);
-      if (lane == 0) Rin[0] = make_double2(1.0, 0.0);     // nothing open, nothing contracted yet: the scalar 1
-      __syncwarp();
       for (int k = 0; k < n; ++k) {
         const TraceStep& s = steps[k];
         if (s.skip) continue;                           // folded into a neighbouring step (warp uniform)
-        if (piped) {                                    // the vertices of this step have landed
-          wait_groups(n_groups - 1);
-          __syncwarp();
-        }
-        const double2* Wv = W + s.vertex * kTrMat + s.sliceW[it];
+        const double2* Wv = W + s.vertex * kTrMatW + s.sliceW[it];
         const int nA = s.nA, nB = s.nB, nC = s.nC, nOut = nA * nB;
+        double2* const Rout = Rin == RA ? RB : RA;
         if (s.big) {
           // R of this step: the partial result, or (first vertex folded in) the first vertex's matrix itself
-          const double2* Rs = s.r_vertex >= 0 ? W + s.r_vertex * kTrMat + steps[0].sliceW[it] : Rin;
+          const double2* Rs = s.r_vertex >= 0 ? W + s.r_vertex * kTrMatW + steps[0].sliceW[it] : Rin;
           // last vertex folded in: it closes all four lines, T = sum_{a,b} R'[a,b] W_last[lastW[a + 16 b]]
-          const double2* Wl = s.fuse_last ? W + steps[n - 1].vertex * kTrMat + steps[n - 1].sliceW[it] : nullptr;
+          const double2* Wl = s.fuse_last ? W + steps[n - 1].vertex * kTrMatW + steps[n - 1].sliceW[it] : nullptr;
           double2 dot = make_double2(0.0, 0.0);
           if (path == 1 && s.block_diag) {
             // charge-conserving vertices: the product is block diagonal in the isospin-pair enumeration, two 8 x 8 x 8
@@ -307,16 +286,14 @@ trace_kernel(const DevTracePlan* __restrict__ plan_g, const double2* __restrict_
           if (nOut == 1) last = v;
         }
         __syncwarp();
-        // the slots this step read are free: request the same vertices of the warp's next sample
-        if (piped) request_group(vbuf, V + nxt * n * 256, n, vgrp, s.grp, nxt < n_sample, lane);
-        double2* t = Rin; Rin = Rout; Rout = t;
+        Rin = Rout;
       }
       total.x += last.x; total.y += last.y;
     }
     if (lane == 0) out[smp] = total;
     __syncwarp();
     if (stages == 2) stage ^= 1;
-    else if (!piped) request_group(vbuf, V + nxt * n * 256, n, vgrp, -1, nxt < n_sample, lane);
+    else request_sample(vbuf, V + nxt * n * 256, n, nxt < n_sample, lane);
   }
 }
 
@@ -377,7 +354,8 @@ int no_trace_init(no_trace_plan** out, int n_vertex, const int* topo, int flags,
   if (const char* e = getenv("NO3N_TRACE_STAGES")) { const int v = atoi(e); if (v == 1 || v == 2) p->stages = v; }   // tuning knobs
   if (const char* e = getenv("NO3N_TRACE_PATH")) { const int v = atoi(e); if (v == 0 || v == 1) p->path = v; }
   const size_t avail = (size_t)smem_optin - trace_plan_bytes(n_vertex) - 128;
-  int warps = (int)(avail / trace_warp_bytes(n_vertex, p->stages));
+  const int r_bufs = p->plan.n_slice_iter == 1 ? 1 : 2;
+  int warps = (int)(avail / trace_warp_bytes(n_vertex, p->stages, r_bufs));
   if (warps > 16) warps = 16;
   if (const char* e = getenv("NO3N_TRACE_WARPS")) { const int v = atoi(e); if (v >= 1 && v < warps) warps = v; }
   if (warps < 1) { delete p; return NO_ERR_INVALID; }
@@ -387,9 +365,7 @@ int no_trace_init(no_trace_plan** out, int n_vertex, const int* topo, int flags,
   DevTracePlan hp;
   hp.n_vertex = p->plan.n_vertex;
   hp.n_slice_iter = p->plan.n_slice_iter;
-  hp.n_groups = (uint8_t)p->plan.n_groups;
-  for (int v = 0; v < kTrMaxVertex; ++v) hp.vgrp[v] = (uint8_t)(v < p->plan.n_vertex ? p->plan.vgrp[v] : 255);
-  hp.pad_ = 0;
+  hp.pad_[0] = hp.pad_[1] = 0;
   for (int k = 0; k < kTrMaxVertex; ++k) hp.steps[k] = p->plan.steps[k];
   e = cudaMalloc((void**)&p->d_plan, sizeof(DevTracePlan));
   if (e != cudaSuccess) { delete p; trace_cuda_fail(e, "cudaMalloc(trace plan)"); return NO_ERR_ALLOC; }
@@ -415,7 +391,7 @@ int no_trace_eval(const no_trace_plan* p, const double* d_vertices, long long n_
   } else {
     blocks = p->n_sm;
   }
-  const size_t smem = trace_plan_bytes(p->plan.n_vertex) + (size_t)warps * trace_warp_bytes(p->plan.n_vertex, p->stages);
+  const size_t smem = trace_plan_bytes(p->plan.n_vertex) + (size_t)warps * trace_warp_bytes(p->plan.n_vertex, p->stages, p->plan.n_slice_iter == 1 ? 1 : 2);
   trace_kernel<<<(unsigned)blocks, warps * 32, smem, static_cast<cudaStream_t>(cuda_stream)>>>(
       p->d_plan, reinterpret_cast<const double2*>(d_vertices), n_sample, reinterpret_cast<double2*>(d_out), p->stages,
       p->path);

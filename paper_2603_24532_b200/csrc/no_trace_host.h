@@ -45,12 +45,17 @@ constexpr int kTrTab = 256;
 constexpr int kTrRow = 17;
 constexpr int kTrMat = 16 * kTrRow;  // elements of one padded 16 x 16 matrix
 inline int tr_pad(int idx) { return idx + (idx >> 4); }   // canonical index (16 row + col) -> padded offset
+// row stride of the VERTEX matrices in shared memory: padded like R (written by 16-byte cp.async).  Unpadded rows
+// filled by one TMA bulk copy per vertex were measured too: 2.12e8 against 2.43e8 samples/s (profiles/r02b.md)
+constexpr int kTrRowW = kTrRow;
+constexpr int kTrMatW = 16 * kTrRowW;
+inline int tr_padw(int idx) { return (idx >> 4) * kTrRowW + (idx & 15); }
 
 inline int slot_off(int slot, int x) {
   const int s = x >> 1, t = x & 1;
   switch (slot) {
-    case 0: return kTrRow * (8 * s + 2 * t);    // outgoing 1: row bits s1, t1
-    case 1: return kTrRow * (4 * s + t);        // outgoing 2: row bits s2, t2
+    case 0: return kTrRowW * (8 * s + 2 * t);   // outgoing 1: row bits s1, t1
+    case 1: return kTrRowW * (4 * s + t);       // outgoing 2: row bits s2, t2
     case 2: return 8 * s + 2 * t;               // incoming 1: column bits
     default: return 4 * s + t;                  // incoming 2
   }
@@ -82,8 +87,7 @@ struct TraceStep {
   // ks_valid bit ks: the k-step contributes).
   uint8_t tile_mask[4];
   uint8_t block_diag, ks_valid;
-  uint8_t grp;                // index of this step among the executed (not skipped) steps
-  uint8_t pad2_[9];
+  uint8_t pad2_[10];
 };
 
 struct TracePlan {
@@ -97,10 +101,6 @@ struct TracePlan {
   long long n_isospin;        // charge-conserving isospin assignments of the lines, for information
   long long dmma_products;    // 8 x 8 x 4 real tensor-core products per sample in the 16 x 16 x 16 steps (after skipping)
   int charge;                 // 1: planned for charge-conserving vertices (structurally zero tiles are skipped)
-  // load pipeline of the kernel: a vertex matrix is read by exactly one executed step, so its shared-memory slot is
-  // free for the NEXT sample's copy as soon as that step is done: n_groups executed steps, vgrp[v] = the one reading v
-  int n_groups;
-  int vgrp[kTrMaxVertex];
   TraceStep steps[kTrMaxVertex];
 };
 
@@ -363,16 +363,6 @@ inline int build_trace_plan(int n, const int* topo, TracePlan& plan, bool charge
       for (int b = 0; b < 16; ++b) sp.lastW[a + 16 * b] = by_offset[sp.outA[a] + sp.outB[b]];
     sp.fuse_last = 1;
     sl.skip = 1;
-  }
-  plan.n_groups = 0;
-  for (int k = 0; k < n; ++k) {
-    TraceStep& st = plan.steps[k];
-    st.grp = 0;
-    if (st.skip) continue;
-    st.grp = (uint8_t)plan.n_groups++;
-    plan.vgrp[st.vertex] = st.grp;
-    if (st.r_vertex >= 0) plan.vgrp[st.r_vertex] = st.grp;
-    if (st.fuse_last) plan.vgrp[plan.steps[n - 1].vertex] = st.grp;
   }
   return 0;
 }

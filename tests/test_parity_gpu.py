@@ -524,6 +524,16 @@ def test_fp64_probe_reports_a_sane_peak():
     print("FP64 DFMA probe:", r)
 
 
+def test_fp64_operand_probe_shows_the_three_register_operand_penalty():
+    """the rule the hot loop is arranged around: a DFMA with three distinct 64-bit register
+    operands holds the FP64 pipe for 3 cycles instead of 2, i.e. runs at about two thirds of the rate"""
+    r = binding.no_probe_fp64_operands(0, 100)
+    ratio = r["three_operands_tflops"] / r["two_operands_tflops"]
+    print("FP64 operand probe:", r, f"ratio {ratio:.3f}")
+    assert 1.0 < r["two_operands_tflops"] < 100.0
+    assert 0.55 < ratio < 0.8
+
+
 def test_native_library_is_the_one_loaded():
     maps = open(f"/proc/{os.getpid()}/maps").read()
     assert "libno3n.so" in maps

@@ -32,12 +32,12 @@ int trace_emu_plan(int n, const int* topo, int charge, long long* info) {
 int trace_emu_eval(int n, const int* topo, int charge, const double* V, long long n_sample, double* out) {
   TracePlan plan;
   if (build_trace_plan(n, topo, plan, charge != 0) != 0) return 1;
-  std::vector<cplx> R(kTrMat), Rn(kTrMat), W(n * kTrMat);
+  std::vector<cplx> R(kTrMat), Rn(kTrMat), W(n * kTrMatW);
   for (long long smp = 0; smp < n_sample; ++smp) {
     // the kernel's shared-memory image of the sample: every matrix row padded to kTrRow elements
     const cplx* Vs = reinterpret_cast<const cplx*>(V) + smp * n * 256;
     for (int v = 0; v < n; ++v)
-      for (int e = 0; e < 256; ++e) W[v * kTrMat + tr_pad(e)] = Vs[v * 256 + e];
+      for (int e = 0; e < 256; ++e) W[v * kTrMatW + tr_padw(e)] = Vs[v * 256 + e];
     cplx total = 0;
     for (int it = 0; it < plan.n_slice_iter; ++it) {
       R.assign(kTrMat, cplx(0, 0));
@@ -45,8 +45,8 @@ int trace_emu_eval(int n, const int* topo, int charge, const double* V, long lon
       for (int k = 0; k < n; ++k) {
         const TraceStep& s = plan.steps[k];
         if (s.skip) continue;                         // folded into a neighbouring step
-        const cplx* Wv = W.data() + s.vertex * kTrMat + s.sliceW[it];
-        const cplx* Rsrc = s.r_vertex >= 0 ? W.data() + s.r_vertex * kTrMat + plan.steps[0].sliceW[it] : R.data();
+        const cplx* Wv = W.data() + s.vertex * kTrMatW + s.sliceW[it];
+        const cplx* Rsrc = s.r_vertex >= 0 ? W.data() + s.r_vertex * kTrMatW + plan.steps[0].sliceW[it] : R.data();
         for (int b = 0; b < s.nB; ++b)
           for (int a = 0; a < s.nA; ++a) {
             cplx v = 0;
@@ -61,7 +61,7 @@ int trace_emu_eval(int n, const int* topo, int charge, const double* V, long lon
         R.swap(Rn);
         if (s.fuse_last) {                            // the last vertex closes everything: one dot product
           const TraceStep& sl = plan.steps[n - 1];
-          const cplx* Wl = W.data() + sl.vertex * kTrMat + sl.sliceW[it];
+          const cplx* Wl = W.data() + sl.vertex * kTrMatW + sl.sliceW[it];
           cplx t = 0;
           for (int b = 0; b < 16; ++b)
             for (int a = 0; a < 16; ++a) t += R[s.outA[a] + s.outB[b]] * Wl[s.lastW[a + 16 * b]];
