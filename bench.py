@@ -329,6 +329,33 @@ def run_b200(args, workload):
     value = replicas.whole_job_rate(evals_step, args.steps, t_dev)
     n_launch = len(runs) * args.steps
 
+    # ---- the same step writing the packed, symmetry-reduced form (no_eval_packed; device resident, not the headline) ----
+    packed_dev = None
+    if world == 1:
+        pk = []
+        for h, r in zip(handles, runs):
+            fmt = binding.NO_PACK_ISOSPIN if binding.no_packed_doubles(h, binding.NO_PACK_ISOSPIN) else binding.NO_PACK_CHARGE
+            pk.append((fmt, torch.empty((r.n_cfg, binding.no_packed_doubles(h, fmt)), dtype=torch.float64, device=dev)))
+
+        def step_packed():
+            for h, c, r, (fmt, o) in zip(handles, dw.d_cfg, runs, pk):
+                binding.no_eval_packed(h, fmt, c.data_ptr(), r.n_cfg, o.data_ptr(), stream.cuda_stream)
+
+        step_packed()
+        kp = max(1, min(args.steps, 3))
+        evp = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(kp)]
+        for a, b in evp:
+            flush.zero_()
+            a.record(stream)
+            step_packed()
+            b.record(stream)
+        torch.cuda.synchronize(dev)
+        ms = sum(a.elapsed_time(b) for a, b in evp)
+        packed_dev = {"evals_per_s": evals_step * kp / (ms * 1e-3), "steps": kp,
+                      "bytes_out_per_step": int(sum(o.numel() * 8 for _, o in pk)),
+                      "api": "no_eval_packed (isospin form where kF_n = kF_p, charge form otherwise), outputs resident in HBM"}
+        del pk
+
     # ---- end to end through the C ABI with HOST buffers (H2D + D2H inside the timed region) ----
     # e2e: no_eval_host_packed, the symmetry-reduced form the paper describes (isospin form for runs
     # with kF_n = kF_p, charge-conserving form otherwise; the full matrix follows by an index map, no_unpack);
@@ -431,7 +458,7 @@ def run_b200(args, workload):
                        "cfg_per_s": world * workload.n_cfg * args.steps / t_dev,
                        "l2": "256 MiB buffer rewritten between timed steps (L2 flush); the kernel is ALU bound",
                        "parallelism": "replicas only: every rank integrates the whole workload",
-                       "per_config": per_config, "small_transactions": small},
+                       "per_config": per_config, "small_transactions": small, "packed_output": packed_dev},
             "clocks": clocks, "e2e": e2e, "e2e_full_matrices": e2e_full, "gpu_launches": n_launch, "roofline": roofline, "cpu_baseline": cpu,
             "wall_s_timed_region": t_wall}
     print(json.dumps(line), flush=True)
@@ -660,6 +687,25 @@ def run_trace(args):
     torch.cuda.synchronize(dev)
     dense_rate = n_sample * len(ed) / (sum(a.elapsed_time(b) for a, b in ed) * 1e-3)
     binding.no_trace_free(plan_d)
+    # the same launch reading the vertices in the packed form no_eval_packed writes (1536 B per vertex)
+    d_P = torch.from_numpy(TW.pack_charge(V)).to(dev)
+    d_out_p = torch.empty_like(d_out)
+    for _ in range(3):
+        binding.no_trace_eval_packed(plan, binding.NO_PACK_CHARGE, d_P.data_ptr(), n_sample, d_out_p.data_ptr(), stream.cuda_stream)
+    ep = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(10)]
+    for a, b in ep:
+        flush.zero_()
+        a.record(stream)
+        binding.no_trace_eval_packed(plan, binding.NO_PACK_CHARGE, d_P.data_ptr(), n_sample, d_out_p.data_ptr(), stream.cuda_stream)
+        b.record(stream)
+    torch.cuda.synchronize(dev)
+    assert torch.equal(d_out_p, d_out)
+    packed_ms = sum(a.elapsed_time(b) for a, b in ep) / len(ep)
+    packed_in = {"samples_per_s": n_sample / (packed_ms * 1e-3), "avg_launch_ms": packed_ms,
+                 "bytes_per_sample": n * 1536 + 16,
+                 "hbm_gbs": n_sample * (n * 1536 + 16) / (packed_ms * 1e-3) / 1e9,
+                 "api": "no_trace_eval_packed (NO_PACK_CHARGE vertices, 2.0 GB per launch)"}
+    del d_P
     bytes_step = n_sample * (n * 4096 + 16)
     peak, peak_src = hbm_peak_gbs()
     achieved = bytes_step * steps / (sum(step_ms) * 1e-3) / 1e9
@@ -741,7 +787,7 @@ def run_trace(args):
                      "fp64_tflops": flops_step * steps / (sum(step_ms) * 1e-3) / 1e12,
                      "fp64_frac_of_nominal": flops_step * steps / (sum(step_ms) * 1e-3) / 1e12 / FP64_PEAK_NOMINAL_TFLOPS,
                      "flops_per_sample": flops_sample,
-                     "dense_plan_samples_per_s": dense_rate,
+                     "dense_plan_samples_per_s": dense_rate, "packed_input": packed_in,
                      "dense_plan_flops_per_sample": 8.0 * info["cmacs_per_sample"]},
         "cpu_baseline": cpu}), flush=True)
 

@@ -64,6 +64,16 @@ int no_trace_init(no_trace_plan **plan, int n_vertex, const int *topo, int flags
 int no_trace_eval(const no_trace_plan *plan, const double *d_vertices, long long n_sample, double *d_out,
                   void *cuda_stream);
 
+/* no_trace_eval reading the vertex matrices in the packed form NO_PACK_CHARGE of include/no.h (what no_eval_packed
+ * writes: the 96 charge-conserving entries, 1536 bytes per vertex instead of 4096): the kernel scatters
+ * them into zeroed shared-memory matrices, so 7.7 instead of 20.5 KB per fifth-order sample cross HBM.
+ *   format   : NO_PACK_CHARGE (NO_ERR_INVALID otherwise)
+ *   d_packed : DEVICE, const, [n_sample][n_vertex][96][2] doubles, 16-byte aligned, dense, caller-owned
+ * Otherwise as no_trace_eval; works with plans made with or without NO_TRACE_CHARGE_CONSERVING (the packed form cannot
+ * express a charge-violating entry) and gives the same bits as no_trace_eval on the unpacked matrices. */
+int no_trace_eval_packed(const no_trace_plan *plan, int format, const double *d_packed, long long n_sample, double *d_out,
+                         void *cuda_stream);
+
 /* Facts about a plan (each pointer may be NULL): complex multiply-adds per sample of the planned contraction,
  * widest frontier (open lines), number of sliced lines, number of charge-conserving isospin assignments of the lines
  * ("the subset of isospin configurations consistent with isospin conservation at each vertex"), the

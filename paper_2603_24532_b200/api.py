@@ -135,6 +135,18 @@ class SpinIsospinTrace:
         s = stream if stream is not None else torch.cuda.current_stream(vertices.device)
         binding.no_trace_eval(self._p, vertices.data_ptr(), n, out.data_ptr(), s.cuda_stream)
 
+    def from_packed(self, packed: torch.Tensor) -> torch.Tensor:
+        """no_trace_eval_packed: packed complex128 CUDA tensor [n_sample, n_vertex, 96] (NormalOrdering.packed(cfg, 1)
+        reshaped) -> complex128 [n_sample]."""
+        assert packed.is_cuda and packed.dtype == torch.complex128
+        packed = packed.contiguous()
+        n = packed.numel() // (self.n_vertex * 96)
+        assert packed.numel() == n * self.n_vertex * 96
+        out = torch.empty((n,), dtype=torch.complex128, device=packed.device)
+        binding.no_trace_eval_packed(self._p, binding.NO_PACK_CHARGE, packed.data_ptr(), n, out.data_ptr(),
+                                     torch.cuda.current_stream(packed.device).cuda_stream)
+        return out
+
     def __call__(self, vertices: torch.Tensor) -> torch.Tensor:
         vertices = vertices.contiguous()
         n = vertices.numel() // (self.n_vertex * 256)

@@ -21,7 +21,8 @@ EXPORTS = ("no_init", "no_init_angular", "no_eval", "no_eval_host", "no_eval_dia
 
 NO_PACK_CHARGE, NO_PACK_ISOSPIN = 1, 2
 
-TRACE_EXPORTS = ("no_trace_init", "no_trace_eval", "no_trace_info", "no_trace_free", "no_trace_last_cuda_error")
+TRACE_EXPORTS = ("no_trace_init", "no_trace_eval", "no_trace_eval_packed", "no_trace_info", "no_trace_free",
+                 "no_trace_last_cuda_error")
 
 
 class no_params(ctypes.Structure):
@@ -85,6 +86,9 @@ def load() -> ctypes.CDLL:
         lib.no_probe_fp64_operands.restype = ctypes.c_int
         lib.no_trace_init.argtypes = [ctypes.POINTER(H), ctypes.c_int, ctypes.c_void_p, ctypes.c_int, ctypes.c_int]
         lib.no_trace_eval.argtypes = [H, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]
+        lib.no_trace_eval_packed.argtypes = [H, ctypes.c_int, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p,
+                                             ctypes.c_void_p]
+        lib.no_trace_eval_packed.restype = ctypes.c_int
         lib.no_trace_info.argtypes = [H, ctypes.POINTER(ctypes.c_longlong), ip, ip, ctypes.POINTER(ctypes.c_longlong), ip,
                                       ctypes.POINTER(ctypes.c_longlong)]
         lib.no_trace_free.argtypes = [H]
@@ -259,6 +263,15 @@ def no_trace_eval(plan, d_vertices_ptr: int, n_sample: int, d_out_ptr: int, stre
                               ctypes.c_void_p(stream_ptr or 0))
     if rc != NO_OK:
         raise NoError(rc, "no_trace_eval")
+
+
+def no_trace_eval_packed(plan, fmt: int, d_packed_ptr: int, n_sample: int, d_out_ptr: int,
+                         stream_ptr: Optional[int] = None) -> None:
+    """no_trace_eval_packed with raw DEVICE pointers: packed vertices [n_sample][n_vertex][96][2] (NO_PACK_CHARGE)."""
+    rc = load().no_trace_eval_packed(plan, fmt, ctypes.c_void_p(d_packed_ptr), n_sample, ctypes.c_void_p(d_out_ptr),
+                                     ctypes.c_void_p(stream_ptr or 0))
+    if rc != NO_OK:
+        raise NoError(rc, "no_trace_eval_packed")
 
 
 def no_trace_info(plan, n_vertex: int) -> dict:

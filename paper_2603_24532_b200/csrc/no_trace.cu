@@ -69,17 +69,42 @@ __device__ __forceinline__ void request_vertex(double2* dst, const double2* src,
   }
 }
 
+// Packed input (NO_PACK_CHARGE of include/no.h: the 96 charge-conserving entries, [16 spin elements][6 isospin blocks]):
+// padded offset of packed entry pk inside a vertex slot, and of the z-th of the 160 entries that form cannot hold
+__device__ __forceinline__ int packed_pos(int pk) {
+  const int sp = pk / 6, nb = pk - 6 * sp;
+  const int to = nb < 4 ? nb : nb - 3, ti = nb < 4 ? nb : 6 - nb;
+  return (4 * (sp >> 2) + to) * kTrRowW + 4 * (sp & 3) + ti;
+}
+__device__ __forceinline__ int forbidden_pos(int z) {
+  const int sp = z / 10, nz = z - 10 * sp;
+  // (to, ti) over (0,1) (0,2) (0,3) (1,0) (1,3) (2,0) (2,3) (3,0) (3,1) (3,2)
+  const int to = (int)((0x3332211000ULL >> (4 * nz)) & 15), ti = (int)((0x2103030321ULL >> (4 * nz)) & 15);
+  return (4 * (sp >> 2) + to) * kTrRowW + 4 * (sp & 3) + ti;
+}
+__device__ __forceinline__ void request_vertex_packed(double2* dst, const double2* src, int v, int lane) {
+#pragma unroll
+  for (int j = 0; j < 3; ++j) {
+    const int pk = lane + 32 * j;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;"
+                 ::"r"(smem_u32(dst + v * kTrMatW + packed_pos(pk))), "l"(src + v * 96 + pk) : "memory");
+  }
+}
+
 // all n vertex matrices of the sample at src as ONE cp.async group
-__device__ __forceinline__ void request_sample(double2* dst, const double2* src, int n, bool valid, int lane) {
+__device__ __forceinline__ void request_sample(double2* dst, const double2* src, int n, bool valid, int lane, int packed) {
   if (valid)
-    for (int v = 0; v < n; ++v) request_vertex(dst, src, v, lane);
+    for (int v = 0; v < n; ++v) {
+      if (packed) request_vertex_packed(dst, src, v, lane);
+      else request_vertex(dst, src, v, lane);
+    }
   asm volatile("cp.async.commit_group;" ::: "memory");
 }
 
 // path: 0 = vector FP64 (DFMA) register tiles, 1 = FP64 tensor cores (DMMA m8n8k4) for the 16 x 16 x 16 steps
 __global__ void __launch_bounds__(512, 1)
 trace_kernel(const DevTracePlan* __restrict__ plan_g, const double2* __restrict__ V, long long n_sample,
-             double2* __restrict__ out, int stages, int path) {
+             double2* __restrict__ out, int stages, int path, int packed) {
   extern __shared__ __align__(128) unsigned char tsm[];
   const int n = plan_g->n_vertex, n_iter = plan_g->n_slice_iter;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
@@ -97,6 +122,9 @@ trace_kernel(const DevTracePlan* __restrict__ plan_g, const double2* __restrict_
   double2* vbuf = reinterpret_cast<double2*>(wb + 16);                   // [stages][n][16][17]
   double2* Rb = vbuf + (size_t)stages * n * kTrMatW;                      // [r_bufs][16][17]
   if (lane == 0) *one = make_double2(1.0, 0.0);
+  const int vs = packed ? 96 : 256;                                       // complex numbers per vertex in HBM
+  if (packed)                                                             // the entries the packed form leaves out stay zero
+    for (int i = lane; i < stages * n * kTrMatW; i += 32) vbuf[i] = make_double2(0.0, 0.0);
   __syncthreads();
 
   const long long first = (long long)blockIdx.x * n_warps + warp, stride = (long long)gridDim.x * n_warps;
@@ -105,13 +133,13 @@ trace_kernel(const DevTracePlan* __restrict__ plan_g, const double2* __restrict_
   // order).  Measured alternatives, both slower (profiles/r02b.md): requesting the next sample's vertices step by step
   // as their slots fall free (one cp.async group per executed step: -11 %, the copies compete with the fragment
   // loads of the running steps), and stages = 2, a second set of slots per warp (4 warps per SM instead of 7).
-  request_sample(vbuf, V + first * n * 256, n, first < n_sample, lane);
+  request_sample(vbuf, V + first * n * vs, n, first < n_sample, lane, packed);
   int stage = 0;
   for (long long smp = first; smp < n_sample; smp += stride) {
     const long long nxt = smp + stride;
     if (stages == 2) {
       // the other buffer's last readers finished before the __syncwarp that ended the previous iteration
-      request_sample(vbuf + (size_t)(stage ^ 1) * n * kTrMatW, V + nxt * n * 256, n, nxt < n_sample, lane);
+      request_sample(vbuf + (size_t)(stage ^ 1) * n * kTrMatW, V + nxt * n * vs, n, nxt < n_sample, lane, packed);
       asm volatile("cp.async.wait_group 1;" ::: "memory");      // this sample has landed; the next one is in flight
     } else {
       asm volatile("cp.async.wait_group 0;" ::: "memory");
@@ -292,8 +320,15 @@ trace_kernel(const DevTracePlan* __restrict__ plan_g, const double2* __restrict_
     }
     if (lane == 0) out[smp] = total;
     __syncwarp();
+    if (packed && r_bufs == 1) {
+      // the slot of the first absorbed vertex served as the second partial-result buffer: the entries the packed
+      // form does not carry must be zero again before the slot's next sample is used
+      double2* slot = vbuf + ((size_t)stage * n + steps[0].vertex) * kTrMatW;
+#pragma unroll
+      for (int j = 0; j < 5; ++j) slot[forbidden_pos(lane + 32 * j)] = make_double2(0.0, 0.0);
+    }
     if (stages == 2) stage ^= 1;
-    else request_sample(vbuf, V + nxt * n * 256, n, nxt < n_sample, lane);
+    else request_sample(vbuf, V + nxt * n * vs, n, nxt < n_sample, lane, packed);
   }
 }
 
@@ -375,7 +410,22 @@ int no_trace_init(no_trace_plan** out, int n_vertex, const int* topo, int flags,
   return NO_OK;
 }
 
+namespace {
+int trace_launch(const no_trace_plan* p, const double* d_vertices, long long n_sample, double* d_out, void* cuda_stream, int packed);
+}
+
 int no_trace_eval(const no_trace_plan* p, const double* d_vertices, long long n_sample, double* d_out, void* cuda_stream) {
+  return trace_launch(p, d_vertices, n_sample, d_out, cuda_stream, 0);
+}
+
+int no_trace_eval_packed(const no_trace_plan* p, int format, const double* d_packed, long long n_sample, double* d_out,
+                         void* cuda_stream) {
+  if (format != NO_PACK_CHARGE) return NO_ERR_INVALID;
+  return trace_launch(p, d_packed, n_sample, d_out, cuda_stream, 1);
+}
+
+namespace {
+int trace_launch(const no_trace_plan* p, const double* d_vertices, long long n_sample, double* d_out, void* cuda_stream, int packed) {
   if (!p || n_sample < 0) return NO_ERR_INVALID;
   if (n_sample == 0) return NO_OK;
   if (!d_vertices || !d_out) return NO_ERR_INVALID;
@@ -394,11 +444,12 @@ int no_trace_eval(const no_trace_plan* p, const double* d_vertices, long long n_
   const size_t smem = trace_plan_bytes(p->plan.n_vertex) + (size_t)warps * trace_warp_bytes(p->plan.n_vertex, p->stages, p->plan.n_slice_iter == 1 ? 1 : 2);
   trace_kernel<<<(unsigned)blocks, warps * 32, smem, static_cast<cudaStream_t>(cuda_stream)>>>(
       p->d_plan, reinterpret_cast<const double2*>(d_vertices), n_sample, reinterpret_cast<double2*>(d_out), p->stages,
-      p->path);
+      p->path, packed);
   const cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return trace_cuda_fail(e, "trace_kernel launch");
   return NO_OK;
 }
+}  // namespace
 
 int no_trace_info(const no_trace_plan* p, long long* cmacs, int* max_open, int* n_sliced, long long* n_iso, int* order,
                   long long* tensor_products) {

@@ -72,3 +72,12 @@ def vertex_matrices(n_sample: int, n_vertex: int, seed: int = 0, stream: int = 0
     if not dense:
         V = V * charge_conserving_mask()[None, None]
     return np.ascontiguousarray(V)
+
+
+def pack_charge(V: np.ndarray) -> np.ndarray:
+    """[..., 16, 16] -> [..., 96]: the NO_PACK_CHARGE layout of include/no.h (an index map, no arithmetic):
+    entry 6 sp + nb, sp = 4 (2 s1' + s2') + (2 s1 + s2), nb over (pp,pp) (pn,pn) (np,np) (nn,nn) (pn,np) (np,pn)."""
+    blocks = ((0, 0), (1, 1), (2, 2), (3, 3), (1, 2), (2, 1))
+    rows = np.array([4 * (sp >> 2) + to for sp in range(16) for to, _ in blocks])
+    cols = np.array([4 * (sp & 3) + ti for sp in range(16) for _, ti in blocks])
+    return np.ascontiguousarray(np.asarray(V)[..., rows, cols])

@@ -104,6 +104,30 @@ def test_ragged_batches_persistent_warps_and_reproducibility(n_sample):
     tr.close()
 
 
+@pytest.mark.parametrize("name,topo", [("ring5", TW.ring(5)), ("ladder4", TW.ladder(4)), ("ladder2", TW.ladder(2)),
+                                       ("complete5", complete5()), ("random4_1", TW.random_closed(4, 1))])
+@pytest.mark.parametrize("charge_plan", [False, True])
+def test_packed_vertex_input_gives_the_same_trace(name, topo, charge_plan):
+    """no_trace_eval_packed reads the 96-entry form no_eval_packed writes; several samples per warp so
+    that the re-zeroing of the aliased slot between samples is exercised; the packing itself is checked against the
+    oracle's definition of the format"""
+    n = len(topo)
+    n_sample = 3000
+    V = TW.vertex_matrices(n_sample, n, seed=8, stream=n)
+    P = TW.pack_charge(V)
+    assert np.array_equal(P.reshape(-1, 96), O.pack(V.reshape(-1, 16, 16), O.PACK_CHARGE))
+    tr = SpinIsospinTrace(topo, charge_conserving=charge_plan)
+    full = tr(torch.from_numpy(V).cuda())
+    packed = tr.from_packed(torch.from_numpy(P).cuda())
+    torch.cuda.synchronize()
+    assert torch.equal(full, packed)
+    idx = np.arange(0, n_sample, 97)
+    check(packed.cpu().numpy()[idx], T.trace_bruteforce(topo, V[idx]), f"{name} packed input")
+    lib = binding.load()
+    assert lib.no_trace_eval_packed(tr._p, binding.NO_PACK_ISOSPIN, None, 0, None, None) == binding.NO_ERR_INVALID
+    tr.close()
+
+
 def test_trace_abi_argument_checks():
     lib = binding.load()
     topo = TW.ladder(3)
@@ -146,6 +170,10 @@ def test_normal_ordering_feeds_the_trace_on_the_device():
     want = T.trace_bruteforce(topo, O.normal_order(cfg, **run.params()).reshape(n_sample, n, 16, 16))
     err = np.abs(got - want) / np.maximum(np.abs(want), 1e-3 * np.sqrt(np.mean(np.abs(want) ** 2)))
     assert err.max() < 1e-9, err.max()       # n factors, each within 1e-10 of the oracle's matrix
+    # the packed hand-over: no_eval_packed -> no_trace_eval_packed, same bits
+    Pk = no.packed(torch.from_numpy(cfg).cuda(), binding.NO_PACK_CHARGE)
+    got_p = tr.from_packed(Pk.reshape(n_sample, n, 96)).cpu().numpy()
+    assert np.array_equal(got_p, got)
     no.close(); tr.close()
 
 
