@@ -286,6 +286,21 @@ def small_batch_rates(dw, dev):
     return {"back_to_back_one_stream_evals_per_s": serial, "graph_4_streams_evals_per_s": graph, "launches": reps}
 
 
+def build_once(world: int, local: int):
+    """compile libno3n.so if it is stale: local rank 0 alone (the other ranks of the node wait), so that N ranks never
+    run nvcc on the same output file"""
+    import torch.distributed as dist
+
+    from paper_2603_24532_b200 import binding, build
+    if world > 1:
+        if local == 0:
+            build.build()
+        dist.barrier()
+    else:
+        build.build()
+    binding.load()
+
+
 def run_b200(args, workload):
     import torch
     import torch.distributed as dist
@@ -300,8 +315,7 @@ def run_b200(args, workload):
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    build.build()
-    binding.load()
+    build_once(world, local)
     dev = torch.device("cuda", local)
     stream = torch.cuda.current_stream(dev)
 
@@ -507,8 +521,7 @@ def run_hf(args):
     torch.cuda.set_device(local)
     if world > 1:
         torch.distributed.init_process_group("nccl", device_id=torch.device("cuda", local))
-    build.build()
-    binding.load()
+    build_once(world, local)
     dev = torch.device("cuda", local)
     stream = torch.cuda.current_stream(dev)
     h = binding.no_init(device=local, **HF_PARAMS)
@@ -638,8 +651,7 @@ def run_trace(args):
     torch.cuda.set_device(local)
     if world > 1:
         torch.distributed.init_process_group("nccl", device_id=torch.device("cuda", local))
-    build.build()
-    binding.load()
+    build_once(world, local)
     dev = torch.device("cuda", local)
     stream = torch.cuda.current_stream(dev)
     # the vertices are charge conserving (as no_eval output is): the plan skips the structurally zero blocks
