@@ -63,7 +63,7 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="cfg5", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "c4", "paper", "hf", "trace5"])
+    ap.add_argument("--workload", default="cfg5", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "c4", "paper", "hf", "trace5", "trace6"])
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg")
@@ -597,7 +597,9 @@ def run_hf(args):
 # the spin-isospin trace (no_trace_eval) as a workload of its own
 # --------------------------------------------------------------------------------------------
 TRACE_BENCH = dict(n_vertex=5, n_sample=1 << 18, seed=7)      # fifth-order ring, 5.4 GB of vertex matrices (> L2)
-TRACE_METRIC = "spin-isospin trace samples/s (fifth-order ring diagram, FP64 complex) on 1 B200"
+TRACE_BENCHES = {"trace5": TRACE_BENCH,
+                 "trace6": dict(n_vertex=6, n_sample=1 << 17, seed=7)}   # sixth order (4^12 labels per sample), 3.2 GB
+TRACE_METRIC = "spin-isospin trace samples/s (ring diagram, FP64 complex) on 1 B200"
 
 
 def hbm_peak_gbs():
@@ -612,7 +614,8 @@ def hbm_peak_gbs():
 def run_trace(args):
     """One step = one no_trace_eval launch over 2^18 samples of 5 vertex matrices (20 KiB per sample, read once)."""
     from paper_2603_24532_b200 import trace_workloads as TW
-    n, n_sample = TRACE_BENCH["n_vertex"], TRACE_BENCH["n_sample"]
+    spec = TRACE_BENCHES[args.workload]
+    n, n_sample = spec["n_vertex"], spec["n_sample"]
     topo = TW.ring(n)
     labels = 4 ** (2 * n)
     if args.impl == "reference":
@@ -622,19 +625,19 @@ def run_trace(args):
             os.environ["OMP_NUM_THREADS"] = str(os.cpu_count() or 1)
         from oracle import trace as T
         T.build()
-        m = args.cpu_sample or 256
-        V = TW.vertex_matrices(m, n, seed=TRACE_BENCH["seed"])
+        m = args.cpu_sample or (256 if n <= 5 else 32)
+        V = TW.vertex_matrices(m, n, seed=spec["seed"])
         for _ in range(args.warmup):
             T.trace_bruteforce(topo, V[:16])
         t0 = time.perf_counter()
         for _ in range(args.steps):
             T.trace_bruteforce(topo, V)
         dt = (time.perf_counter() - t0) / args.steps
-        sample = f"first {m} samples of the workload, brute-force sum over all 4^10 label configurations each"
+        sample = f"first {m} samples of the workload, brute-force sum over all 4^{2 * n} label configurations each"
         print(json.dumps({"impl": "reference", "metric": TRACE_METRIC, "value": m / dt, "unit": "samples/s",
                           "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3,
                           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                          "config": {"workload": "trace5", "sample": sample},
+                          "config": {"workload": args.workload, "sample": sample},
                           "cpu_baseline": {"value": m / dt, "unit": "samples/s", "cores": os.cpu_count(), "kind": "oracle (brute force)",
                                            "sample": sample},
                           "e2e": {"value": m / dt, "unit": "samples/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -657,7 +660,7 @@ def run_trace(args):
     # the vertices are charge conserving (as no_eval output is): the plan skips the structurally zero blocks
     plan = binding.no_trace_init(topo, local, binding.NO_TRACE_CHARGE_CONSERVING)
     info = binding.no_trace_info(plan, n)
-    V = TW.vertex_matrices(n_sample, n, seed=TRACE_BENCH["seed"])
+    V = TW.vertex_matrices(n_sample, n, seed=spec["seed"])
     d_V = torch.from_numpy(V).to(dev)
     d_out = torch.empty((n_sample,), dtype=torch.complex128, device=dev)
     flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)
@@ -710,8 +713,9 @@ def run_trace(args):
         a.record(stream)
         binding.no_trace_eval_packed(plan, binding.NO_PACK_CHARGE, d_P.data_ptr(), n_sample, d_out_p.data_ptr(), stream.cuda_stream)
         b.record(stream)
+    binding.no_trace_eval(plan, d_V.data_ptr(), n_sample, d_out.data_ptr(), stream.cuda_stream)
     torch.cuda.synchronize(dev)
-    assert torch.equal(d_out_p, d_out)
+    assert torch.equal(d_out_p, d_out)                   # same plan, same bits from either input form
     packed_ms = sum(a.elapsed_time(b) for a, b in ep) / len(ep)
     packed_in = {"samples_per_s": n_sample / (packed_ms * 1e-3), "avg_launch_ms": packed_ms,
                  "bytes_per_sample": n * 1536 + 16,
@@ -771,11 +775,11 @@ def run_trace(args):
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         from oracle import trace as T
-        mcpu = args.cpu_sample or 1024
+        mcpu = args.cpu_sample or (1024 if n <= 5 else 64)
         t0 = time.perf_counter()
         T.trace_bruteforce(topo, V[:mcpu])
         dt = time.perf_counter() - t0
-        cpu = {"value": mcpu / dt, "unit": "samples/s", "cores": os.cpu_count(), "kind": "oracle (brute force over 4^10 label configurations, long double)",
+        cpu = {"value": mcpu / dt, "unit": "samples/s", "cores": os.cpu_count(), "kind": f"oracle (brute force over 4^{2 * n} label configurations, long double)",
                "sample": f"first {mcpu} samples of the workload ({dt:.1f} s)"}
     binding.no_trace_free(plan)
     if world > 1:
@@ -786,14 +790,14 @@ def run_trace(args):
         "metric": TRACE_METRIC, "value": value, "unit": "samples/s", "n_gpus": world, "steps": steps, "warmup": warmup,
         "ms_per_step": t_dev / steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "trace5", "description": "spin-isospin trace of a fifth-order ring diagram (5 vertices, 10 lines, "
-                   "4^10 label configurations per sample), 2^18 samples of seeded charge-conserving complex 16x16 vertex matrices",
+        "config": {"workload": args.workload, "description": f"spin-isospin trace of an order-{n} ring diagram ({n} vertices, {2 * n} lines, "
+                   f"4^{2 * n} label configurations per sample), {n_sample} samples of seeded charge-conserving complex 16x16 vertex matrices",
                    "n_sample": n_sample, "label_configurations_per_s": value * labels, "plan": info,
-                   "l2": "256 MiB buffer rewritten between timed steps (L2 flush); the input (5.4 GB) exceeds L2",
+                   "l2": "256 MiB buffer rewritten between timed steps (L2 flush); the input (3-5 GB) exceeds L2",
                    "parallelism": "replicas only: every rank traces the whole batch"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": steps,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get("trace5"), "traffic_source": NCU_DRAM_SOURCE.get("trace5"),
+                     "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(args.workload), "traffic_source": NCU_DRAM_SOURCE.get(args.workload),
                      "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_step,
                      "bytes_per_sample": n * 4096 + 16, "kernel": "trace_kernel", "avg_launch_ms": sum(step_ms) / steps,
                      "fp64_tflops": flops_step * steps / (sum(step_ms) * 1e-3) / 1e12,
@@ -809,7 +813,7 @@ def main():
     if args.workload == "hf":
         run_hf(args)
         return
-    if args.workload == "trace5":
+    if args.workload in TRACE_BENCHES:
         run_trace(args)
         return
     from paper_2603_24532_b200 import workloads
