@@ -223,7 +223,7 @@ inline int build_trace_plan(int n, const int* topo, TracePlan& plan, bool charge
   plan.dmma_products = 0;
   // isospin-major enumeration of a pair of line labels (16 x 16 x 16 steps): digit j of enumeration e
   static const int iso_t[4][2] = {{0, 1}, {1, 0}, {0, 0}, {1, 1}};
-  auto big_digit = [](int e, int j) { return 2 * (((e & 3) >> j) & 1) + iso_t[e >> 2][j]; };
+  auto big_digit = [](int e, int j) { return 2 * (((e & 3) >> j) & 1) + iso_t[(e >> 2) & 3][j]; };   // e < 16 is meaningful
 
   // tables of every step
   int open[kTrMaxLines], open_sigma[kTrMaxLines], n_open = 0;

@@ -231,3 +231,19 @@ def test_angular_rule_with_non_unit_directions_is_refused():
     bad[0, :3] = 0.0
     with pytest.raises(ValueError):
         emu.emu_eval_angular(cfg, bad, **kw)
+
+
+def test_host_logic_and_kernel_arithmetic_run_clean_under_sanitizers(tmp_path):
+    """no_host.h + no_core.h (the product's planner and the kernel's arithmetic, compiled for the host) under
+    -fsanitize=address,undefined: every kernel variant, both matter geometries, grid and direction list, maximum orders"""
+    import os
+    import subprocess
+    here = os.path.dirname(__file__)
+    exe = str(tmp_path / "host_emu_sanitized")
+    subprocess.run(["g++", "-O1", "-g", "-std=c++17", "-ffp-contract=off", "-fsanitize=address,undefined",
+                    "-fno-sanitize-recover=all", "-fno-omit-frame-pointer", "-o", exe,
+                    os.path.join(here, "host_emu_sanitize_main.cpp")], check=True)
+    r = subprocess.run([exe], capture_output=True, text=True, env=dict(os.environ, ASAN_OPTIONS="detect_leaks=1"))
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert "runtime error" not in r.stderr and "AddressSanitizer" not in r.stderr
+    assert "runs ok" in r.stdout

@@ -82,3 +82,19 @@ def test_malformed_topologies_are_refused():
     assert E.plan([[0, 1, 0, 0]]) is None
     assert E.plan([[0, 1, 2, 3], [2, 3, 0, 4]]) is None
     assert E.plan(np.zeros((7, 4), dtype=np.int32)) is None
+
+
+def test_planner_runs_clean_under_address_and_undefined_behaviour_sanitizers(tmp_path):
+    """the product's host planner (no_trace_host.h) as a standalone program under -fsanitize=address,undefined: chains
+    of order 1-6 and 300 pseudo-random closed topologies, with and without the charge flag; every tabulated offset
+    must stay inside the kernel's shared-memory buffers"""
+    import os
+    import subprocess
+    here = os.path.dirname(__file__)
+    exe = str(tmp_path / "trace_plan_sanitized")
+    subprocess.run(["g++", "-O1", "-g", "-std=c++17", "-fsanitize=address,undefined", "-fno-sanitize-recover=all",
+                    "-fno-omit-frame-pointer", "-o", exe, os.path.join(here, "trace_plan_sanitize_main.cpp")], check=True)
+    r = subprocess.run([exe], capture_output=True, text=True, env=dict(os.environ, ASAN_OPTIONS="detect_leaks=1"))
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert "runtime error" not in r.stderr and "AddressSanitizer" not in r.stderr
+    assert "plans ok" in r.stdout

@@ -186,3 +186,18 @@ def test_charge_violating_vertex_gives_zero_and_isospin_subset_counts():
                 term = term * Vd[0, v, pair(x[r[0]], x[r[1]]), pair(x[r[2]], x[r[3]])]
             tot += term
     assert full == pytest.approx(tot, rel=1e-12)
+
+
+def test_trace_oracle_runs_clean_under_address_and_undefined_behaviour_sanitizers(tmp_path):
+    """SURVEY.md section 5 for the second oracle: oracle/trace_oracle.c (included verbatim by
+    tests/trace_oracle_sanitize_main.c) under -fsanitize=address,undefined, no report, every check held."""
+    import os
+    import subprocess
+    here = os.path.dirname(__file__)
+    exe = str(tmp_path / "trace_oracle_sanitized")
+    subprocess.run(["gcc", "-O1", "-g", "-std=c99", "-fsanitize=address,undefined", "-fno-sanitize-recover=all",
+                    "-fno-omit-frame-pointer", "-o", exe, os.path.join(here, "trace_oracle_sanitize_main.c"), "-lm"], check=True)
+    r = subprocess.run([exe], capture_output=True, text=True, env=dict(os.environ, ASAN_OPTIONS="detect_leaks=1"))
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert "runtime error" not in r.stderr and "AddressSanitizer" not in r.stderr and "LeakSanitizer" not in r.stderr
+    assert "trace oracle sanitized: ok" in r.stdout
