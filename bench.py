@@ -33,8 +33,8 @@ UNIT = "evals/s"
 FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum per launch (mean over the launches of one step) of the workload's
 # kernel, from the ncu capture named beside it (profiles/); None = no capture of that workload exists
-NCU_DRAM_BYTES_PER_LAUNCH = {"cfg5": 1675959125, "trace5": 5376942696}
-NCU_DRAM_SOURCE = {"cfg5": "profiles/r02a.md (r02a_cfg5_dram.csv: all six launches of one cfg5 step, 10.06 GB of DRAM "
+NCU_DRAM_BYTES_PER_LAUNCH = {"cfg5": 1655888896, "trace5": 5376942696}
+NCU_DRAM_SOURCE = {"cfg5": "profiles/r02a.md (r02a_cfg5_dram.csv: all six launches of one cfg5 step, 9.94 GB of DRAM "
                            "traffic against 9.83 GB algorithmic: 4.4 GB of output per 2^20-configuration launch cannot stay in the 126 MB L2)",
                    "trace5": "profiles/r02b.md (ncu --set full of one launch: 5.3688 GB read + 0.0082 GB written against 5.3729 GB "
                              "algorithmic)"}
