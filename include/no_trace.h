@@ -64,13 +64,16 @@ int no_trace_init(no_trace_plan **plan, int n_vertex, const int *topo, int flags
 int no_trace_eval(const no_trace_plan *plan, const double *d_vertices, long long n_sample, double *d_out,
                   void *cuda_stream);
 
-/* no_trace_eval reading the vertex matrices in the packed form NO_PACK_CHARGE of include/no.h (what no_eval_packed
- * writes: the 96 charge-conserving entries, 1536 bytes per vertex instead of 4096): the kernel scatters
- * them into zeroed shared-memory matrices, so 7.7 instead of 20.5 KB per fifth-order sample cross HBM.
- *   format   : NO_PACK_CHARGE (NO_ERR_INVALID otherwise)
- *   d_packed : DEVICE, const, [n_sample][n_vertex][96][2] doubles, 16-byte aligned, dense, caller-owned
- * Otherwise as no_trace_eval; works with plans made with or without NO_TRACE_CHARGE_CONSERVING (the packed form cannot
- * express a charge-violating entry) and gives the same bits as no_trace_eval on the unpacked matrices. */
+/* no_trace_eval reading the vertex matrices in a packed form of include/no.h (what no_eval_packed writes):
+ *   NO_PACK_CHARGE  : the 96 charge-conserving entries, 1536 bytes per vertex instead of 4096; the kernel scatters
+ *                     them into zeroed shared-memory matrices (7.7 instead of 20.5 KB per fifth-order sample cross HBM);
+ *                     d_packed is [n_sample][n_vertex][96][2] doubles
+ *   NO_PACK_ISOSPIN : isospin-symmetric matter, 32 entries = 512 bytes per vertex; the kernel rebuilds the other
+ *                     charge-conserving entries as no_unpack does ((np,np) = (pn,pn), (np,pn) = (pn,np),
+ *                     (pp,pp) = (nn,nn) = (pn,pn) + (pn,np)); d_packed is [n_sample][n_vertex][32][2] doubles
+ * Any other format: NO_ERR_INVALID.  d_packed: DEVICE, const, 16-byte aligned, dense, caller-owned.
+ * Otherwise as no_trace_eval; works with plans made with or without NO_TRACE_CHARGE_CONSERVING (a packed form cannot
+ * express a charge-violating entry) and gives the same bits as no_trace_eval on the matrices no_unpack rebuilds. */
 int no_trace_eval_packed(const no_trace_plan *plan, int format, const double *d_packed, long long n_sample, double *d_out,
                          void *cuda_stream);
 

@@ -135,15 +135,16 @@ class SpinIsospinTrace:
         s = stream if stream is not None else torch.cuda.current_stream(vertices.device)
         binding.no_trace_eval(self._p, vertices.data_ptr(), n, out.data_ptr(), s.cuda_stream)
 
-    def from_packed(self, packed: torch.Tensor) -> torch.Tensor:
-        """no_trace_eval_packed: packed complex128 CUDA tensor [n_sample, n_vertex, 96] (NormalOrdering.packed(cfg, 1)
-        reshaped) -> complex128 [n_sample]."""
+    def from_packed(self, packed: torch.Tensor, fmt: int = binding.NO_PACK_CHARGE) -> torch.Tensor:
+        """no_trace_eval_packed: packed complex128 CUDA tensor [n_sample, n_vertex, 96] (fmt 1) or [n_sample, n_vertex, 32]
+        (fmt 2, isospin-symmetric matter), i.e. NormalOrdering.packed(cfg, fmt) reshaped -> complex128 [n_sample]."""
         assert packed.is_cuda and packed.dtype == torch.complex128
         packed = packed.contiguous()
-        n = packed.numel() // (self.n_vertex * 96)
-        assert packed.numel() == n * self.n_vertex * 96
+        per = 96 if fmt == binding.NO_PACK_CHARGE else 32
+        n = packed.numel() // (self.n_vertex * per)
+        assert packed.numel() == n * self.n_vertex * per
         out = torch.empty((n,), dtype=torch.complex128, device=packed.device)
-        binding.no_trace_eval_packed(self._p, binding.NO_PACK_CHARGE, packed.data_ptr(), n, out.data_ptr(),
+        binding.no_trace_eval_packed(self._p, fmt, packed.data_ptr(), n, out.data_ptr(),
                                      torch.cuda.current_stream(packed.device).cuda_stream)
         return out
 

@@ -91,18 +91,40 @@ __device__ __forceinline__ void request_vertex_packed(double2* dst, const double
   }
 }
 
-// all n vertex matrices of the sample at src as ONE cp.async group
+// NO_PACK_ISOSPIN (isospin-symmetric matter): 32 entries per vertex, [16 spin elements][(pn,pn), (pn,np)].  Lane 2 sp + h
+// copies its entry to the two places it stands for, (pn,pn) and (np,np) or (pn,np) and (np,pn); the pp and nn entries
+// are their sum and are filled in after the copies have landed (isospin_fixup).
+__device__ __forceinline__ int iso_pos(int sp, int to, int ti) { return (4 * (sp >> 2) + to) * kTrRowW + 4 * (sp & 3) + ti; }
+__device__ __forceinline__ void request_vertex_iso(double2* dst, const double2* src, int v, int lane) {
+  const int sp = lane >> 1, h = lane & 1;
+  const double2* g = src + v * 32 + lane;
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;"
+               ::"r"(smem_u32(dst + v * kTrMatW + iso_pos(sp, 1, h ? 2 : 1))), "l"(g) : "memory");
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;"
+               ::"r"(smem_u32(dst + v * kTrMatW + iso_pos(sp, 2, h ? 1 : 2))), "l"(g) : "memory");
+}
+__device__ __forceinline__ void isospin_fixup(double2* slots, int n, int lane) {
+  const int sp = lane >> 1, h = lane & 1;
+  for (int v = 0; v < n; ++v) {
+    double2* m = slots + v * kTrMatW;
+    const double2 d = m[iso_pos(sp, 1, 1)], x = m[iso_pos(sp, 1, 2)];
+    m[h ? iso_pos(sp, 3, 3) : iso_pos(sp, 0, 0)] = make_double2(d.x + x.x, d.y + x.y);   // T = 1: pp = nn = (pn,pn) + (pn,np)
+  }
+}
+
+// all n vertex matrices of the sample at src as ONE cp.async group (packed: 0 full matrices, 1 NO_PACK_CHARGE, 2 NO_PACK_ISOSPIN)
 __device__ __forceinline__ void request_sample(double2* dst, const double2* src, int n, bool valid, int lane, int packed) {
   if (valid)
     for (int v = 0; v < n; ++v) {
-      if (packed) request_vertex_packed(dst, src, v, lane);
+      if (packed == 2) request_vertex_iso(dst, src, v, lane);
+      else if (packed == 1) request_vertex_packed(dst, src, v, lane);
       else request_vertex(dst, src, v, lane);
     }
   asm volatile("cp.async.commit_group;" ::: "memory");
 }
 
 // path: 0 = vector FP64 (DFMA) register tiles, 1 = FP64 tensor cores (DMMA m8n8k4) for the 16 x 16 x 16 steps
-__global__ void __launch_bounds__(512, 1)
+__global__ void __launch_bounds__(384, 1)
 trace_kernel(const DevTracePlan* __restrict__ plan_g, const double2* __restrict__ V, long long n_sample,
              double2* __restrict__ out, int stages, int path, int packed) {
   extern __shared__ __align__(128) unsigned char tsm[];
@@ -122,7 +144,7 @@ trace_kernel(const DevTracePlan* __restrict__ plan_g, const double2* __restrict_
   double2* vbuf = reinterpret_cast<double2*>(wb + 16);                   // [stages][n][16][17]
   double2* Rb = vbuf + (size_t)stages * n * kTrMatW;                      // [r_bufs][16][17]
   if (lane == 0) *one = make_double2(1.0, 0.0);
-  const int vs = packed ? 96 : 256;                                       // complex numbers per vertex in HBM
+  const int vs = packed == 2 ? 32 : (packed ? 96 : 256);                  // complex numbers per vertex in HBM
   if (packed)                                                             // the entries the packed form leaves out stay zero
     for (int i = lane; i < stages * n * kTrMatW; i += 32) vbuf[i] = make_double2(0.0, 0.0);
   __syncthreads();
@@ -145,6 +167,10 @@ trace_kernel(const DevTracePlan* __restrict__ plan_g, const double2* __restrict_
       asm volatile("cp.async.wait_group 0;" ::: "memory");
     }
     __syncwarp();
+    if (packed == 2) {
+      isospin_fixup(vbuf + (size_t)stage * n * kTrMatW, n, lane);
+      __syncwarp();
+    }
     const double2* W = vbuf + (size_t)stage * n * kTrMatW;
 
     double2 total = make_double2(0.0, 0.0);
@@ -391,7 +417,7 @@ int no_trace_init(no_trace_plan** out, int n_vertex, const int* topo, int flags,
   const size_t avail = (size_t)smem_optin - trace_plan_bytes(n_vertex) - 128;
   const int r_bufs = p->plan.n_slice_iter == 1 ? 1 : 2;
   int warps = (int)(avail / trace_warp_bytes(n_vertex, p->stages, r_bufs));
-  if (warps > 16) warps = 16;
+  if (warps > 12) warps = 12;      // __launch_bounds__(384): up to 170 registers per thread, no spills
   if (const char* e = getenv("NO3N_TRACE_WARPS")) { const int v = atoi(e); if (v >= 1 && v < warps) warps = v; }
   if (warps < 1) { delete p; return NO_ERR_INVALID; }
   p->warps = warps;
@@ -420,8 +446,8 @@ int no_trace_eval(const no_trace_plan* p, const double* d_vertices, long long n_
 
 int no_trace_eval_packed(const no_trace_plan* p, int format, const double* d_packed, long long n_sample, double* d_out,
                          void* cuda_stream) {
-  if (format != NO_PACK_CHARGE) return NO_ERR_INVALID;
-  return trace_launch(p, d_packed, n_sample, d_out, cuda_stream, 1);
+  if (format != NO_PACK_CHARGE && format != NO_PACK_ISOSPIN) return NO_ERR_INVALID;
+  return trace_launch(p, d_packed, n_sample, d_out, cuda_stream, format == NO_PACK_CHARGE ? 1 : 2);
 }
 
 namespace {

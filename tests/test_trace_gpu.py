@@ -123,8 +123,17 @@ def test_packed_vertex_input_gives_the_same_trace(name, topo, charge_plan):
     assert torch.equal(full, packed)
     idx = np.arange(0, n_sample, 97)
     check(packed.cpu().numpy()[idx], T.trace_bruteforce(topo, V[idx]), f"{name} packed input")
+    # isospin form: vertices of the form A + B tau_1.tau_2 (what SNM normal ordering gives); the kernel rebuilds the
+    # matrix as the oracle's unpack does
+    Pi = np.ascontiguousarray(P.reshape(n_sample, n, 16, 6)[..., [1, 4]].reshape(n_sample, n, 32))
+    Vi = O.unpack(Pi.reshape(-1, 32), O.PACK_ISOSPIN).reshape(n_sample, n, 16, 16)
+    from_iso = tr.from_packed(torch.from_numpy(Pi).cuda(), binding.NO_PACK_ISOSPIN)
+    ref_iso = tr(torch.from_numpy(np.ascontiguousarray(Vi)).cuda())
+    torch.cuda.synchronize()
+    assert torch.equal(from_iso, ref_iso)
+    check(from_iso.cpu().numpy()[idx], T.trace_bruteforce(topo, Vi[idx]), f"{name} isospin-packed input")
     lib = binding.load()
-    assert lib.no_trace_eval_packed(tr._p, binding.NO_PACK_ISOSPIN, None, 0, None, None) == binding.NO_ERR_INVALID
+    assert lib.no_trace_eval_packed(tr._p, 3, None, 0, None, None) == binding.NO_ERR_INVALID
     tr.close()
 
 
@@ -174,6 +183,11 @@ def test_normal_ordering_feeds_the_trace_on_the_device():
     Pk = no.packed(torch.from_numpy(cfg).cuda(), binding.NO_PACK_CHARGE)
     got_p = tr.from_packed(Pk.reshape(n_sample, n, 96)).cpu().numpy()
     assert np.array_equal(got_p, got)
+    # cfg3 is symmetric matter: the 512-byte isospin form carries the same information (pp = nn = pn,pn + pn,np to rounding)
+    Pi = no.packed(torch.from_numpy(cfg).cuda(), binding.NO_PACK_ISOSPIN)
+    got_i = tr.from_packed(Pi.reshape(n_sample, n, 32), binding.NO_PACK_ISOSPIN).cpu().numpy()
+    err_i = np.abs(got_i - want) / np.maximum(np.abs(want), 1e-3 * np.sqrt(np.mean(np.abs(want) ** 2)))
+    assert err_i.max() < 1e-9, err_i.max()
     no.close(); tr.close()
 
 
