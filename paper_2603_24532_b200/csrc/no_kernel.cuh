@@ -177,17 +177,24 @@ no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg,
     __syncwarp();
 
     // ---- a3: reduce the moments over the 32 lanes (fixed order) ----
-    for (int row = lane; row < L::kRows; row += kLanes) {
-      // four independent chains of eight (fixed order: bit reproducible), then a fixed tree
-      double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+    // a lane adds one PAIR of adjacent rows over the 32 lanes: 16-byte loads, four independent chains of eight
+    // (fixed order: bit reproducible), then a fixed tree.  Lane l starts at source lane 2 l: with an odd number of
+    // 16-byte units per lane (29 or 41) the eight lanes of a quarter warp then hit eight different bank groups.
+    {
+      const Pair* acc2 = reinterpret_cast<const Pair*>(acc);
+      Pair* mom2 = reinterpret_cast<Pair*>(mom);
+      constexpr int kUnits = L::kStride / 2;
+      for (int pr = lane; pr < kUnits; pr += kLanes) {
+        Pair s0 = {0.0, 0.0}, s1 = {0.0, 0.0}, s2 = {0.0, 0.0}, s3 = {0.0, 0.0};
 #pragma unroll
-      for (int t = 0; t < 8; ++t) {
-        s0 += acc[((lane + t) & 31) * L::kStride + row];
-        s1 += acc[((lane + t + 8) & 31) * L::kStride + row];
-        s2 += acc[((lane + t + 16) & 31) * L::kStride + row];
-        s3 += acc[((lane + t + 24) & 31) * L::kStride + row];
+        for (int t = 0; t < 8; ++t) {
+          const Pair a0 = acc2[((2 * lane + t) & 31) * kUnits + pr], a1 = acc2[((2 * lane + t + 8) & 31) * kUnits + pr];
+          const Pair a2 = acc2[((2 * lane + t + 16) & 31) * kUnits + pr], a3 = acc2[((2 * lane + t + 24) & 31) * kUnits + pr];
+          s0.x += a0.x; s0.y += a0.y; s1.x += a1.x; s1.y += a1.y;
+          s2.x += a2.x; s2.y += a2.y; s3.x += a3.x; s3.y += a3.y;
+        }
+        mom2[pr] = Pair{(s0.x + s1.x) + (s2.x + s3.x), (s0.y + s1.y) + (s2.y + s3.y)};
       }
-      mom[row] = (s0 + s1) + (s2 + s3);
     }
     __syncwarp();
 

@@ -34,7 +34,7 @@ static void emu_cfg(const HostPlan& plan, const double* cfg, double* out /*[512]
   const DevParams& P = plan.dp;
   CfgConst c;
   cfg_setup<NREG>(P, cfg, c);
-  std::vector<double> acc(L::kStride * kLanes + 2), mom(L::kRows), rec(kRecDoubles), coef(32 * 6, 0.0);
+  std::vector<double> acc(L::kStride * kLanes + 2), mom(L::kStride), rec(kRecDoubles), coef(32 * 6, 0.0);
   double* acc16 = acc.data() + ((reinterpret_cast<uintptr_t>(acc.data()) & 15) ? 1 : 0);   // 16-byte aligned rows
   std::vector<double> ttab(kRadT * P.n_r_pad);
   const double* e2tab = plan.tab.data();
@@ -68,12 +68,14 @@ static void emu_cfg(const HostPlan& plan, const double* cfg, double* out /*[512]
       }
     }
     for (int lane = 0; lane < kLanes; ++lane)
-      for (int row = lane; row < L::kRows; row += kLanes) {
-        double s4[4] = {0.0, 0.0, 0.0, 0.0};
-        for (int t = 0; t < 8; ++t)
-          for (int q = 0; q < 4; ++q) s4[q] += acc16[((lane + t + 8 * q) & 31) * L::kStride + row];
-        mom[row] = (s4[0] + s4[1]) + (s4[2] + s4[3]);
-      }
+      for (int pr = lane; pr < L::kStride / 2; pr += kLanes)       // a lane adds one pair of adjacent rows (see the kernel)
+        for (int h = 0; h < 2; ++h) {
+          const int row = 2 * pr + h;
+          double s4[4] = {0.0, 0.0, 0.0, 0.0};
+          for (int t = 0; t < 8; ++t)
+            for (int q = 0; q < 4; ++q) s4[q] += acc16[((2 * lane + t + 8 * q) & 31) * L::kStride + row];
+          mom[row] = (s4[0] + s4[1]) + (s4[2] + s4[3]);
+        }
     for (int lane = 0; lane < 6; ++lane) phase1_job<C4>(P, c, mom.data(), lane, rec.data());
     for (int lane = 0; lane < kLanes; ++lane)
       phase2_lane(rec.data(), lane, P.nsp[pass], P.esum[pass], NREG >= 0 ? exp(-c.E0) : 1.0, &coef[lane * 6]);

@@ -60,7 +60,8 @@ TOPOS = ([(f"ladder{n}", TW.ladder(n)) for n in (1, 2, 3, 4, 5, 6)] + [(f"ring{n
          [("ladder5x", TW.exchange_slots(TW.ladder(5), out_mask=0b01010, in_mask=0b00110)),
           ("ring5x", TW.relabel(TW.exchange_slots(TW.ring(5), out_mask=0b10001), 3)),
           ("complete5", complete5())] +
-         [(f"random{n}_{s}", TW.random_closed(n, s)) for n in (2, 3, 4, 5) for s in range(4)])
+         [(f"random{n}_{s}", TW.random_closed(n, s)) for n in (2, 3, 4, 5) for s in range(4)] +
+         [(f"random6_{s}", TW.random_closed(6, s)) for s in range(2)])
 
 
 @pytest.mark.parametrize("name,topo", TOPOS)
