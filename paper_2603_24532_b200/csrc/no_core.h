@@ -422,10 +422,13 @@ NO_HD void nodes(const double* rs, int n_reg, const double* e2tab, const DirCons
 struct alignas(16) Pair { double x, y; };
 
 // a: 10 consecutive rows of one lane (16-byte aligned): 1 | u | u u^T
+// FIRST: the rows hold nothing yet (first direction of the lane in this pass): they are written, not updated, which
+// saves the zero fill of the accumulators and one round of loads; fma(a, b, 0) and a * b round alike.
+template <bool FIRST>
 NO_HD void rmw_rank012(double* a, const double* wt, double s0, double s1, double s2) {
   Pair* p = reinterpret_cast<Pair*>(a);
   Pair v[5];
-  for (int k = 0; k < 5; ++k) v[k] = p[k];
+  for (int k = 0; k < 5; ++k) v[k] = FIRST ? Pair{0.0, 0.0} : p[k];
   v[0].x = fma(wt[0], s0, v[0].x); v[0].y = fma(wt[1], s1, v[0].y);
   v[1].x = fma(wt[2], s1, v[1].x); v[1].y = fma(wt[3], s1, v[1].y);
   v[2].x = fma(wt[4], s2, v[2].x); v[2].y = fma(wt[5], s2, v[2].y);
@@ -436,7 +439,7 @@ NO_HD void rmw_rank012(double* a, const double* wt, double s0, double s1, double
 
 // FWD: the rows of legs 2, 3 and of pair 3 are left untouched (the kernel copies them from legs 0, 1 and pair 2
 // after the lane reduction)
-template <bool C4, bool FWD = false>
+template <bool C4, bool FWD = false, bool FIRST = false>
 NO_HD void second_level(const First& f, const DirConst& d, const double* gam, double w, double* acc /* this lane's rows */) {
   const double ux = d.u[0], uy = d.u[1], uz = d.u[2];
   double wt[10];      // w * (1, ux, uy, uz, ux ux, ux uy, ux uz, uy uy, uy uz, uz uz)
@@ -445,19 +448,19 @@ NO_HD void second_level(const First& f, const DirConst& d, const double* gam, do
   NO_FENCE();
   for (int l = 0; l < (FWD ? 2 : 4); ++l) {
     const double S2 = fma(-gam[l], f.S[l][0], fma(-d.bet[l], f.S[l][1], f.R0));   // sum wF r^2 / D_l
-    rmw_rank012(acc + Layout<C4>::kRowLeg + 10 * l, wt, f.S[l][0], f.S[l][1], S2);
+    rmw_rank012<FIRST>(acc + Layout<C4>::kRowLeg + 10 * l, wt, f.S[l][0], f.S[l][1], S2);
   }
   if (C4) {
     for (int t = 0; t < (FWD ? 3 : 4); ++t) {
       const int x = NO_PAIR_X(t), y = FWD ? (NO_PAIR_Y(t) - 2) : NO_PAIR_Y(t);          // FWD: leg y coincides with y - 2
       const double G2 = fma(-gam[x], f.G[t][0], fma(-d.bet[x], f.G[t][1], f.S[y][0]));   // sum wF r^2/(D_x D_y)
-      rmw_rank012(acc + Layout<C4>::kRowPair + 10 * t, wt, f.G[t][0], f.G[t][1], G2);     // Gm0, Gm1, Gm2
+      rmw_rank012<FIRST>(acc + Layout<C4>::kRowPair + 10 * t, wt, f.G[t][0], f.G[t][1], G2);     // Gm0, Gm1, Gm2
     }
   } else {
     Pair* p = reinterpret_cast<Pair*>(acc + Layout<C4>::kRowPair);   // Gm0, Gm1[3] of the four pairs
     constexpr int np = FWD ? 3 : 4;
     Pair v[8];
-    for (int k = 0; k < 2 * np; ++k) v[k] = p[k];
+    for (int k = 0; k < 2 * np; ++k) v[k] = FIRST ? Pair{0.0, 0.0} : p[k];
     for (int t = 0; t < np; ++t) {
       v[2 * t].x = fma(wt[0], f.G[t][0], v[2 * t].x);
       v[2 * t].y = fma(wt[1], f.G[t][1], v[2 * t].y);
@@ -466,7 +469,7 @@ NO_HD void second_level(const First& f, const DirConst& d, const double* gam, do
     }
     for (int k = 0; k < 2 * np; ++k) p[k] = v[k];
   }
-  acc[Layout<C4>::kRowR0] = fma(w, f.R0, acc[Layout<C4>::kRowR0]);
+  acc[Layout<C4>::kRowR0] = FIRST ? w * f.R0 : fma(w, f.R0, acc[Layout<C4>::kRowR0]);
   NO_FENCE();
 }
 

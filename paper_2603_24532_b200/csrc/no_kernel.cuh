@@ -139,16 +139,18 @@ no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg,
     const double* sph = cph + P.n_phi;
     const double* wph = sph + P.n_phi;
     for (int i = lane; i < P.n_r_pad; i += kLanes) radial_entry(*cc, rad[2 * i], ttab + kRadT * i);
-    {
+    // ---- a2 + a3: hot loop over the k3 nodes of this sphere ----
+    const int n_dir = P.n_list > 0 ? P.n_list : P.n_cos * P.n_phi;
+    const int dstep = kLanes * SPLIT, m0 = lane + kLanes * part;
+    // a lane's accumulator rows are WRITTEN by its first direction of the pass (second_level<.., FIRST>) and updated
+    // by the others; only a lane without any direction clears its rows (in FWD launches the rows of the duplicate legs
+    // are never written: the lane reduction adds whatever they hold and the copy after it overwrites the result)
+    if (m0 >= n_dir) {
       Pair* z = reinterpret_cast<Pair*>(acc + lane * L::kStride);
 #pragma unroll
       for (int k = 0; k < L::kStride / 2; ++k) z[k] = Pair{0.0, 0.0};
     }
     __syncwarp();
-
-    // ---- a2 + a3: hot loop over the k3 nodes of this sphere ----
-    const int n_dir = P.n_list > 0 ? P.n_list : P.n_cos * P.n_phi;
-    const int dstep = kLanes * SPLIT, m0 = lane + kLanes * part;
     const int dj = dstep / P.n_phi, dl = dstep - dj * P.n_phi;     // (j, l) advance by dstep directions per trip
     int j = m0 / P.n_phi, l = m0 - j * P.n_phi;
     const double4* dlist = reinterpret_cast<const double4*>(ct);   // list mode: (ux, uy, uz, w), 32-byte aligned
@@ -170,7 +172,8 @@ no3n_kernel(const __grid_constant__ DevParams P, const double* __restrict__ cfg,
       first_zero(f);
       if (flush) radial_loop<NREG, true, FWD>(P, pass, rsp, e2tab, d, tt2, ttab, f);
       else radial_loop<NREG, false, FWD>(P, pass, rsp, e2tab, d, tt2, ttab, f);
-      second_level<C4, FWD>(f, d, cc->gam, w, acc + lane * L::kStride);
+      if (m == m0) second_level<C4, FWD, true>(f, d, cc->gam, w, acc + lane * L::kStride);
+      else second_level<C4, FWD, false>(f, d, cc->gam, w, acc + lane * L::kStride);
       j += dj; l += dl;
       if (l >= P.n_phi) { l -= P.n_phi; ++j; }
     }

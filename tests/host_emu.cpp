@@ -28,6 +28,8 @@ static void trip(const double* rs, int n_reg, const double* e2tab, const DirCons
   else nodes<NREG, kNodesPerTrip, false>(rs, n_reg, e2tab, d, r, wr, T, f);
 }
 
+static int n_dir_of(const DevParams& P) { return P.n_list > 0 ? P.n_list : P.n_cos * P.n_phi; }
+
 template <int NREG, bool C4>
 static void emu_cfg(const HostPlan& plan, const double* cfg, double* out /*[512]*/) {
   using L = Layout<C4>;
@@ -47,7 +49,11 @@ static void emu_cfg(const HostPlan& plan, const double* cfg, double* out /*[512]
     const double* cph = wc + P.n_cos;
     const double* sph = cph + P.n_phi;
     const double* wph = sph + P.n_phi;
-    std::fill(acc.begin(), acc.end(), 0.0);
+    // as in the kernel: rows are written by a lane's first direction; only lanes without a direction clear theirs.
+    // NaN everywhere else, so that a row the first direction failed to write cannot go unnoticed
+    std::fill(acc.begin(), acc.end(), NAN);
+    for (int lane = n_dir_of(P); lane < kLanes; ++lane)
+      for (int row = 0; row < L::kStride; ++row) acc16[lane * L::kStride + row] = 0.0;
     const int n_dir = P.n_list > 0 ? P.n_list : P.n_cos * P.n_phi;
     for (int lane = 0; lane < kLanes; ++lane) {
       for (int m = lane; m < n_dir; m += kLanes) {
@@ -64,7 +70,8 @@ static void emu_cfg(const HostPlan& plan, const double* cfg, double* out /*[512]
         First f;
         first_zero(f);
         for (int i = 0; i < P.n_r_pad; i += kNodesPerTrip) trip<NREG>(c.rs, P.n_reg, e2tab, d, rad, ttab.data(), i, f, NREG >= 0 && needs_flush(c));
-        second_level<C4>(f, d, c.gam, w, acc16 + lane * L::kStride);
+        if (m == lane) second_level<C4, false, true>(f, d, c.gam, w, acc16 + lane * L::kStride);   // first direction writes
+        else second_level<C4>(f, d, c.gam, w, acc16 + lane * L::kStride);
       }
     }
     for (int lane = 0; lane < kLanes; ++lane)
