@@ -38,6 +38,8 @@ extern "C" {
                               concurrent call of a non-re-entrant entry point on one handle  */
 #define NO_ERR_CUDA    2   /* CUDA runtime or launch failure; text via no_last_cuda_error() */
 #define NO_ERR_ALLOC   3   /* host or device allocation failed                              */
+#define NO_ERR_LIMIT   4   /* the problem does not fit the fixed capacity of an entry point that never
+                              allocates (no_hf_energy_static); nothing was launched            */
 
 typedef struct no_handle no_handle;   /* opaque; owns its device tables (and host-path scratch) */
 
@@ -168,6 +170,45 @@ int no_eval_diag(const no_handle *h, const double *d_cfg, long long n_cfg, doubl
  * double *e_over_v.  With kF_n = kF_p the four (t1, t2) pair grids coincide and are integrated once.
  * Uses a grow-only device scratch owned by the handle (not re-entrant for one handle, see no_eval_host). */
 int no_hf_energy(no_handle *h, int n_r, int n_cos, int n_phi, double *e_over_v, void *cuda_stream);
+
+/* no_hf_energy for callers that are not allowed to allocate GPU memory.
+ *
+ * Who that is.  The paper drives one GPU from many Monte-Carlo worker threads and MPI ranks at once
+ * (PAPER.md:182-186).  cudaMalloc and cudaFree are device-wide operations: they take the driver's
+ * allocation lock and wait for work in flight, so one worker that allocates stalls the transactions of all
+ * the others, and it does so at a moment nobody chose (no_hf_energy grows its arena whenever a call needs
+ * more than the last one did).  Other callers have no memory left to ask for: a host application that hands
+ * all of HBM to its own pool at start-up (a framework's caching allocator, a fixed-budget service) makes
+ * every later cudaMalloc fail with out-of-memory although the pool has room.  And some code simply runs
+ * under a rule of "no allocation after initialisation" so that it cannot fail or fragment hours into a run.
+ *
+ * What it does.  Same arguments, same result (to rounding: the pair configurations go through the kernels
+ * in passes of 65536 instead of 2^20, so the fixed summation order differs), same synchronisation of
+ * `cuda_stream`, same HOST result pointer as no_hf_energy.  The only difference is where the intermediates
+ * live: not in a handle-owned cudaMalloc arena but in ONE array of NO_HF_STATIC_BYTES (7.25 MiB) that is
+ * compiled into libno3n.so as a `static __device__` variable.  Every GPU on which this process loads the
+ * library carries that array from module load until the process exits, used or not; that is the price.
+ * The call itself performs no cudaMalloc / cudaFree / cudaMallocAsync / cudaHostAlloc, creates no stream or
+ * event and calls no library that could; the handle `h` (whose tables no_init did allocate) must exist already.
+ * On the host it uses a little ordinary heap (the quadrature nodes, 32 bytes per node).
+ *
+ * Limit.  n_r * n_cos * n_phi <= NO_HF_STATIC_MAX_NODES (4096, e.g. 16 x 16 x 16); above that the call
+ * returns NO_ERR_LIMIT before touching the GPU (use no_hf_energy).  The k3 grid of the handle is not limited.
+ *
+ * First call.  The first call on a device looks up where that device keeps the array
+ * (cudaGetSymbolAddress with that device current) and remembers it; make this first call during
+ * start-up, outside any stream capture.  Later calls only enqueue copies, a memset and kernels.
+ *
+ * Sharing.  There is one array per device, not per handle or per call, and it is not cleared between
+ * calls: it holds the previous call's leftovers.  The function zeroes the one accumulator it adds into and
+ * writes everything else before reading it, so a call never sees stale data.  Two calls working in the
+ * array at the same time on one device would corrupt each other; the function therefore takes a per-device
+ * lock for its whole duration (it returns only after its stream has drained), so threads of one process may
+ * call it freely and are served one after the other, whatever handles and streams they use.  Do not defeat
+ * this by other means.  Other processes have their own copy of the array. */
+#define NO_HF_STATIC_MAX_NODES 4096
+#define NO_HF_STATIC_BYTES     7602432
+int no_hf_energy_static(no_handle *h, int n_r, int n_cos, int n_phi, double *e_over_v, void *cuda_stream);
 
 /* 3N part of the Hartree-Fock single-particle energy (self-energy) of Eq. (9), isospin
  * dependent and spin averaged (unpolarised matter):

@@ -90,6 +90,12 @@ class NormalOrdering:
         """no_hf_energy: 3N Hartree-Fock energy per volume (fm^-4) on the given grids for particles 1 and 2."""
         return binding.no_hf_energy(self._h, n_r, n_cos, n_phi, torch.cuda.current_stream(self.device).cuda_stream)
 
+    def hf_energy_static(self, n_r: int, n_cos: int, n_phi: int) -> float:
+        """no_hf_energy_static: hf_energy for callers that must not allocate GPU memory (workers sharing a GPU, hosts
+        whose own pool owns all of HBM): intermediates in the library's fixed device array, n_r n_cos n_phi <= 4096."""
+        return binding.no_hf_energy_static(self._h, n_r, n_cos, n_phi,
+                                           torch.cuda.current_stream(self.device).cuda_stream)
+
     def sp_energy(self, k1, n_r: int, n_cos: int, n_phi: int):
         """no_sp_energy: 3N Hartree-Fock self-energy Sigma[n, 2] (proton, neutron; fm^-1) at momenta k1[n, 3]."""
         return binding.no_sp_energy(self._h, k1, n_r, n_cos, n_phi, torch.cuda.current_stream(self.device).cuda_stream)

@@ -13,11 +13,12 @@ from typing import Optional
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libno3n.so")
 
-NO_OK, NO_ERR_INVALID, NO_ERR_CUDA, NO_ERR_ALLOC = 0, 1, 2, 3
+NO_OK, NO_ERR_INVALID, NO_ERR_CUDA, NO_ERR_ALLOC, NO_ERR_LIMIT = 0, 1, 2, 3, 4
 
 EXPORTS = ("no_init", "no_init_angular", "no_eval", "no_eval_host", "no_eval_diag", "no_hf_energy", "no_sp_energy", "no_set_layout", "no_free", "no_strerror", "no_last_cuda_error",
            "no_kernel_info", "no_evals_per_cfg", "no_probe_fp64_peak",
-           "no_packed_doubles", "no_eval_packed", "no_unpack", "no_eval_host_packed", "no_probe_fp64_operands")
+           "no_packed_doubles", "no_eval_packed", "no_unpack", "no_eval_host_packed", "no_probe_fp64_operands",
+           "no_hf_energy_static")
 
 NO_PACK_CHARGE, NO_PACK_ISOSPIN = 1, 2
 
@@ -60,6 +61,8 @@ def load() -> ctypes.CDLL:
         lib.no_eval_diag.argtypes = [H, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]
         lib.no_hf_energy.argtypes = [H, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double),
                                      ctypes.c_void_p]
+        lib.no_hf_energy_static.argtypes = lib.no_hf_energy.argtypes
+        lib.no_hf_energy_static.restype = ctypes.c_int
         lib.no_sp_energy.argtypes = [H, ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                      ctypes.c_void_p, ctypes.c_void_p]
         lib.no_set_layout.argtypes = [H, ctypes.c_int]
@@ -182,6 +185,16 @@ def no_hf_energy(h, n_r: int, n_cos: int, n_phi: int, stream_ptr: Optional[int] 
     rc = load().no_hf_energy(h, n_r, n_cos, n_phi, ctypes.byref(e), ctypes.c_void_p(stream_ptr or 0))
     if rc != NO_OK:
         raise NoError(rc, "no_hf_energy")
+    return float(e.value)
+
+
+def no_hf_energy_static(h, n_r: int, n_cos: int, n_phi: int, stream_ptr: Optional[int] = None) -> float:
+    """no_hf_energy_static: no_hf_energy without any GPU allocation (intermediates in the library's fixed 7.25 MiB
+    device array; n_r * n_cos * n_phi <= 4096, NO_ERR_LIMIT beyond).  Synchronises the stream."""
+    e = ctypes.c_double(0.0)
+    rc = load().no_hf_energy_static(h, n_r, n_cos, n_phi, ctypes.byref(e), ctypes.c_void_p(stream_ptr or 0))
+    if rc != NO_OK:
+        raise NoError(rc, "no_hf_energy_static")
     return float(e.value)
 
 

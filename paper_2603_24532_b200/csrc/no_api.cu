@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -519,6 +520,7 @@ const char* no_strerror(int code) {
     case NO_ERR_INVALID: return "invalid argument (parameter out of range, null or misaligned pointer, n_cfg < 0)";
     case NO_ERR_CUDA: return "CUDA runtime or launch failure (see no_last_cuda_error)";
     case NO_ERR_ALLOC: return "allocation failed";
+    case NO_ERR_LIMIT: return "problem larger than the fixed, compiled-in capacity of an entry point that never allocates";
     default: return "unknown error code";
   }
 }
@@ -644,3 +646,89 @@ int no_probe_fp64_operands(int device, int millis, double* tflops_two, double* t
 }
 
 }  // extern "C"
+
+
+// ---- no_hf_energy_static: the Hartree-Fock energy for callers that must not allocate --------------------------------
+// no_hf_energy keeps its intermediates (pair grids, generated configurations, weights, traced diagonals, the
+// accumulator) in a handle-owned arena that it cudaMallocs and grows on demand.  The variant below runs the same
+// kernels with the same arguments except that the arena is this fixed array, which is part of the library image:
+// the CUDA runtime places it in the memory of every GPU whose context loads libno3n.so and keeps it until the
+// process exits, whether or not the entry point is ever called.
+namespace {
+
+constexpr long long kStaticMaxNodes = NO_HF_STATIC_MAX_NODES;   // n_r n_cos n_phi of particles 1 and 2
+constexpr long long kStaticChunk = 1LL << 16;                   // pair configurations per pass through the kernels
+constexpr long long kStaticAccSlot = 32;                        // doubles reserved for the accumulator (256 bytes)
+constexpr long long kStaticDoubles = kStaticAccSlot + 8 * kStaticMaxNodes + 14 * kStaticChunk;
+static_assert(kStaticDoubles * 8 == NO_HF_STATIC_BYTES, "include/no.h states the size of the static scratch");
+
+static __device__ __align__(256) double g_hf_static[kStaticDoubles];
+
+// In host code `g_hf_static` names a host-side shadow of the array, NOT memory a kernel can use; the address the
+// kernels need is a per-device fact that cudaGetSymbolAddress reports for the device that is current.  It is
+// looked up once per device (first call on that device) and kept here.  The mutex of a slot also serialises the
+// calls on that device: they all work in the one array, so two of them in flight together would corrupt each other.
+constexpr int kStaticMaxDevices = 64;
+struct StaticSlot {
+  std::mutex mu;
+  double* base = nullptr;
+};
+StaticSlot g_static_slot[kStaticMaxDevices];
+
+}  // namespace
+
+extern "C" int no_hf_energy_static(no_handle* h, int n_r, int n_cos, int n_phi, double* e_over_v, void* cuda_stream) {
+  if (!h || !e_over_v) return NO_ERR_INVALID;
+  if (n_r < 1 || n_r > kMaxOrder || n_cos < 1 || n_cos > kMaxOrder || n_phi < 1 || n_phi > kMaxOrder) return NO_ERR_INVALID;
+  const long long n1 = (long long)n_r * n_cos * n_phi;
+  if (n1 > kStaticMaxNodes) return NO_ERR_LIMIT;                 // the array cannot hold the two pair grids
+  if (h->device < 0 || h->device >= kStaticMaxDevices) return NO_ERR_LIMIT;
+  DeviceGuard guard(h->device);
+  if (!guard.ok) return cuda_fail(cudaGetLastError(), "cudaSetDevice");
+  StaticSlot& slot = g_static_slot[h->device];
+  std::lock_guard<std::mutex> serial(slot.mu);                   // held until this call's stream has drained
+  if (!slot.base) {
+    // set-up, once per device, with that device current (DeviceGuard above)
+    double* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress((void**)&p, g_hf_static);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetSymbolAddress(static HF scratch)");
+    if (!p) return cuda_fail(cudaErrorInvalidSymbol, "cudaGetSymbolAddress(static HF scratch) returned NULL");
+    slot.base = p;
+  }
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  const int layout = h->layout.load(std::memory_order_relaxed) == 2 ? 2 : 1;
+  const double kf[2] = {h->plan.kf_p, h->plan.kf_n};
+  const bool fused = kf[0] > 0 && kf[0] == kf[1];                // as in no_hf_energy: one pair grid serves all four
+  std::vector<double> nodes[2];                                  // host heap only (a few KB of quadrature nodes)
+  for (int t = 0; t < 2; ++t)
+    if (kf[t] > 0 && !(fused && t == 1)) sphere_nodes(n_r, n_cos, n_phi, kf[t], nodes[t]);
+  const long long chunk = n1 * n1 < kStaticChunk ? n1 * n1 : kStaticChunk;
+  double* d_acc = slot.base;
+  double* d_nodes[2] = {slot.base + kStaticAccSlot, fused ? slot.base + kStaticAccSlot : slot.base + kStaticAccSlot + 4 * n1};
+  double *d_cfg = slot.base + kStaticAccSlot + 8 * kStaticMaxNodes, *d_w = d_cfg + 9 * chunk, *d_diag = d_w + chunk;
+  for (int t = 0; t < 2; ++t)
+    if (!nodes[t].empty())
+      NO_CUDA(cudaMemcpyAsync(d_nodes[t], nodes[t].data(), sizeof(double) * 4 * (size_t)n1, cudaMemcpyHostToDevice, s));
+  // the array still holds whatever the previous call left: the accumulator is the one place that is added to
+  // before it is written, so it is cleared here; every other element read below is written first in this call
+  NO_CUDA(cudaMemsetAsync(d_acc, 0, sizeof(double), s));
+  for (int t1 = 0; t1 < 2; ++t1)
+    for (int t2 = 0; t2 < 2; ++t2) {
+      if (!(kf[t1] > 0) || !(kf[t2] > 0)) continue;
+      if (fused && (t1 || t2)) continue;
+      for (long long c0 = 0; c0 < n1 * n1; c0 += chunk) {
+        const long long count = n1 * n1 - c0 < chunk ? n1 * n1 - c0 : chunk;
+        hf_pairs_kernel<<<(unsigned)((count + 255) / 256), 256, 0, s>>>(d_nodes[t1], d_nodes[t2], n1, c0, count, d_cfg, d_w);
+        NO_CUDA(cudaGetLastError());
+        const int rc = launch(h, d_cfg, count, d_diag, s, layout, kModeDiag, true);   // p' = p by construction
+        if (rc != NO_OK) { cudaStreamSynchronize(s); return rc; }
+        hf_reduce_kernel<<<1, 1024, 0, s>>>(d_diag, d_w, count, fused ? -1 : 2 * t1 + t2, d_acc);
+        NO_CUDA(cudaGetLastError());
+      }
+    }
+  double acc = 0.0;
+  NO_CUDA(cudaMemcpyAsync(&acc, d_acc, sizeof(double), cudaMemcpyDeviceToHost, s));
+  NO_CUDA(cudaStreamSynchronize(s));
+  *e_over_v = acc / 6.0;
+  return NO_OK;
+}
