@@ -1,9 +1,11 @@
 #!/usr/bin/env python
-"""Regenerates tests/golden/survey_appendix_a.txt (pin P12): a plain numpy transcription of the
+"""Recomputes the table of tests/golden/survey_appendix_a.txt (pin P12): a plain numpy transcription of the
 level-0 definition of SURVEY.md section 8(c) / DESIGN.md section 1-3.
 
     python tests/golden/make_survey_appendix_a.py            # prints the table
-    python tests/golden/make_survey_appendix_a.py --write    # rewrites survey_appendix_a.txt
+
+It never writes the golden file: the stored values are the survey session's originals and stay byte for byte as
+first committed; this script is checked AGAINST them (tests/test_oracle_pins.py, 1e-13), not the other way round.
 
 It imports nothing from oracle/ or paper_2603_24532_b200/ (numpy only: np.kron for the Pauli-Kronecker
 products, numpy's leggauss for the quadrature rule) and is a THIRD implementation next to the C++ oracle
@@ -150,7 +152,7 @@ HEADER = """# Cross-implementation values for pin P12.
 # Source: /root/repo/SURVEY.md, Appendix A ("cross-implementation values from this session's scratch"):
 # a numpy transcription of the level-0 definition written by the survey's author, independent of
 # oracle/no_oracle.cpp.  NOT from the paper (the paper prints no matrix element, SURVEY.md section 4).
-# Regenerable: tests/golden/make_survey_appendix_a.py (numpy only) reproduces every value below.
+# (recomputed by tests/golden/make_survey_appendix_a.py; the committed file keeps the survey's original digits)
 # Inputs: p=(0.3,-0.2,0.5) p'=(-0.1,0.4,0.2) P=(0.2,0.1,-0.3) fm^-1; kf_p=0.9 kf_n=1.2;
 # c1=-0.81 c3=-3.2 GeV^-1 cD=1.0 cE=-0.5 gA=1.27 fpi=92.4 mpi=138.04 Lchi=700 Lambda=500 MeV n_reg=4;
 # grid 4x4x4; output fm^2; idx = 8 s1 + 4 s2 + 2 t1 + t2, t=0 proton.
@@ -161,11 +163,7 @@ HEADER = """# Cross-implementation values for pin P12.
 def main():
     rows = table()
     text = HEADER + "".join(f"{c4:.1f}  {r:2d} {c:2d}  {re:.15e}  {im:.15e}\n" for c4, r, c, re, im in rows)
-    if "--write" in sys.argv:
-        with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "survey_appendix_a.txt"), "w") as f:
-            f.write(text)
-    else:
-        sys.stdout.write(text)
+    sys.stdout.write(text)
 
 
 if __name__ == "__main__":

@@ -419,8 +419,8 @@ def test_P8_hartree_fock_identity(geo):
 
 
 # ----------------------------------------------------------------------------------------------
-# P12: values of an independent transcription -- a third opinion; regenerable
-# with tests/golden/make_survey_appendix_a.py.
+# P12: values of an independent transcription -- a third opinion.  The stored values are the
+# survey's originals (never regenerated); tests/golden/make_survey_appendix_a.py is checked against them.
 # ----------------------------------------------------------------------------------------------
 def test_P12_cross_implementation_values():
     path = os.path.join(os.path.dirname(__file__), "golden", "survey_appendix_a.txt")
@@ -443,7 +443,7 @@ def test_P12_cross_implementation_values():
 
 def test_P12_golden_file_is_regenerable_by_the_committed_numpy_transcription():
     """tests/golden/make_survey_appendix_a.py (numpy only; imports neither oracle/ nor the product package)
-    reproduces every stored value: the golden file is the output of a committed, independent script."""
+    reproduces every stored value (the survey's original digits) to 1e-13; the script never writes the file."""
     import subprocess
     import sys
     here = os.path.dirname(__file__)
@@ -456,6 +456,7 @@ def test_P12_golden_file_is_regenerable_by_the_committed_numpy_transcription():
         elif isinstance(node, ast.ImportFrom):
             mods.add((node.module or "").split(".")[0])
     assert mods <= {"itertools", "os", "sys", "numpy"}, mods
+    assert "--write" not in open(script).read() and 'open(' not in open(script).read()
     out = subprocess.run([sys.executable, script], check=True, capture_output=True, text=True).stdout
 
     def rows(text):
