@@ -484,6 +484,12 @@ def run_b200(args, workload):
 HF_PARAMS = dict(kf_n=1.33, kf_p=1.33, c1=-0.81, c3=-3.2, c4=0.0, cD=1.0, cE=-0.5, gA=1.27, fpi=92.4, mpi=138.04,
                  lambda_chi=700.0, Lambda=500.0, n_reg=4, n_r=16, n_cos=16, n_phi=16)
 HF_PAIR_GRID = (12, 12, 12)          # particles 1 and 2: 1728 nodes per Fermi sphere, 4 species pairs in SNM
+# Both arms count the SAME unit of work: (pair configurations of ONE pair grid) x (k3 nodes), i.e. what one energy
+# needs once the coinciding isospin pair grids of kF_n = kF_p are integrated once (as no_hf_energy does).  The oracle
+# as it stands loops over all four (t1, t2) grids; that redundancy is its own and is not credited.  Both in f64.
+HF_CPU_EVALS = 8 * 8 * 4096
+HF_CPU_SAMPLE = ("pair grid 2x2x2 per sphere: 64 pair configurations x 16^3 k3 nodes counted per step (the oracle evaluates "
+                 "them once per isospin pair, 4x, uncredited), level-1 oracle in f64")
 
 
 def run_hf(args):
@@ -500,10 +506,10 @@ def run_hf(args):
         O.build()
         t0 = time.perf_counter()
         for _ in range(args.steps):
-            e = O.hf_energy(2, 2, 2, **HF_PARAMS)
+            e = O.hf_energy(2, 2, 2, precision="f64", **HF_PARAMS)
         dt = (time.perf_counter() - t0) / args.steps
-        evals = 4 * 64 * 4096
-        sample = "pair grid 2x2x2 per sphere (256 pair configurations x 16^3 k3 nodes per step), level-1 long double"
+        evals = HF_CPU_EVALS
+        sample = HF_CPU_SAMPLE
         print(json.dumps({"impl": "reference", "metric": METRIC, "value": evals / dt, "unit": UNIT, "n_gpus": args.gpus,
                           "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
                           "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -555,17 +561,18 @@ def run_hf(args):
     t_dev = replicas.max_over_ranks(sum(step_ms) * 1e-3, dev)
     t_wall = replicas.max_over_ranks(sum(wall), dev)
     value = replicas.whole_job_rate(evals_step, args.steps, t_dev)
-    flops = 59.0      # forward fast path (p' = p): 20 DFMA + 12 DMUL + 7 DADD per node
+    # forward fast path (p' = p): 20 DFMA + 12 DMUL + 7 DADD per node = 59 flop (tests/test_sass_flops.py reads the count from the binary)
+    flops = flops_per_eval(HF_PARAMS["n_reg"], HF_PARAMS["Lambda"] > 0, forward=True)
     achieved = flops * evals_step * args.steps / (sum(step_ms) * 1e-3) / 1e12
     probe = binding.no_probe_fp64_peak(local, 200, stream.cuda_stream)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         from oracle import oracle as O
         t0 = time.perf_counter()
-        O.hf_energy(2, 2, 2, **HF_PARAMS)
+        O.hf_energy(2, 2, 2, precision="f64", **HF_PARAMS)
         dt = time.perf_counter() - t0
-        cpu = {"value": 4 * 64 * 4096 / dt, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
-               "sample": f"pair grid 2x2x2 per sphere (256 pair configurations x 16^3 k3 nodes, {dt:.1f} s), level-1 long double"}
+        cpu = {"value": HF_CPU_EVALS / dt, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
+               "sample": f"{HF_CPU_SAMPLE} ({dt:.1f} s)"}
     binding.no_free(h)
     if world > 1:
         torch.distributed.destroy_process_group()
@@ -725,6 +732,7 @@ def run_trace(args):
     bytes_step = n_sample * (n * 4096 + 16)
     peak, peak_src = hbm_peak_gbs()
     achieved = bytes_step * steps / (sum(step_ms) * 1e-3) / 1e9
+    useful_gbs = n_sample * (n * 1536 + 16) * steps / (sum(step_ms) * 1e-3) / 1e9
     # FP64 work actually issued: 8x8x4 tensor-core products (512 flops each) of the 16x16x16 steps + the folded last
     # vertex (256 complex multiply-adds)
     flops_sample = 512.0 * info["tensor_products_per_sample"] + 8.0 * 256
@@ -796,9 +804,17 @@ def run_trace(args):
                    "l2": "256 MiB buffer rewritten between timed steps (L2 flush); the input (3-5 GB) exceeds L2",
                    "parallelism": "replicas only: every rank traces the whole batch"},
         "clocks": clocks, "e2e": e2e, "gpu_launches": steps,
-        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+        # The numerator is the USEFUL bytes: with a charge-conserving plan the method needs only the 96 allowed entries of
+        # a vertex (1536 B), whichever form the caller passes.  The unpacked launch also reads the 160
+        # structural zeros of every matrix; that rate is reported beside it (`hbm_gbs_all_bytes_read`), not as the fraction.
+        "roofline": {"bound": "hbm", "achieved": useful_gbs, "peak": peak, "unit": "GB/s", "frac": useful_gbs / peak,
+                     "limiter": "latency / shared-memory occupancy (8 warps per SM, profiles/r02b.md), not HBM: the packed input "
+                                "moves 2.66x fewer bytes at the same samples/s",
+                     "useful_bytes_per_sample": n * 1536 + 16,
+                     "hbm_gbs_all_bytes_read": achieved, "frac_all_bytes_read": achieved / peak,
                      "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(args.workload), "traffic_source": NCU_DRAM_SOURCE.get(args.workload),
-                     "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_step,
+                     "peak_source": peak_src, "algorithmic_bytes_per_launch": n_sample * (n * 1536 + 16),
+                     "bytes_read_per_launch": bytes_step,
                      "bytes_per_sample": n * 4096 + 16, "kernel": "trace_kernel", "avg_launch_ms": sum(step_ms) / steps,
                      "fp64_tflops": flops_step * steps / (sum(step_ms) * 1e-3) / 1e12,
                      "fp64_frac_of_nominal": flops_step * steps / (sum(step_ms) * 1e-3) / 1e12 / FP64_PEAK_NOMINAL_TFLOPS,
