@@ -34,10 +34,12 @@ extern "C" {
 #endif
 
 #define NO_OK          0
-#define NO_ERR_INVALID 1   /* bad parameter, null pointer, n_cfg < 0, misaligned pointer, or a second
-                              concurrent call of a non-re-entrant entry point on one handle  */
+#define NO_ERR_INVALID 1   /* bad parameter, null pointer, n_cfg < 0, misaligned pointer: a caller bug */
 #define NO_ERR_CUDA    2   /* CUDA runtime or launch failure; text via no_last_cuda_error() */
 #define NO_ERR_ALLOC   3   /* host or device allocation failed                              */
+#define NO_ERR_BUSY    5   /* a second concurrent call of a non-re-entrant entry point (no_eval_host[_packed],
+                              no_hf_energy, no_sp_energy) on ONE handle: returned at once, nothing was
+                              launched, the call may simply be retried (or use one handle per thread)  */
 #define NO_ERR_LIMIT   4   /* the problem does not fit the fixed capacity of an entry point that never
                               allocates (no_hf_energy_static); nothing was launched            */
 
@@ -99,13 +101,20 @@ int no_eval(const no_handle *h, const double *d_cfg, long long n_cfg, double *d_
  * no_hf_energy / no_sp_energy calls. */
 int no_set_layout(no_handle *h, int layout);
 
+/* Test hook, not a tuning parameter: cap the number of CTAs per kernel launch for this handle (0 restores the
+ * hardware limit of 2^31 - 1).  A batch that needs more is cut into several launches on the same stream, with the
+ * same bits as a single launch; the hardware limit itself cannot be reached in a test, so the GPU tests lower it
+ * to drive that path.  Not atomic: call it before the handle is used from other threads.  The library reads no
+ * environment variables. */
+int no_set_max_grid(no_handle *h, long long max_ctas);
+
 /* Same operation with HOST buffers (pageable or pinned): copies h_cfg to a device scratch owned
  * by the handle, runs the kernels, copies the result back and SYNCHRONISES `cuda_stream` before
  * returning.  The batch is cut into chunks of a few waves: the device-to-host copy of a finished chunk
  * runs on an internal stream under the kernel of the next one (pinned h_out is needed for the copies to
  * be asynchronous; pageable memory is still correct).  Not re-entrant for one handle (the scratch is
  * shared): while one of no_eval_host / no_hf_energy / no_sp_energy runs on a handle, a second such call on
- * the same handle returns NO_ERR_INVALID (no_eval / no_eval_diag stay re-entrant).  On a CUDA failure both
+ * the same handle returns NO_ERR_BUSY (no_eval / no_eval_diag stay re-entrant).  On a CUDA failure both
  * streams are drained before the call returns.  Used for the end-to-end measurement. */
 int no_eval_host(no_handle *h, const double *h_cfg, long long n_cfg, double *h_out, void *cuda_stream);
 

@@ -13,12 +13,12 @@ from typing import Optional
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libno3n.so")
 
-NO_OK, NO_ERR_INVALID, NO_ERR_CUDA, NO_ERR_ALLOC, NO_ERR_LIMIT = 0, 1, 2, 3, 4
+NO_OK, NO_ERR_INVALID, NO_ERR_CUDA, NO_ERR_ALLOC, NO_ERR_LIMIT, NO_ERR_BUSY = 0, 1, 2, 3, 4, 5
 
 EXPORTS = ("no_init", "no_init_angular", "no_eval", "no_eval_host", "no_eval_diag", "no_hf_energy", "no_sp_energy", "no_set_layout", "no_free", "no_strerror", "no_last_cuda_error",
            "no_kernel_info", "no_evals_per_cfg", "no_probe_fp64_peak",
            "no_packed_doubles", "no_eval_packed", "no_unpack", "no_eval_host_packed", "no_probe_fp64_operands",
-           "no_hf_energy_static")
+           "no_hf_energy_static", "no_set_max_grid")
 
 NO_PACK_CHARGE, NO_PACK_ISOSPIN = 1, 2
 
@@ -66,6 +66,8 @@ def load() -> ctypes.CDLL:
         lib.no_sp_energy.argtypes = [H, ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                      ctypes.c_void_p, ctypes.c_void_p]
         lib.no_set_layout.argtypes = [H, ctypes.c_int]
+        lib.no_set_max_grid.argtypes = [H, ctypes.c_longlong]
+        lib.no_set_max_grid.restype = ctypes.c_int
         lib.no_packed_doubles.argtypes = [H, ctypes.c_int]
         lib.no_eval_packed.argtypes = [H, ctypes.c_int, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]
         lib.no_unpack.argtypes = [ctypes.c_int, ctypes.c_void_p, ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p]
@@ -208,6 +210,13 @@ def no_sp_energy(h, k1, n_r: int, n_cos: int, n_phi: int, stream_ptr: Optional[i
     if rc != NO_OK:
         raise NoError(rc, "no_sp_energy")
     return out
+
+
+def no_set_max_grid(h, max_ctas: int) -> None:
+    """test hook: cap the CTAs per launch of this handle (0 = hardware limit), include/no.h."""
+    rc = load().no_set_max_grid(h, max_ctas)
+    if rc != NO_OK:
+        raise NoError(rc, "no_set_max_grid")
 
 
 def no_set_layout(h, layout: int) -> None:

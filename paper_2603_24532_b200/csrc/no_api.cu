@@ -94,7 +94,7 @@ struct no_handle {
   std::atomic<int> layout;    // 0 automatic, 1 always one warp per configuration, 2 always one CTA per configuration;
                               // every entry point reads it ONCE per call (no_set_layout may run concurrently)
   std::atomic_flag busy;      // set while an entry point that uses the handle-owned scratch is running
-  long long max_grid;         // CTAs per launch (kMaxGrid; the test knob NO3N_MAX_GRID lowers it)
+  long long max_grid;         // CTAs per launch (kMaxGrid; the test hook no_set_max_grid lowers it)
   long long wave_cfg;         // configurations of one full wave of resident CTAs (chunk granularity of the host path)
   cudaStream_t copy_stream;   // device-to-host copies of finished chunks overlap the next chunk's kernel
   cudaEvent_t ev_chunk[2], ev_copied;
@@ -183,10 +183,7 @@ int no_init_angular(no_handle** out, const no_params* p, const double* h_dirs, i
   h->d_tab = nullptr; h->d_cfg = nullptr; h->d_out = nullptr; h->scratch_cfg = 0; h->scratch_out = 0; h->host_path_ready = false;
   h->layout.store(0); h->busy.clear();
   h->max_grid = kMaxGrid;
-  if (const char* e = getenv("NO3N_MAX_GRID")) {          // testing knob: exercises the multi-launch path at small sizes
-    const long long v = atoll(e);
-    if (v >= 1 && v < kMaxGrid) h->max_grid = v;
-  } h->hf_arena = nullptr; h->hf_arena_doubles = 0;
+  h->hf_arena = nullptr; h->hf_arena_doubles = 0;
   int rc = build_plan(p, h->plan, h_dirs, n_dir);
   if (rc != NO_OK) { delete h; return rc; }
   int n_dev = 0;
@@ -245,6 +242,12 @@ int no_set_layout(no_handle* h, int layout) {
   return NO_OK;
 }
 
+int no_set_max_grid(no_handle* h, long long max_ctas) {
+  if (!h || max_ctas < 0 || max_ctas > kMaxGrid) return NO_ERR_INVALID;
+  h->max_grid = max_ctas == 0 ? kMaxGrid : max_ctas;
+  return NO_OK;
+}
+
 int no_eval_diag(const no_handle* h, const double* d_cfg, long long n_cfg, double* d_out, void* cuda_stream) {
   if (!h || n_cfg < 0) return NO_ERR_INVALID;
   if (n_cfg == 0) return NO_OK;
@@ -259,7 +262,7 @@ int no_hf_energy(no_handle* h, int n_r, int n_cos, int n_phi, double* e_over_v, 
   if (!h || !e_over_v) return NO_ERR_INVALID;
   if (n_r < 1 || n_r > kMaxOrder || n_cos < 1 || n_cos > kMaxOrder || n_phi < 1 || n_phi > kMaxOrder) return NO_ERR_INVALID;
   BusyGuard busy(h);
-  if (!busy.ok) return NO_ERR_INVALID;
+  if (!busy.ok) return NO_ERR_BUSY;
   DeviceGuard guard(h->device);
   if (!guard.ok) return cuda_fail(cudaGetLastError(), "cudaSetDevice");
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
@@ -311,7 +314,7 @@ int no_sp_energy(no_handle* h, const double* h_k1, int n_k, int n_r, int n_cos, 
   if (!h_k1 || !h_sigma) return NO_ERR_INVALID;
   if (n_r < 1 || n_r > kMaxOrder || n_cos < 1 || n_cos > kMaxOrder || n_phi < 1 || n_phi > kMaxOrder) return NO_ERR_INVALID;
   BusyGuard busy(h);
-  if (!busy.ok) return NO_ERR_INVALID;
+  if (!busy.ok) return NO_ERR_BUSY;
   DeviceGuard guard(h->device);
   if (!guard.ok) return cuda_fail(cudaGetLastError(), "cudaSetDevice");
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
@@ -401,7 +404,7 @@ int eval_host_mode(no_handle* h, const double* h_cfg, long long n_cfg, double* h
   if (n_cfg == 0) return NO_OK;
   if (!h_cfg || !h_out) return NO_ERR_INVALID;
   BusyGuard busy(h);
-  if (!busy.ok) return NO_ERR_INVALID;
+  if (!busy.ok) return NO_ERR_BUSY;
   DeviceGuard guard(h->device);
   if (!guard.ok) return cuda_fail(cudaGetLastError(), "cudaSetDevice");
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
@@ -517,9 +520,10 @@ int no_free(no_handle* h) {
 const char* no_strerror(int code) {
   switch (code) {
     case NO_OK: return "success";
-    case NO_ERR_INVALID: return "invalid argument (parameter out of range, null or misaligned pointer, n_cfg < 0)";
+    case NO_ERR_INVALID: return "invalid argument (parameter out of range, null or misaligned pointer, n_cfg < 0, format not applicable)";
     case NO_ERR_CUDA: return "CUDA runtime or launch failure (see no_last_cuda_error)";
     case NO_ERR_ALLOC: return "allocation failed";
+    case NO_ERR_BUSY: return "handle busy: another thread is inside a non-re-entrant entry point on it (retry later; not an argument error)";
     case NO_ERR_LIMIT: return "problem larger than the fixed, compiled-in capacity of an entry point that never allocates";
     default: return "unknown error code";
   }

@@ -412,13 +412,10 @@ int no_trace_init(no_trace_plan** out, int n_vertex, const int* topo, int flags,
   // one CTA per SM, as many warps (samples in flight) as its shared memory holds
   p->stages = kTrStagesDefault;
   p->path = kTrPathDefault;
-  if (const char* e = getenv("NO3N_TRACE_STAGES")) { const int v = atoi(e); if (v == 1 || v == 2) p->stages = v; }   // tuning knobs
-  if (const char* e = getenv("NO3N_TRACE_PATH")) { const int v = atoi(e); if (v == 0 || v == 1) p->path = v; }
   const size_t avail = (size_t)smem_optin - trace_plan_bytes(n_vertex) - 128;
   const int r_bufs = p->plan.n_slice_iter == 1 ? 1 : 2;
   int warps = (int)(avail / trace_warp_bytes(n_vertex, p->stages, r_bufs));
   if (warps > 12) warps = 12;      // __launch_bounds__(384): up to 170 registers per thread, no spills
-  if (const char* e = getenv("NO3N_TRACE_WARPS")) { const int v = atoi(e); if (v >= 1 && v < warps) warps = v; }
   if (warps < 1) { delete p; return NO_ERR_INVALID; }
   p->warps = warps;
   e = cudaFuncSetAttribute((const void*)trace_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin);

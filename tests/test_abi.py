@@ -54,8 +54,9 @@ def test_params_struct_layout_matches_header():
 
 def test_error_strings_and_null_handling(lib):
     assert lib.no_strerror(0) == b"success"
-    for code in (1, 2, 3, 99):
+    for code in (1, 2, 3, 4, 5, 99):
         assert len(lib.no_strerror(code)) > 0
+    assert b"busy" in lib.no_strerror(binding.NO_ERR_BUSY) and b"busy" not in lib.no_strerror(binding.NO_ERR_INVALID)
     assert lib.no_free(None) == binding.NO_OK                      # NULL is a no-op
     assert lib.no_init(None, None) == binding.NO_ERR_INVALID
     assert lib.no_eval(None, None, 0, None, None) == binding.NO_ERR_INVALID

@@ -303,9 +303,9 @@ def test_abi_pointer_checks_streams_and_host_path():
         binding.no_init(device=99, **run.params())
 
 
-def test_batches_larger_than_one_grid_are_cut_into_several_launches(monkeypatch):
+def test_batches_larger_than_one_grid_are_cut_into_several_launches():
     """A batch that needs more CTAs than gridDim.x allows is chunked, not refused.  The limit (2^31 - 1 CTAs)
-    cannot be reached in a test, so the testing knob NO3N_MAX_GRID lowers it: same bits as one launch."""
+    cannot be reached in a test, so the test hook no_set_max_grid lowers it: same bits as one launch."""
     run = W.workload("cfg4").runs[0].shrunk(37, 6)
     cfg = torch.from_numpy(run.configurations()).cuda()
     ref = {}
@@ -314,9 +314,9 @@ def test_batches_larger_than_one_grid_are_cut_into_several_launches(monkeypatch)
         ref[layout] = no(cfg).cpu().numpy()
         ref[layout, "diag"] = no.diag(cfg).cpu().numpy()
         no.close()
-    monkeypatch.setenv("NO3N_MAX_GRID", "3")
     for layout in (1, 2):
         no = NormalOrdering(device=0, layout=layout, **run.params())          # 37 configurations: 7 or 13 launches
+        binding.no_set_max_grid(no._h, 3)
         assert np.array_equal(no(cfg).cpu().numpy(), ref[layout])
         assert np.array_equal(no.diag(cfg).cpu().numpy(), ref[layout, "diag"])
         h_out = np.empty((37, 16, 16, 2))
@@ -341,7 +341,7 @@ def test_host_path_uses_one_layout_per_call_and_refuses_concurrent_use():
     h_out = torch.empty((4000, 16, 16, 2), dtype=torch.float64, pin_memory=True)
     binding.no_eval_host(h, cfg.ctypes.data, 4000, h_out.data_ptr(), None)
     assert torch.equal(h_out, d_out.cpu())                       # tail included: bit-identical to the one-warp layout
-    # two threads on one handle: every call either succeeds with the right bits or is refused with NO_ERR_INVALID
+    # two threads on one handle: every call either succeeds with the right bits or is refused with NO_ERR_BUSY
     lib, results = binding.load(), []
     outs = [torch.empty((4000, 16, 16, 2), dtype=torch.float64, pin_memory=True) for _ in range(2)]
     streams = [torch.cuda.Stream(), torch.cuda.Stream()]
@@ -355,7 +355,7 @@ def test_host_path_uses_one_layout_per_call_and_refuses_concurrent_use():
     th = [threading.Thread(target=work, args=(i,)) for i in range(2)]
     [t.start() for t in th]
     [t.join() for t in th]
-    assert all(rc in (binding.NO_OK, binding.NO_ERR_INVALID) and good for rc, good in results)
+    assert all(rc in (binding.NO_OK, binding.NO_ERR_BUSY) and good for rc, good in results)
     assert any(rc == binding.NO_OK for rc, _ in results)
     binding.no_free(h)
 
