@@ -68,6 +68,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg")
     ap.add_argument("--no-per-config", action="store_true", help="skip the short runs of the other BASELINE configs")
+    ap.add_argument("--no-per-workload", action="store_true",
+                    help="skip the short legs of the section-8(f) workloads (paper quadrature, hf, trace5) on the default line")
     ap.add_argument("--cpu-sample", type=int, default=0, help="configurations in the oracle sample (0 = auto)")
     return ap.parse_args()
 
@@ -456,6 +458,13 @@ def run_b200(args, workload):
             del d2
             torch.cuda.empty_cache()
 
+    # ---- the section-8(f) workloads on the same line: short legs, each the code path of `bench.py --workload X` ----
+    per_workload = None
+    if world == 1 and workload.name == "cfg5" and not args.no_per_workload:
+        del flush
+        torch.cuda.empty_cache()
+        per_workload = per_workload_legs()
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu, _ = time_oracle(workload, args.cpu_sample)
@@ -472,10 +481,57 @@ def run_b200(args, workload):
                        "cfg_per_s": world * workload.n_cfg * args.steps / t_dev,
                        "l2": "256 MiB buffer rewritten between timed steps (L2 flush); the kernel is ALU bound",
                        "parallelism": "replicas only: every rank integrates the whole workload",
-                       "per_config": per_config, "small_transactions": small, "packed_output": packed_dev},
+                       "per_config": per_config, "per_workload": per_workload, "small_transactions": small,
+                       "packed_output": packed_dev},
             "clocks": clocks, "e2e": e2e, "e2e_full_matrices": e2e_full, "gpu_launches": n_launch, "roofline": roofline, "cpu_baseline": cpu,
             "wall_s_timed_region": t_wall}
     print(json.dumps(line), flush=True)
+
+
+def per_workload_legs():
+    """Short legs (3 timed steps after 3 warm-up steps; the trace leg keeps its 20 one-millisecond launches) of the
+    workloads of SURVEY.md 8(f): the paper's quadrature (f2), the Hartree-Fock contraction (f1,
+    PAPER.md:188) and the fifth-order trace with unpacked and packed input (f4).  Each leg IS
+    `bench.py --workload X` (same L2 flush, CUDA-event timing, clock sampling, e2e through the public API), run as a
+    child process on the same GPU after this process has released its buffers, so the default line carries its
+    roofline object, e2e and clocks.  A leg that fails is reported as {"error": ...}; it never fails the line."""
+    legs = {}
+    keep_roofline = ("bound", "achieved", "peak", "unit", "frac", "flops_per_eval", "useful_bytes_per_sample",
+                     "frac_all_bytes_read", "hbm_gbs_all_bytes_read", "limiter", "avg_launch_ms", "kernel",
+                     "peak_measured_dfma_probe", "fp64_tflops")
+    for name in ("paper", "hf", "trace5"):
+        cmd = [sys.executable, os.path.abspath(__file__), "--workload", name, "--steps", "3", "--warmup", "3",
+               "--no-cpu-baseline", "--no-per-config", "--no-per-workload"]
+        t0 = time.perf_counter()
+        try:
+            r = subprocess.run(cmd, capture_output=True, text=True, timeout=900, cwd=ROOT)
+            rows = [l for l in r.stdout.splitlines() if l.startswith("{")]
+            if r.returncode != 0 or not rows:
+                legs[name] = {"error": f"rc {r.returncode}: {r.stderr.strip()[-300:]}"}
+                continue
+            d = json.loads(rows[-1])
+        except (subprocess.TimeoutExpired, OSError, ValueError) as exc:
+            legs[name] = {"error": repr(exc)[:300]}
+            continue
+        rf = d.get("roofline") or {}
+        e2e = d.get("e2e") or {}
+        legs[name] = {"metric": d["metric"], "value": d["value"], "unit": d["unit"], "ms_per_step": d["ms_per_step"],
+                      "steps": d["steps"], "warmup": d["warmup"], "gpu_launches": d["gpu_launches"],
+                      "roofline": {k: rf[k] for k in keep_roofline if k in rf},
+                      "e2e": {k: e2e[k] for k in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "ms_per_step", "api")
+                              if k in e2e},
+                      "clocks": d.get("clocks"), "description": d["config"].get("description"),
+                      "wall_s": time.perf_counter() - t0}
+        if name == "trace5" and "packed_input" in rf:
+            pk, peak = rf["packed_input"], rf["peak"]
+            legs["trace5_packed_input"] = {
+                "metric": d["metric"], "value": pk["samples_per_s"], "unit": d["unit"], "ms_per_step": pk["avg_launch_ms"],
+                "steps": 10, "warmup": 3, "gpu_launches": 10,
+                "roofline": {"bound": "hbm", "achieved": pk["hbm_gbs"], "peak": peak, "unit": "GB/s", "frac": pk["hbm_gbs"] / peak,
+                             "bytes_per_sample": pk["bytes_per_sample"], "avg_launch_ms": pk["avg_launch_ms"],
+                             "kernel": "trace_kernel (no_trace_eval_packed, NO_PACK_CHARGE input)", "limiter": rf.get("limiter")},
+                "e2e": None, "clocks": d.get("clocks"), "description": pk["api"]}
+    return legs
 
 
 # --------------------------------------------------------------------------------------------
