@@ -73,6 +73,8 @@ class NormalOrdering:
         if cfg.is_cuda:
             binding.no_eval_packed(self._h, fmt, cfg.data_ptr(), n, out.data_ptr(), s)
         elif n:
+            if fmt & binding.NO_PACK_FORWARD:
+                raise ValueError("NO_PACK_FORWARD applies to device configurations (no_eval_packed) only")
             binding.no_eval_host_packed(self._h, fmt, cfg.data_ptr(), n, out.data_ptr(), s)
         return torch.view_as_complex(out)
 

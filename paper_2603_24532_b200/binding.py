@@ -21,6 +21,7 @@ EXPORTS = ("no_init", "no_init_angular", "no_eval", "no_eval_host", "no_eval_dia
            "no_hf_energy_static", "no_set_max_grid")
 
 NO_PACK_CHARGE, NO_PACK_ISOSPIN = 1, 2
+NO_PACK_FORWARD = 0x100      # flag ORed into the format of no_eval_packed: every configuration has p' == p (include/no.h)
 
 TRACE_EXPORTS = ("no_trace_init", "no_trace_eval", "no_trace_eval_packed", "no_trace_info", "no_trace_free",
                  "no_trace_last_cuda_error")

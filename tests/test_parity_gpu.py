@@ -604,6 +604,35 @@ def test_packed_output_and_unpack_match_the_oracle(matter, layout):
     no.close()
 
 
+@pytest.mark.parametrize("matter", ["snm", "asym", "pnm"])
+def test_forward_flag_of_the_packed_entry_point_matches_the_oracle(matter):
+    """NO_PACK_FORWARD: configurations with p' = p through the forward kernel in packed mode, against
+    the oracle's packed matrices and against the general kernel on the same configurations; at p' = p the matrix is
+    Hermitian (pin P4), checked on the reconstruction."""
+    kf = {"snm": (1.33, 1.33), "pnm": (1.2, 0.0), "asym": (1.3, 0.9)}[matter]
+    kw = dict(PHYS, c4=5.4 if matter == "asym" else 0.0, kf_n=kf[0], kf_p=kf[1], n_r=6, n_cos=7, n_phi=5)
+    cfg = W.momentum_configurations(13, 0, 41, 2.5, 2.0 * max(kf))
+    cfg[:, 3:6] = cfg[:, 0:3]                                      # forward: p' = p
+    want = O.normal_order(cfg, **kw)
+    d_cfg = torch.from_numpy(cfg).cuda()
+    for layout in (1, 2):
+        no = NormalOrdering(device=0, layout=layout, **kw)
+        for fmt in [binding.NO_PACK_CHARGE] + ([binding.NO_PACK_ISOSPIN] if kf[0] == kf[1] else []):
+            assert binding.no_packed_doubles(no._h, fmt | binding.NO_PACK_FORWARD) == 2 * O.PACKED_COMPLEX[fmt]
+            fwd = no.packed(d_cfg, fmt | binding.NO_PACK_FORWARD)
+            gen = no.packed(d_cfg, fmt)
+            torch.cuda.synchronize()
+            worst = _check_packed(fwd.cpu().numpy(), O.pack(want, fmt), f"{matter} forward packed fmt {fmt} layout {layout}")
+            _check_packed(fwd.cpu().numpy(), gen.cpu().numpy(), f"{matter} forward vs general kernel fmt {fmt}")
+            if layout == 2:
+                assert torch.equal(fwd, gen)                       # small-batch layout: the flag changes nothing
+            M = NormalOrdering.unpack(fwd, fmt).cpu().numpy()
+            mx = np.abs(M).max(axis=(1, 2), keepdims=True)
+            assert (np.abs(M - np.conj(np.swapaxes(M, 1, 2))) <= 1e-12 * mx).all()
+            print(f"{matter} forward fmt {fmt} layout {layout}: max rel err {worst:.2e}")
+        no.close()
+
+
 def test_packed_abi_argument_checks_and_full_size_launch():
     """raw C-ABI calls: bad formats, null / misaligned pointers, n = 0; then the bench-size paper-quadrature launch in
     packed form against the full no_eval launch (every configuration, bit for bit) and sampled against the oracle."""
